@@ -1,0 +1,174 @@
+/* promoe.h — C-ABI of the B200-native ProMoE hot path (expert-offloaded MoE decoder step).
+ *
+ * Paper: arxiv 2410.22134 "ProMoE" (PAPER.md; P:NNN = its line NNN).  The five core calls follow
+ * BASELINE.json `north_star`: promoe_create(model shape, cache_slots, stride), promoe_load_experts(host
+ * ptrs), promoe_prefill, promoe_decode, promoe_stats.  The remaining calls hand over the always-resident
+ * non-expert parameters ("non-expert parameters are always kept on the GPU"), expose traces for
+ * parity tests, and micro-entry points for single hot-path steps.
+ *
+ * Conventions
+ *  - every call returns 0 (PROMOE_OK) or a negative PROMOE_E* code; no exception or abort crosses the ABI;
+ *    promoe_last_error() returns a static/handle-owned message for the last failing call.
+ *  - one handle = one model instance on the CUDA device that is current at promoe_create; calls on one
+ *    handle are not thread-safe.
+ *  - "device ptr" = CUDA device memory, "host ptr" = ordinary host memory, "pinned host ptr" = page-locked
+ *    host memory (the library cudaHostRegister()s unpinned expert buffers and counts that in the stats).
+ *  - borrowed pointers (dense weights, expert host images) must outlive the handle; the library owns the
+ *    slot region (ONE contiguous allocation), KV cache, traces, streams and events.
+ *  - weights are row-major [out_features, in_features]; bf16 (wdtype 1) or fp32 (wdtype 0); all
+ *    activations, the KV cache and accumulators are fp32 (reading G1).
+ */
+#ifndef PROMOE_H
+#define PROMOE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PROMOE_OK 0
+#define PROMOE_EINVAL (-1)   /* bad argument / unsupported shape */
+#define PROMOE_ENOMEM (-2)   /* device or host allocation failed */
+#define PROMOE_ECUDA (-3)    /* a CUDA call or kernel failed; see promoe_last_error */
+#define PROMOE_ESTATE (-4)   /* call out of order (e.g. decode before load) or sequence overflow */
+#define PROMOE_ETIMEOUT (-5) /* an expert kernel gave up waiting for a chunk-ready flag */
+
+typedef struct promoe promoe_t;
+
+/* "model shape" (BASELINE.json configs; Table 1 P:39-48 names the families). */
+typedef struct {
+  int32_t n_layers, hidden, n_q_heads, n_kv_heads, head_dim, vocab, max_seq;
+  int32_t n_experts, top_k, expert_inter;
+  int32_t n_shared_inter;  /* 0 = no shared expert; c2 5632; c3 2816 (two always-on experts = one MLP) */
+  int32_t shared_gate;     /* 1 = sigmoid scalar gate on the shared expert (c2) */
+  int32_t n_dense_layers;  /* leading layers with a dense FFN (c3: 1) */
+  int32_t dense_inter;
+  int32_t router_bias;     /* 1 = per-expert logit bias (c3) */
+  int32_t pred_hidden;     /* predictor MLP hidden width ("2-layer MLP") */
+  int32_t wdtype;          /* 0 fp32 (c1), 1 bf16 */
+  float rope_theta, rms_eps;
+} promoe_shape_t;
+
+/* predictor_mode */
+#define PROMOE_PRED_NONE 0   /* reactive cache, no prefetch (BASELINE.json config 5 baseline) */
+#define PROMOE_PRED_MLP 1    /* learned stride predictor */
+#define PROMOE_PRED_TRACE 2  /* injected prediction lists (oracle-routing upper bound) */
+/* flags */
+#define PROMOE_F_PREEMPT 1   /* early preemption: drop un-issued LOW chunks of a layer at its gate */
+#define PROMOE_F_REORDER 2   /* reordered inference: cached -> being prefetched -> missing */
+#define PROMOE_F_WARM 4      /* warm start: experts 0..C-1 resident in every layer (G4) */
+#define PROMOE_F_TRACE 8     /* record routing / permutation / cache traces for promoe_get_trace */
+#define PROMOE_F_TENSOR 16   /* prefill GEMMs on tcgen05 tensor cores (bf16 weights only); else SIMT fp32 */
+
+typedef struct {
+  int32_t cache_slots;     /* TOTAL slots; per MoE layer = cache_slots / n_moe_layers (must divide), G14 */
+  int32_t stride;          /* predictor at MoE layer m targets MoE layer m+stride; >= 1 */
+  uint64_t chunk_bytes;    /* H2D chunk size; 0 = library default (measured curve) */
+  int32_t predictor_mode;
+  int32_t flags;
+  int32_t max_inflight;    /* chunks kept in flight on the copy stream (P:191 bounded delay); 0 = default 2 */
+  int32_t reserved;
+  void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
+} promoe_opts_t;
+
+/* Device pointers to the always-resident parameters.  Per-layer arrays are HOST arrays of n_layers DEVICE
+ * pointers (entries for layers that lack the tensor are NULL).  Norm gains and router bias are fp32; every
+ * other tensor has the model's wdtype. */
+typedef struct {
+  const void* emb;         /* [vocab, hidden] */
+  const void* lm_head;     /* [vocab, hidden] */
+  const float* final_norm; /* [hidden] */
+  const float* const* ln1; /* [hidden] pre-attention RMSNorm gain */
+  const float* const* ln2; /* [hidden] pre-FFN RMSNorm gain */
+  const void* const* wqkv; /* [(nq+2nkv)*d, hidden], rows: q heads | k heads | v heads */
+  const void* const* wo;   /* [hidden, nq*d] */
+  const void* const* router;        /* [E, hidden]  (MoE layers) */
+  const float* const* router_bias;  /* [E] or NULL */
+  const void* const* pred_w1;       /* [pred_hidden, hidden] (MoE layers) */
+  const void* const* pred_w2;       /* [E, pred_hidden] */
+  const void* const* ffn_gate;      /* shared expert (MoE layers) or dense FFN (dense layers): [I', hidden] */
+  const void* const* ffn_up;        /* [I', hidden] */
+  const void* const* ffn_down;      /* [hidden, I'] */
+  const void* const* shared_gate_w; /* [1, hidden] or NULL */
+} promoe_dense_t;
+
+/* Cumulative since create / reset.  Logical counters follow DESIGN.md "logical-time cache"; physical
+ * ones are measured on the copy stream. */
+typedef struct {
+  uint64_t steps, tokens;
+  uint64_t accesses, hits_resident, hits_prefetch, misses;   /* class A / B / C at the gate */
+  uint64_t evictions, predicted, predicted_correct, pred_allocs;
+  uint64_t need_experts;        /* sum |needed \ resident at step start| (B_need / expert_bytes) */
+  uint64_t chunks_issued, chunks_cancelled, chunks_high, chunks_low;
+  uint64_t h2d_bytes;           /* bytes physically copied */
+  uint64_t fetched_at_gate, fetched_at_gate_of;  /* FetchRate numerator / denominator */
+  uint64_t registered_host_bytes; /* expert host bytes the library had to cudaHostRegister */
+  double copy_busy_ms;          /* copy-stream busy time, from per-chunk events */
+  double step_ms;               /* sum of step times (compute-stream events) */
+  double last_step_ms;
+  int32_t timeouts;             /* kernels that gave up on a ready flag */
+  int32_t reserved;
+} promoe_stats_t;
+
+/* trace kinds for promoe_get_trace (valid until the next step call; library-owned HOST memory) */
+#define PROMOE_TRACE_SEL 0       /* int32 [n_moe, T, k]   selected experts, descending logit */
+#define PROMOE_TRACE_GATES 1     /* float [n_moe, T, k]   renormalised gate weights */
+#define PROMOE_TRACE_MARGIN 2    /* float [n_moe, T]      z_(k) - z_(k+1) */
+#define PROMOE_TRACE_PERM 3      /* int32 [n_moe, E + (E+1) + 2*T*k]  count | offset | perm | inv */
+#define PROMOE_TRACE_PRECISE 4   /* int32 [n_moe, 1 + 5*E]  n, then (expert, class, slot, victim, dep) in launch order */
+#define PROMOE_TRACE_PRED 5      /* int32 [n_moe, 1 + 4*E]  n, then (expert, action, slot, victim) in listed order; row m = push INTO layer m */
+#define PROMOE_TRACE_HIDDEN 6    /* float [T, hidden]     residual stream after the full stack */
+#define PROMOE_TRACE_PREDLIST 7  /* int32 [n_moe, 1 + E]  n, list predicted BY the predictor at layer m (uncapped by G5) */
+#define PROMOE_TRACE_ZLOGITS 8   /* float [n_moe, T, E]   router logits */
+
+int promoe_create(const promoe_shape_t* shape, const promoe_opts_t* opts, promoe_t** out);
+void promoe_destroy(promoe_t* h);
+const char* promoe_last_error(const promoe_t* h); /* h may be NULL: last create error */
+
+/* Hand over the non-expert parameters (device pointers, borrowed). */
+int promoe_load_dense(promoe_t* h, const promoe_dense_t* w);
+
+/* host_ptrs[m*E + e] = host image of routed expert e of MoE layer m: [Wgate (I x H) | Wup (I x H) | Wdown
+ * (H x I)] contiguous, expert_bytes = 3*H*I*sizeof(w) (three linears).  Borrowed until destroy.
+ * With PROMOE_F_WARM the first C experts of every layer are copied into their slots here. */
+int promoe_load_experts(promoe_t* h, const void* const* host_ptrs, size_t expert_bytes);
+
+/* Prefill: ids_host = host ptr to n_tokens int32 ids; positions continue from the current sequence length.
+ * logits_out = HOST ptr to vocab floats (last token) or NULL.  Synchronous: returns when logits are valid. */
+int promoe_prefill(promoe_t* h, const int32_t* ids_host, int32_t n_tokens, float* logits_out);
+/* Decode one token (caller samples; tests teacher-force).  logits_out as above. */
+int promoe_decode(promoe_t* h, int32_t token_id, float* logits_out);
+
+/* predictor_mode TRACE: lists for the NEXT step call; pred[m*(1+E)] = n, then n expert ids = the list the
+ * predictor at MoE layer m would emit for layer m+stride.  Host ptr, copied. */
+int promoe_set_prediction_trace(promoe_t* h, const int32_t* pred, size_t n_int32);
+
+int promoe_stats(promoe_t* h, promoe_stats_t* out);
+int promoe_get_trace(promoe_t* h, int which, const void** data, size_t* bytes);
+int promoe_reset(promoe_t* h);   /* clears KV cache, cache state (re-warms if F_WARM) and stats */
+
+/* Current logical slot table of MoE layer m: slot_expert_out = host ptr to C int32 (-1 = empty). */
+int promoe_get_slots(promoe_t* h, int32_t moe_layer, int32_t* slot_expert_out);
+
+/* Measured pinned host->device bandwidth (GB/s) for `bytes`-sized copies at queue depth `depth`
+ * (chunk size is chosen from this curve).  Allocates and frees its own buffers. */
+int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out);
+
+/* Micro entry points: single hot-path steps on caller-provided DEVICE buffers (used by kernel-level parity
+ * tests and bench.py's per-kernel roofline).  stream = cudaStream_t or NULL (default stream).
+ * All are asynchronous on `stream`. */
+/* y[T,N] = x[T,K] . W[N,K]^T ; x,y fp32; W wdtype (0 fp32 / 1 bf16). path: 0 auto, 1 gemv, 2 simt gemm, 3 tcgen05 */
+int promoe_op_linear(const float* x, const void* w, float* y, int32_t T, int32_t N, int32_t K, int32_t wdtype,
+                     int32_t path, void* stream);
+/* router row A4: z = u.R^T (+b); top-k (ties -> lower index); gates = softmax over selected. */
+int promoe_op_route(const float* u, const void* router, const float* bias, int32_t T, int32_t H, int32_t E,
+                    int32_t k, int32_t wdtype, float* z_out, int32_t* sel_out, float* gates_out,
+                    float* margin_out, void* stream);
+/* permutation row A8: sel [T,k] -> count[E], offset[E+1], perm[T*k], inv[T*k] */
+int promoe_op_permute(const int32_t* sel, int32_t T, int32_t k, int32_t E, int32_t* count, int32_t* offset,
+                      int32_t* perm, int32_t* inv, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PROMOE_H */

@@ -1,0 +1,129 @@
+// common.cuh — device helpers shared by the ProMoE sm_100a kernels (product code; shares nothing with oracle/).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace promoe {
+
+constexpr int kWarp = 32;
+
+// ---- 16-byte vectorised weight loads, widened exactly to fp32 (weights are bf16 or fp32; G1) -------------
+template <typename WT> struct WVec;
+template <> struct WVec<float> {
+  static constexpr int N = 4;  // elements per 16-byte load
+  __device__ __forceinline__ static void load(const float* p, float (&v)[4]) {
+    float4 r = __ldcs(reinterpret_cast<const float4*>(p));
+    v[0] = r.x; v[1] = r.y; v[2] = r.z; v[3] = r.w;
+  }
+};
+template <> struct WVec<__nv_bfloat16> {
+  static constexpr int N = 8;
+  __device__ __forceinline__ static void load(const __nv_bfloat16* p, float (&v)[8]) {
+    uint4 r = __ldcs(reinterpret_cast<const uint4*>(p));
+    // bf16 -> fp32 is a 16-bit shift
+    v[0] = __uint_as_float(r.x << 16); v[1] = __uint_as_float(r.x & 0xffff0000u);
+    v[2] = __uint_as_float(r.y << 16); v[3] = __uint_as_float(r.y & 0xffff0000u);
+    v[4] = __uint_as_float(r.z << 16); v[5] = __uint_as_float(r.z & 0xffff0000u);
+    v[6] = __uint_as_float(r.w << 16); v[7] = __uint_as_float(r.w & 0xffff0000u);
+  }
+};
+__device__ __forceinline__ float wload1(const float* p) { return *p; }
+__device__ __forceinline__ float wload1(const __nv_bfloat16* p) { return __bfloat162float(*p); }
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float silu(float a) { return a / (1.0f + expf(-a)); }
+
+// ---- one weight row · x, fp32 accumulate: the HBM-streaming inner loop of every decode GEMV -------------------
+// K must be a multiple of the 16-byte vector width; the summation order depends on (K, lane) only, so results
+// are bit-identical wherever the row lives (slot, shared expert, any launch order).
+template <typename WT>
+__device__ __forceinline__ float row_dot(const WT* __restrict__ wrow, const float* __restrict__ x, int K, int lane) {
+  constexpr int V = WVec<WT>::N;
+  constexpr int UNR = 4;
+  float acc[UNR] = {0.f, 0.f, 0.f, 0.f};
+  int k = lane * V;
+  const int step = 32 * V;
+  for (; k + (UNR - 1) * step + V <= K; k += UNR * step) {
+    float wv[UNR][V];
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) WVec<WT>::load(wrow + k + u * step, wv[u]);
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) {
+      const float4* xp = reinterpret_cast<const float4*>(x + k + u * step);
+#pragma unroll
+      for (int q = 0; q < V / 4; ++q) {
+        float4 xv = __ldg(xp + q);
+        acc[u] = fmaf(wv[u][4 * q + 0], xv.x, acc[u]);
+        acc[u] = fmaf(wv[u][4 * q + 1], xv.y, acc[u]);
+        acc[u] = fmaf(wv[u][4 * q + 2], xv.z, acc[u]);
+        acc[u] = fmaf(wv[u][4 * q + 3], xv.w, acc[u]);
+      }
+    }
+  }
+  for (; k + V <= K; k += step) {
+    float wv[V];
+    WVec<WT>::load(wrow + k, wv);
+#pragma unroll
+    for (int q = 0; q < V; ++q) acc[0] = fmaf(wv[q], __ldg(x + k + q), acc[0]);
+  }
+  return warp_sum((acc[0] + acc[1]) + (acc[2] + acc[3]));
+}
+
+
+// ---- chunk-ready flags (Alg. 1 l.10 `ready_chunk`) --------------------------------------
+// flag[c] holds the allocation generation whose chunk c has landed in this slot.  Written by the copy stream
+// (DMA), read here with a system-scope acquire load.
+__device__ __forceinline__ unsigned ld_acquire_sys(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+constexpr unsigned long long kFlagTimeoutNs = 4000000000ull;  // 4 s: then give up and raise the error word
+
+// One thread waits until flags[c0..c1] == gen.  Returns false on timeout (error word set).
+__device__ inline bool wait_chunks(const unsigned* flags, int c0, int c1, unsigned gen, int* err) {
+  if (flags == nullptr) return true;
+  unsigned long long t0 = 0;
+  for (int c = c0; c <= c1; ++c) {
+    while (ld_acquire_sys(flags + c) != gen) {
+      if (t0 == 0) t0 = globaltimer_ns();
+      if (globaltimer_ns() - t0 > kFlagTimeoutNs || *reinterpret_cast<volatile int*>(err) != 0) {
+        atomicExch(err, 1);
+        return false;
+      }
+      __nanosleep(256);
+    }
+  }
+  return true;
+}
+
+// One FFN problem = one SwiGLU MLP applied to a row range.  Routed experts: written
+// by the slot-table kernel; shared/dense FFNs: written once at load time.
+struct FfnProblem {
+  const void* wg;          // [inter, H]
+  const void* wu;          // [inter, H]
+  const void* wd;          // [H, inter]
+  const unsigned* flags;   // chunk flags of the slot, or nullptr (always resident)
+  unsigned gen;            // generation the flags must show
+  int inter;
+  int row0, nrows;         // rows of the (permuted) activation matrix this problem covers
+  int expert;              // routed expert id, or -1
+  int pad;
+};
+
+}  // namespace promoe

@@ -1,0 +1,258 @@
+// kernels_attn.cu — RoPE + KV append (A2), decode attention (A3, split over positions) and causal prefill
+// attention (A3, fp32 flash-style SIMT).  All fp32: the KV cache stays fp32 (reading G1).
+#include "kernels.h"
+
+namespace promoe {
+
+// ---------------------------------------------------------------------------------------------------------
+// A2: rotate-half RoPE on q and k heads in place, then append k, v to the cache.
+// grid (T, nq + nkv), block d/2 threads: thread i handles the pair (i, i + d/2) of one head.
+__global__ void rope_append_kernel(float* __restrict__ qkv, const float* __restrict__ cos_t,
+                                   const float* __restrict__ sin_t, float* __restrict__ kcache,
+                                   float* __restrict__ vcache, int pos0, int nq, int nkv, int d, int max_seq) {
+  const int t = blockIdx.x, hh = blockIdx.y, i = threadIdx.x, half = d >> 1;
+  const int pos = pos0 + t;
+  float* row = qkv + (size_t)t * (nq + 2 * nkv) * d;
+  const float c = cos_t[(size_t)pos * half + i], s = sin_t[(size_t)pos * half + i];
+  float* p = row + (size_t)hh * d;           // q heads then k heads are contiguous
+  const float x1 = p[i], x2 = p[i + half];
+  const float r1 = x1 * c - x2 * s, r2 = x2 * c + x1 * s;
+  p[i] = r1; p[i + half] = r2;
+  if (hh >= nq) {
+    const int g = hh - nq;
+    float* kd = kcache + ((size_t)g * max_seq + pos) * d;
+    kd[i] = r1; kd[i + half] = r2;
+    const float* v = row + (size_t)(nq + nkv + g) * d;
+    float* vd = vcache + ((size_t)g * max_seq + pos) * d;
+    vd[i] = v[i]; vd[i + half] = v[i + half];
+  }
+}
+void launch_rope_append(float* qkv, const float* cos_t, const float* sin_t, float* kcache, float* vcache, int T,
+                        int pos0, int nq, int nkv, int d, int max_seq, cudaStream_t st) {
+  rope_append_kernel<<<dim3(T, nq + nkv), d / 2, 0, st>>>(qkv, cos_t, sin_t, kcache, vcache, pos0, nq, nkv, d,
+                                                         max_seq);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// A3 decode: one query token.  grid (nq, nsplit), 128 threads.  8 lanes share a key (each owns d/8
+// contiguous floats, float4 loads → a warp reads 4 whole key rows, 2 KB coalesced); online softmax per
+// 8-lane group; groups are merged through shared memory, splits through the workspace + a second kernel.
+template <int D>
+__global__ void __launch_bounds__(128) attn_decode_kernel(const float* __restrict__ qkv,
+                                                          const float* __restrict__ kcache,
+                                                          const float* __restrict__ vcache, float* __restrict__ ws,
+                                                          int n_pos, int nq, int nkv, int max_seq, int nsplit) {
+  constexpr int PER = D / 8;                 // floats per lane
+  const int h = blockIdx.x, sp = blockIdx.y;
+  const int g = h / (nq / nkv);
+  const int sub = threadIdx.x & 7;           // lane within the 8-lane key group
+  const int grp = threadIdx.x >> 3;          // 0..15 key groups in the CTA
+  const float scale = rsqrtf((float)D);
+  float q[PER];
+#pragma unroll
+  for (int i = 0; i < PER; ++i) q[i] = qkv[(size_t)h * D + sub * PER + i] * scale;
+  const int per_split = (n_pos + nsplit - 1) / nsplit;
+  const int p0 = sp * per_split, p1 = min(n_pos, p0 + per_split);
+  const float* kb = kcache + (size_t)g * max_seq * D;
+  const float* vb = vcache + (size_t)g * max_seq * D;
+  float m = -INFINITY, l = 0.f, o[PER];
+#pragma unroll
+  for (int i = 0; i < PER; ++i) o[i] = 0.f;
+  for (int p = p0 + grp; p < p1; p += 16) {
+    const float4* kr = reinterpret_cast<const float4*>(kb + (size_t)p * D + sub * PER);
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < PER / 4; ++i) {
+      float4 kv = __ldcs(kr + i);
+      s = fmaf(q[4 * i], kv.x, s); s = fmaf(q[4 * i + 1], kv.y, s);
+      s = fmaf(q[4 * i + 2], kv.z, s); s = fmaf(q[4 * i + 3], kv.w, s);
+    }
+    s += __shfl_xor_sync(0xffffffffu, s, 1);
+    s += __shfl_xor_sync(0xffffffffu, s, 2);
+    s += __shfl_xor_sync(0xffffffffu, s, 4);
+    const float mn = fmaxf(m, s);
+    const float corr = expf(m - mn), pw = expf(s - mn);
+    l = l * corr + pw;
+    const float4* vr = reinterpret_cast<const float4*>(vb + (size_t)p * D + sub * PER);
+#pragma unroll
+    for (int i = 0; i < PER / 4; ++i) {
+      float4 vv = __ldcs(vr + i);
+      o[4 * i] = o[4 * i] * corr + pw * vv.x; o[4 * i + 1] = o[4 * i + 1] * corr + pw * vv.y;
+      o[4 * i + 2] = o[4 * i + 2] * corr + pw * vv.z; o[4 * i + 3] = o[4 * i + 3] * corr + pw * vv.w;
+    }
+    m = mn;
+  }
+  // merge the 16 key groups (fixed order → deterministic)
+  __shared__ float sm_m[16], sm_l[16], sm_o[16][D];
+  if (sub == 0) { sm_m[grp] = m; sm_l[grp] = l; }
+#pragma unroll
+  for (int i = 0; i < PER; ++i) sm_o[grp][sub * PER + i] = o[i];
+  __syncthreads();
+  float M = -INFINITY;
+  for (int i = 0; i < 16; ++i) M = fmaxf(M, sm_m[i]);
+  float* out = ws + ((size_t)h * nsplit + sp) * (D + 2);
+  for (int c = threadIdx.x; c < D; c += 128) {
+    float acc = 0.f;
+    for (int i = 0; i < 16; ++i) if (sm_m[i] != -INFINITY) acc += sm_o[i][c] * expf(sm_m[i] - M);
+    out[c] = acc;
+  }
+  if (threadIdx.x == 0) {
+    float L = 0.f;
+    for (int i = 0; i < 16; ++i) if (sm_m[i] != -INFINITY) L += sm_l[i] * expf(sm_m[i] - M);
+    out[D] = M; out[D + 1] = L;
+  }
+}
+__global__ void attn_decode_merge_kernel(const float* __restrict__ ws, float* __restrict__ out, int d, int nsplit) {
+  const int h = blockIdx.x;
+  const float* base = ws + (size_t)h * nsplit * (d + 2);
+  float M = -INFINITY;
+  for (int s = 0; s < nsplit; ++s) M = fmaxf(M, base[(size_t)s * (d + 2) + d]);
+  float L = 0.f;
+  for (int s = 0; s < nsplit; ++s) {
+    const float ms = base[(size_t)s * (d + 2) + d];
+    if (ms != -INFINITY) L += base[(size_t)s * (d + 2) + d + 1] * expf(ms - M);
+  }
+  for (int c = threadIdx.x; c < d; c += blockDim.x) {
+    float acc = 0.f;
+    for (int s = 0; s < nsplit; ++s) {
+      const float ms = base[(size_t)s * (d + 2) + d];
+      if (ms != -INFINITY) acc += base[(size_t)s * (d + 2) + c] * expf(ms - M);
+    }
+    out[(size_t)h * d + c] = acc / L;
+  }
+}
+void launch_attn_decode(const float* qkv, const float* kcache, const float* vcache, float* out, float* ws,
+                        int n_pos, int nq, int nkv, int d, int max_seq, int nsplit, cudaStream_t st) {
+  dim3 grid(nq, nsplit);
+  if (d == 128) attn_decode_kernel<128><<<grid, 128, 0, st>>>(qkv, kcache, vcache, ws, n_pos, nq, nkv, max_seq, nsplit);
+  else attn_decode_kernel<64><<<grid, 128, 0, st>>>(qkv, kcache, vcache, ws, n_pos, nq, nkv, max_seq, nsplit);
+  attn_decode_merge_kernel<<<nq, 128, 0, st>>>(ws, out, d, nsplit);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// A3 prefill: causal flash attention in fp32.  grid (ceil(T/64), nq), 256 threads; 64 queries x 64 keys per
+// tile; S = Q.K^T and O += P.V on CUDA cores (≤ 3 % of a prefill step); online softmax.
+template <int D>
+__global__ void __launch_bounds__(256) attn_prefill_kernel(const float* __restrict__ qkv,
+                                                           const float* __restrict__ kcache,
+                                                           const float* __restrict__ vcache, float* __restrict__ out,
+                                                           int T, int pos0, int nq, int nkv, int max_seq) {
+  constexpr int BM = 64, BN = 64, LD = BM + 4, OC = D / 16;   // OC output columns per thread
+  extern __shared__ float smem[];
+  float* Qt = smem;                 // [D][LD]   Q transposed (pre-scaled)
+  float* Kt = Qt + D * LD;          // [D][LD]   K tile transposed
+  float* Vs = Kt + D * LD;          // [BN][D]
+  float* Ss = Vs + BN * D;          // [BM][LD]  probabilities
+  const int h = blockIdx.y, g = h / (nq / nkv), m0 = blockIdx.x * BM;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  const int qstride = (nq + 2 * nkv) * D;
+  const float scale = rsqrtf((float)D);
+  for (int idx = threadIdx.x; idx < BM * D; idx += 256) {
+    const int r = idx / D, c = idx % D;
+    const int t = m0 + r;
+    Qt[c * LD + r] = (t < T) ? qkv[(size_t)t * qstride + (size_t)h * D + c] * scale : 0.f;
+  }
+  float o[4][OC], mrow[4], lrow[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    mrow[i] = -INFINITY; lrow[i] = 0.f;
+#pragma unroll
+    for (int c = 0; c < OC; ++c) o[i][c] = 0.f;
+  }
+  const float* kb = kcache + (size_t)g * max_seq * D;
+  const float* vb = vcache + (size_t)g * max_seq * D;
+  const int last_q = min(T, m0 + BM) - 1;
+  const int n_keys = pos0 + last_q + 1;           // keys 0..pos0+last_q
+  for (int n0 = 0; n0 < n_keys; n0 += BN) {
+    __syncthreads();                              // previous tile fully consumed (and Qt written)
+    for (int idx = threadIdx.x; idx < BN * D; idx += 256) {
+      const int r = idx / D, c = idx % D;
+      const int p = n0 + r;
+      const bool ok = p < n_keys;
+      Kt[c * LD + r] = ok ? kb[(size_t)p * D + c] : 0.f;
+      Vs[r * D + c] = ok ? vb[(size_t)p * D + c] : 0.f;
+    }
+    __syncthreads();
+    float s[4][4] = {};
+#pragma unroll 8
+    for (int kk = 0; kk < D; ++kk) {
+      const float4 a = *reinterpret_cast<const float4*>(Qt + kk * LD + ty * 4);
+      const float4 b = *reinterpret_cast<const float4*>(Kt + kk * LD + tx * 4);
+      const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) s[i][j] = fmaf(av[i], bv[j], s[i][j]);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int qpos = pos0 + m0 + ty * 4 + i;
+      float mx = -INFINITY;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int p = n0 + tx * 4 + j;
+        if (p > qpos || p >= n_keys) s[i][j] = -INFINITY;
+        mx = fmaxf(mx, s[i][j]);
+      }
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
+      const float mn = fmaxf(mrow[i], mx);
+      const float corr = (mn == -INFINITY) ? 1.f : expf(mrow[i] - mn);
+      float sum = 0.f;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float pw = (s[i][j] == -INFINITY) ? 0.f : expf(s[i][j] - mn);
+        Ss[(ty * 4 + i) * LD + tx * 4 + j] = pw;
+        sum += pw;
+      }
+      sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+      sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+      sum += __shfl_xor_sync(0xffffffffu, sum, 4);
+      sum += __shfl_xor_sync(0xffffffffu, sum, 8);
+      lrow[i] = lrow[i] * corr + sum;
+      mrow[i] = mn;
+#pragma unroll
+      for (int c = 0; c < OC; ++c) o[i][c] *= corr;
+    }
+    __syncthreads();
+#pragma unroll 4
+    for (int n = 0; n < BN; ++n) {
+      float vv[OC];
+#pragma unroll
+      for (int c4 = 0; c4 < OC / 4; ++c4) {
+        const float4 v4 = *reinterpret_cast<const float4*>(Vs + n * D + tx * OC + c4 * 4);
+        vv[c4 * 4] = v4.x; vv[c4 * 4 + 1] = v4.y; vv[c4 * 4 + 2] = v4.z; vv[c4 * 4 + 3] = v4.w;
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float pw = Ss[(ty * 4 + i) * LD + n];
+#pragma unroll
+        for (int c = 0; c < OC; ++c) o[i][c] = fmaf(pw, vv[c], o[i][c]);
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int t = m0 + ty * 4 + i;
+    if (t >= T) continue;
+    const float inv = 1.f / lrow[i];
+#pragma unroll
+    for (int c = 0; c < OC; ++c) out[(size_t)t * nq * D + (size_t)h * D + tx * OC + c] = o[i][c] * inv;
+  }
+}
+void launch_attn_prefill(const float* qkv, const float* kcache, const float* vcache, float* out, int T, int pos0,
+                         int nq, int nkv, int d, int max_seq, cudaStream_t st) {
+  dim3 grid((T + 63) / 64, nq);
+  const size_t smem = (size_t)(2 * d * 68 + 64 * d + 64 * 68) * sizeof(float);
+  if (d == 128) {
+    cudaFuncSetAttribute(attn_prefill_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attn_prefill_kernel<128><<<grid, 256, smem, st>>>(qkv, kcache, vcache, out, T, pos0, nq, nkv, max_seq);
+  } else {
+    cudaFuncSetAttribute(attn_prefill_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attn_prefill_kernel<64><<<grid, 256, smem, st>>>(qkv, kcache, vcache, out, T, pos0, nq, nkv, max_seq);
+  }
+}
+
+}  // namespace promoe

@@ -1,0 +1,169 @@
+// kernels_slot.cu — A6: the device-resident expert-cache slot table (lookup, hit/miss classes, LRU touch,
+// eviction, launch order, copy commands).  Logical-time reading of PAPER.md Alg. 2 + Alg. 1 l.3-5
+// + §5.3 + §6.1: every table transition happens here, in program order on
+// the compute stream; wall-clock only decides how long a consumer waits for bytes.
+#include "kernels.h"
+
+namespace promoe {
+
+constexpr int kMaxE = 256;
+
+struct SlotView {
+  int32_t* slot_expert; int32_t* expert_slot; unsigned long long* stamp; uint32_t* gen; uint8_t* origin;
+  unsigned long long* clock; int C, E;
+  __device__ void touch(int s) { stamp[s] = ++(*clock); }
+  // Alg. 1 l.4 cache.replace_with: lowest EMPTY slot, else smallest stamp among unprotected slots; -1 if none.
+  __device__ int victim(const uint8_t* prot) const {
+    for (int s = 0; s < C; ++s) if (slot_expert[s] < 0) return s;
+    int best = -1; unsigned long long bs = 0;
+    for (int s = 0; s < C; ++s) {
+      if (prot[slot_expert[s]]) continue;
+      if (best < 0 || stamp[s] < bs) { best = s; bs = stamp[s]; }
+    }
+    return best;
+  }
+  __device__ int install(int s, int e, uint8_t org) {
+    const int old = slot_expert[s];
+    if (old >= 0) expert_slot[old] = -1;
+    slot_expert[s] = e; expert_slot[e] = s; origin[s] = org;
+    touch(s);
+    gen[s] = (uint32_t)(*clock);
+    return old;
+  }
+};
+
+__global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, int stride,
+                                                         const int32_t* __restrict__ sel, int T, int k,
+                                                         const int32_t* __restrict__ offset,
+                                                         const int32_t* __restrict__ pred_list,
+                                                         const uint8_t* slot_base, size_t slot_bytes,
+                                                         const uint32_t* flag_base, int flags_per_slot, int H,
+                                                         int inter, int wbytes, FfnProblem* problems,
+                                                         int32_t* n_problems, int32_t* row_of, LayerCmd* cmd,
+                                                         uint32_t seq, int32_t* trace_precise,
+                                                         int32_t* trace_pred) {
+  __shared__ uint8_t needed[kMaxE];
+  __shared__ uint8_t prot[kMaxE];
+  __shared__ int16_t order[kMaxE];
+  __shared__ uint8_t cls[kMaxE];
+  __shared__ int32_t rec[6 * kMaxE];    // staged command records (mapped host memory is write-only here)
+  __shared__ int32_t prec[5 * kMaxE];
+  __shared__ int s_n, s_np;
+  const int E = tbl.E, C = tbl.C;
+  for (int e = threadIdx.x; e < kMaxE; e += blockDim.x) { needed[e] = 0; prot[e] = 0; }
+  __syncthreads();
+  for (int i = threadIdx.x; i < T * k; i += blockDim.x) needed[sel[i]] = 1;   // same-value writes
+  __syncthreads();
+  if (threadIdx.x == 0) {
+
+  SlotView v{tbl.slot_expert + (size_t)m * C, tbl.expert_slot + (size_t)m * E, tbl.stamp + (size_t)m * C,
+             tbl.gen + (size_t)m * C, tbl.origin + (size_t)m * C, tbl.clock, C, E};
+  // ---- PushPrecise(m): classes A (cached) → B (being prefetched) → C (not begun), ascending id inside
+  int n = 0, nA = 0, nB = 0;
+  for (int e = 0; e < E; ++e)
+    if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] != 1) { order[n] = e; cls[n++] = 0; }
+  nA = n;
+  for (int e = 0; e < E; ++e)
+    if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] == 1) { order[n] = e; cls[n++] = 1; }
+  nB = n - nA;
+  for (int e = 0; e < E; ++e)
+    if (needed[e] && v.expert_slot[e] < 0) { order[n] = e; cls[n++] = 2; }
+  (void)nB;
+  if (trace_precise) trace_precise[0] = n;
+  // touch A then B (Alg. 2 l.15-17)
+  for (int i = 0; i < n && cls[i] != 2; ++i) {
+    const int e = order[i], s = v.expert_slot[e];
+    v.touch(s);
+    int32_t* r = rec + 6 * i;
+    r[0] = e; r[1] = cls[i]; r[2] = s; r[3] = -1; r[4] = -1; r[5] = (int32_t)v.gen[s];
+  }
+  // class C: alloc; a needed expert not yet computed in launch order is pinned (G2); all pinned → wait for the
+  // next finish in launch order
+  for (int e = 0; e < E; ++e) prot[e] = needed[e];
+  int fin = 0;
+  for (int i = 0; i < n; ++i) {
+    if (cls[i] != 2) continue;
+    const int e = order[i];
+    int dep = -1;
+    int s = v.victim(prot);
+    while (s < 0) { prot[order[fin]] = 0; dep = fin; ++fin; s = v.victim(prot); }
+    const int old = v.install(s, e, 2);
+    int32_t* r = rec + 6 * i;
+    r[0] = e; r[1] = 2; r[2] = s; r[3] = old; r[4] = dep; r[5] = (int32_t)v.gen[s];
+  }
+  for (int s = 0; s < C; ++s) v.origin[s] = 0;
+  // problem table + decode row map + trace
+  const size_t hi = (size_t)H * inter * wbytes;
+  for (int i = 0; i < n; ++i) {
+    const int32_t* r = rec + 6 * i;
+    const int e = order[i];
+    // the slot recorded at e's own alloc/touch (a later deferred alloc may recycle it after e finished)
+    const int s = r[2];
+    const uint8_t* img = slot_base + ((size_t)m * C + s) * slot_bytes;
+    FfnProblem pb;
+    pb.wg = img; pb.wu = img + hi; pb.wd = img + 2 * hi;
+    pb.flags = flag_base + ((size_t)m * C + s) * flags_per_slot;
+    pb.gen = (uint32_t)r[5];
+    pb.inter = inter;
+    pb.row0 = offset ? offset[e] : i;
+    pb.nrows = offset ? offset[e + 1] - offset[e] : 1;
+    pb.expert = e; pb.pad = 0;
+    problems[i] = pb;
+    if (trace_precise) for (int q = 0; q < 5; ++q) trace_precise[1 + 5 * i + q] = r[q];
+  }
+  *n_problems = n;
+  if (row_of && T == 1)
+    for (int j = 0; j < k; ++j)
+      for (int i = 0; i < n; ++i) if (order[i] == sel[j]) row_of[j] = i;
+
+  // ---- PushPredicted(m + stride) (Alg. 2 l.1-10): touch cached, alloc missing as PRED; one push never evicts
+  // its own predictions; no victim → skip.
+  int np = 0;
+  const int mt = m + stride;
+  if (pred_list && mt < tbl.Lm) {
+    SlotView t{tbl.slot_expert + (size_t)mt * C, tbl.expert_slot + (size_t)mt * E, tbl.stamp + (size_t)mt * C,
+               tbl.gen + (size_t)mt * C, tbl.origin + (size_t)mt * C, tbl.clock, C, E};
+    np = pred_list[0];
+    for (int e = 0; e < E; ++e) prot[e] = 0;
+    for (int i = 0; i < np; ++i) prot[pred_list[1 + i]] = 1;
+    for (int i = 0; i < np; ++i) {
+      const int e = pred_list[1 + i];
+      int32_t* r = prec + 5 * i;
+      int s = t.expert_slot[e];
+      if (s >= 0) { t.touch(s); r[0] = e; r[1] = 0; r[2] = s; r[3] = -1; r[4] = (int32_t)t.gen[s]; }
+      else {
+        s = t.victim(prot);
+        if (s < 0) { r[0] = e; r[1] = 2; r[2] = -1; r[3] = -1; r[4] = 0; }
+        else { const int old = t.install(s, e, 1); r[0] = e; r[1] = 1; r[2] = s; r[3] = old; r[4] = (int32_t)t.gen[s]; }
+      }
+      if (trace_pred) for (int q = 0; q < 4; ++q) trace_pred[1 + 4 * i + q] = r[q];
+    }
+  }
+  if (trace_pred) trace_pred[0] = np;
+  s_n = n; s_np = np;
+  }  // thread 0
+  __syncthreads();
+  // publish the command to the host issuer (posted writes to mapped pinned memory), seq last
+  for (int i = threadIdx.x; i < 6 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
+  for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) cmd->pred[i] = prec[i];
+  if (threadIdx.x == 0) { cmd->n_needed = s_n; cmd->n_pred = s_np; cmd->pred_target = m + stride; }
+  __threadfence_system();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence_system();
+    cmd->seq = seq;        // release: the host issuer polls this word
+  }
+}
+
+void launch_slot_table(SlotTable tbl, int m, int stride, const int32_t* sel, int T, int k, const int32_t* offset,
+                       const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
+                       const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
+                       FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
+                       int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st) {
+  (void)reorder;
+  slot_table_kernel<<<1, 256, 0, st>>>(tbl, m, stride, sel, T, k, offset, pred_list, slot_base, slot_bytes,
+                                       flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of,
+                                       cmd, seq, trace_precise, trace_pred);
+}
+
+}  // namespace promoe
