@@ -4,7 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-namespace promoe {
+namespace pmk {
 
 constexpr int kWarp = 32;
 
@@ -126,4 +126,4 @@ struct FfnProblem {
   int pad;
 };
 
-}  // namespace promoe
+}  // namespace pmk

@@ -1,0 +1,95 @@
+// engine.h — the promoe handle: device buffers, slot region, copy engine state.  Internal to the library.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <deque>
+#include <string>
+#include <vector>
+
+#include "../../include/promoe.h"
+#include "kernels.h"
+
+namespace pmk {
+
+// One expert fill = all chunks of one expert image into one slot (Alg. 1: tasks of one expert, in chunk order).
+struct FillJob {
+  int layer, slot, expert;
+  uint32_t gen;
+  int prio;  // 0 HIGH, 1 LOW
+};
+// Physical state of a slot (what the copy stream has been asked to do), as opposed to the logical table on
+// the device.  issued = chunks of generation `gen` already enqueued on the copy stream, in chunk order.
+struct SlotPhys {
+  uint32_t gen = 0;
+  int expert = -1;
+  int issued = 0;
+  cudaEvent_t done = nullptr;   // recorded after the last chunk of the current generation
+  bool done_valid = false;
+};
+
+}  // namespace pmk
+
+struct promoe {
+  promoe_shape_t s{};
+  promoe_opts_t o{};
+  int Lm = 0, C = 0, wb = 2, n_chunks = 0, max_inflight = 2;
+  size_t Be = 0, chunk_bytes = 0;
+  int maxT = 0, qkv_w = 0, ffn_w = 0, nsplit = 1;
+  cudaStream_t cs = nullptr, ps = nullptr;
+  bool own_cs = false, dense_loaded = false, experts_loaded = false;
+  std::string err;
+
+  // dense weights: host copies of the per-layer device-pointer arrays
+  const void *emb = nullptr, *lm_head = nullptr;
+  const float* final_norm = nullptr;
+  std::vector<const float*> ln1, ln2, router_bias;
+  std::vector<const void*> wqkv, wo, router, pred_w1, pred_w2, ffn_gate, ffn_up, ffn_down, shared_gate_w;
+  std::vector<const void*> expert_host;   // [Lm*E] pinned host images
+  std::vector<void*> registered;          // buffers we had to cudaHostRegister
+
+  // activations (fp32)
+  float *x = nullptr, *u1 = nullptr, *u = nullptr, *qkv = nullptr, *attn = nullptr, *zraw = nullptr;
+  float *p1 = nullptr, *p2 = nullptr, *act = nullptr, *yexp = nullptr, *sact = nullptr, *sy = nullptr;
+  float *sgate = nullptr, *attn_ws = nullptr, *xf = nullptr, *logits = nullptr;
+  float *kcache = nullptr, *vcache = nullptr, *cos_t = nullptr, *sin_t = nullptr;
+  int32_t* ids = nullptr;
+  // per-MoE-layer routing / permutation buffers (double as traces)
+  int32_t *sel = nullptr, *count = nullptr, *offset = nullptr, *perm = nullptr, *inv = nullptr;
+  float *gates = nullptr, *margin = nullptr, *z = nullptr;
+  int32_t *pred_list = nullptr, *trace_precise = nullptr, *trace_pred = nullptr, *row_of = nullptr,
+          *n_prob = nullptr;
+  pmk::FfnProblem *problems = nullptr, *shared_prob = nullptr;
+  int* err_dev = nullptr;
+
+  // expert cache
+  uint8_t* slots = nullptr;       // ONE contiguous region [Lm, C, Be]
+  uint32_t* flags = nullptr;      // [Lm, C, n_chunks]
+  pmk::SlotTable tbl{};
+  pmk::LayerCmd* cmd_host = nullptr;   // mapped pinned, [Lm]
+  pmk::LayerCmd* cmd_dev = nullptr;
+  uint32_t* flagsrc_host = nullptr;       // pinned ring of flag values (fallback flag writes)
+  size_t flagsrc_pos = 0;
+  void* fn_write32 = nullptr;             // cuStreamWriteValue32, if the driver exposes it
+
+  // copy engine (host)
+  std::vector<pmk::SlotPhys> phys;     // [Lm*C]
+  std::deque<pmk::FillJob> low;
+  std::vector<cudaEvent_t> ev_ring;       // per-chunk end events (timing enabled)
+  std::vector<cudaEvent_t> ev_ring_start;
+  size_t ev_head = 0, ev_tail = 0;        // in flight = [tail, head)
+  std::vector<int> ev_is_low;
+  int low_inflight = 0;
+  std::vector<cudaEvent_t> done_ev;       // prefill: per launch position "expert finished" events
+  cudaEvent_t step_start = nullptr, step_end = nullptr;
+
+  // host mirror for statistics
+  std::vector<int32_t> mirror;            // [Lm*C] slot -> expert
+  std::vector<uint8_t> start_resident;    // [Lm*E]
+  std::vector<std::vector<int32_t>> pending_pred;  // per target layer
+  std::vector<int32_t> trace_pred_host_lists;      // predictor_mode TRACE input [Lm*(1+E)]
+  promoe_stats_t st{};
+  int pos = 0;
+  uint32_t step_seq = 0;
+  int last_T = 0;
+  std::vector<uint8_t> trace_buf;         // host staging for promoe_get_trace
+};

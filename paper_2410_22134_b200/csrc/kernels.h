@@ -6,7 +6,7 @@
 
 #include "common.cuh"
 
-namespace promoe {
+namespace pmk {
 
 // A0 embedding lookup: x[t,:] = Emb[ids[t],:] widened to fp32.
 void launch_embed(const int32_t* ids, const void* emb, float* x, int T, int H, int wdtype, cudaStream_t st);
@@ -60,8 +60,8 @@ struct LayerCmd {
   int32_t n_needed;
   int32_t n_pred;            // entries of the push INTO layer (m + stride), 0 if none
   int32_t pred_target;
-  // needed experts in launch order: expert, class (0 A,1 B,2 C), slot, victim, dep, gen
-  int32_t need[6 * 256];
+  // needed experts in launch order: expert, class (0 A,1 B,2 C), slot, victim, dep, gen, nrows
+  int32_t need[7 * 256];
   // predicted experts in listed order: expert, action (0 touch,1 alloc,2 skip), slot, victim, gen
   int32_t pred[5 * 256];
 };
@@ -84,10 +84,10 @@ void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* pr
 // A9 prefill grouped SwiGLU FFN, SIMT fp32: problems [p0, p0+np) each with its row range; x rows are gathered
 // through row_src (permuted position -> row_src[pos] / src_div = token) or direct when row_src == nullptr.
 void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src_div, const FfnProblem* probs,
-                                 int p0, int np, int max_rows, int max_inter, int H, float* act, int act_stride, int wdtype,
-                                 cudaStream_t st);
+                                 int p0, int np, int max_rows, int rows_override, int max_inter, int H, float* act,
+                                 int act_stride, int wdtype, cudaStream_t st);
 void launch_ffn_down_gemm_simt(const float* act, int act_stride, const FfnProblem* probs, int p0, int np,
-                               int max_rows, int max_inter, int H, float* y, int wdtype, cudaStream_t st);
+                               int max_rows, int rows_override, int max_inter, int H, float* y, int wdtype, cudaStream_t st);
 
 // A10 combine: out[t,:] = hres[t,:] + sum_j (fixed j order) g[t,j] * yexp[row(t,j),:] (+ sgate[t]*shared[t,:]).
 //  row(t,j) = inv[t*k+j] (prefill) or pos_of_j[j] (decode).  shared may be nullptr; sgate nullptr => 1.
@@ -96,4 +96,4 @@ void launch_combine(const float* hres, const float* yexp, const int32_t* row_of,
 // out[t,:] = a[t,:] + b[t,:]  (dense layer residual)
 void launch_add(const float* a, const float* b, float* out, size_t n, cudaStream_t st);
 
-}  // namespace promoe
+}  // namespace pmk

@@ -2,7 +2,7 @@
 // attention (A3, fp32 flash-style SIMT).  All fp32: the KV cache stays fp32 (reading G1).
 #include "kernels.h"
 
-namespace promoe {
+namespace pmk {
 
 // ---------------------------------------------------------------------------------------------------------
 // A2: rotate-half RoPE on q and k heads in place, then append k, v to the cache.
@@ -255,4 +255,4 @@ void launch_attn_prefill(const float* qkv, const float* kcache, const float* vca
   }
 }
 
-}  // namespace promoe
+}  // namespace pmk

@@ -2,7 +2,7 @@
 // Rows A0, A1 and the linear parts of A2/A3/A4/A5/A10 of DESIGN.md.
 #include "kernels.h"
 
-namespace promoe {
+namespace pmk {
 
 // ---------------------------------------------------------------------------------------------------------
 // A0 embedding lookup
@@ -141,4 +141,4 @@ void launch_add(const float* a, const float* b, float* out, size_t n, cudaStream
   add_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, b, out, n);
 }
 
-}  // namespace promoe
+}  // namespace pmk

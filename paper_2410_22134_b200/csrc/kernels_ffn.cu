@@ -3,7 +3,7 @@
 // (Alg. 1 l.10 `ready_chunk`).  Prefill: grouped SIMT fp32 GEMMs (correctness path; tcgen05 path: gemm_tc.cu).
 #include "kernels.h"
 
-namespace promoe {
+namespace pmk {
 
 // chunk index range [c0, c1] covering bytes [b0, b1) of the slot image
 __device__ __forceinline__ void chunk_range(size_t b0, size_t b1, size_t chunk_bytes, int* c0, int* c1) {
@@ -88,8 +88,9 @@ template <typename WT, bool SWIGLU>
 __global__ void __launch_bounds__(256) ffn_gemm_simt_kernel(const float* __restrict__ a, int lda,
                                                             const int32_t* __restrict__ row_src, int src_div,
                                                             const FfnProblem* __restrict__ probs, int p0, int H,
-                                                            float* __restrict__ out, int ldo) {
-  const FfnProblem pb = probs[p0 + blockIdx.z];
+                                                            float* __restrict__ out, int ldo, int rows_override) {
+  FfnProblem pb = probs[p0 + blockIdx.z];
+  if (rows_override > 0) pb.nrows = rows_override;
   const int m0 = blockIdx.y * FB;
   if (m0 >= pb.nrows) return;
   const int N = SWIGLU ? pb.inter : H;          // output features
@@ -171,22 +172,23 @@ void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* pr
                                                                                   tiles, H, y, chunk_bytes, err)));
 }
 void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src_div, const FfnProblem* probs,
-                                 int p0, int np, int max_rows, int max_inter, int H, float* act, int act_stride,
-                                 int wdtype, cudaStream_t st) {
+                                 int p0, int np, int max_rows, int rows_override, int max_inter, int H, float* act,
+                                 int act_stride, int wdtype, cudaStream_t st) {
   dim3 grid((max_inter + FB - 1) / FB, (max_rows + FB - 1) / FB, np);
   WDISPATCH((ffn_gemm_simt_kernel<float, true><<<grid, 256, 0, st>>>(x, H, row_src, src_div, probs, p0, H, act,
-                                                                     act_stride)),
+                                                                     act_stride, rows_override)),
             (ffn_gemm_simt_kernel<__nv_bfloat16, true><<<grid, 256, 0, st>>>(x, H, row_src, src_div, probs, p0, H,
-                                                                             act, act_stride)));
+                                                                             act, act_stride, rows_override)));
 }
 void launch_ffn_down_gemm_simt(const float* act, int act_stride, const FfnProblem* probs, int p0, int np,
-                               int max_rows, int max_inter, int H, float* y, int wdtype, cudaStream_t st) {
+                               int max_rows, int rows_override, int max_inter, int H, float* y, int wdtype,
+                               cudaStream_t st) {
   (void)max_inter;
   dim3 grid((H + FB - 1) / FB, (max_rows + FB - 1) / FB, np);
   WDISPATCH((ffn_gemm_simt_kernel<float, false><<<grid, 256, 0, st>>>(act, act_stride, nullptr, 1, probs, p0, H, y,
-                                                                      H)),
+                                                                      H, rows_override)),
             (ffn_gemm_simt_kernel<__nv_bfloat16, false><<<grid, 256, 0, st>>>(act, act_stride, nullptr, 1, probs, p0,
-                                                                              H, y, H)));
+                                                                              H, y, H, rows_override)));
 }
 
-}  // namespace promoe
+}  // namespace pmk

@@ -2,7 +2,7 @@
 // weighted combine (A10).  sm_100a.
 #include "kernels.h"
 
-namespace promoe {
+namespace pmk {
 
 // ---------------------------------------------------------------------------------------------------------
 // Warp-shuffle top-k.  One warp per token; lane holds experts lane, lane+32, ... (NPL per lane, E <= 32*NPL).
@@ -252,4 +252,4 @@ void launch_combine(const float* hres, const float* yexp, const int32_t* row_of,
   combine_kernel<<<T, 256, 0, st>>>(hres, yexp, row_of, gates, k, H, shared, sgate_logit, out);
 }
 
-}  // namespace promoe
+}  // namespace pmk

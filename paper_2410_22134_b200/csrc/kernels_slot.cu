@@ -4,7 +4,7 @@
 // the compute stream; wall-clock only decides how long a consumer waits for bytes.
 #include "kernels.h"
 
-namespace promoe {
+namespace pmk {
 
 constexpr int kMaxE = 256;
 
@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   __shared__ uint8_t prot[kMaxE];
   __shared__ int16_t order[kMaxE];
   __shared__ uint8_t cls[kMaxE];
-  __shared__ int32_t rec[6 * kMaxE];    // staged command records (mapped host memory is write-only here)
+  __shared__ int32_t rec[7 * kMaxE];    // staged command records (mapped host memory is write-only here)
   __shared__ int32_t prec[5 * kMaxE];
   __shared__ int s_n, s_np;
   const int E = tbl.E, C = tbl.C;
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   for (int i = 0; i < n && cls[i] != 2; ++i) {
     const int e = order[i], s = v.expert_slot[e];
     v.touch(s);
-    int32_t* r = rec + 6 * i;
+    int32_t* r = rec + 7 * i;
     r[0] = e; r[1] = cls[i]; r[2] = s; r[3] = -1; r[4] = -1; r[5] = (int32_t)v.gen[s];
   }
   // class C: alloc; a needed expert not yet computed in launch order is pinned (G2); all pinned → wait for the
@@ -88,14 +88,14 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
     int s = v.victim(prot);
     while (s < 0) { prot[order[fin]] = 0; dep = fin; ++fin; s = v.victim(prot); }
     const int old = v.install(s, e, 2);
-    int32_t* r = rec + 6 * i;
+    int32_t* r = rec + 7 * i;
     r[0] = e; r[1] = 2; r[2] = s; r[3] = old; r[4] = dep; r[5] = (int32_t)v.gen[s];
   }
   for (int s = 0; s < C; ++s) v.origin[s] = 0;
   // problem table + decode row map + trace
   const size_t hi = (size_t)H * inter * wbytes;
   for (int i = 0; i < n; ++i) {
-    const int32_t* r = rec + 6 * i;
+    const int32_t* r = rec + 7 * i;
     const int e = order[i];
     // the slot recorded at e's own alloc/touch (a later deferred alloc may recycle it after e finished)
     const int s = r[2];
@@ -109,6 +109,7 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
     pb.nrows = offset ? offset[e + 1] - offset[e] : 1;
     pb.expert = e; pb.pad = 0;
     problems[i] = pb;
+    rec[7 * i + 6] = pb.nrows;
     if (trace_precise) for (int q = 0; q < 5; ++q) trace_precise[1 + 5 * i + q] = r[q];
   }
   *n_problems = n;
@@ -144,7 +145,7 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   }  // thread 0
   __syncthreads();
   // publish the command to the host issuer (posted writes to mapped pinned memory), seq last
-  for (int i = threadIdx.x; i < 6 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
+  for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
   for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) cmd->pred[i] = prec[i];
   if (threadIdx.x == 0) { cmd->n_needed = s_n; cmd->n_pred = s_np; cmd->pred_target = m + stride; }
   __threadfence_system();
@@ -166,4 +167,4 @@ void launch_slot_table(SlotTable tbl, int m, int stride, const int32_t* sel, int
                                        cmd, seq, trace_precise, trace_pred);
 }
 
-}  // namespace promoe
+}  // namespace pmk
