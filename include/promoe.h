@@ -26,6 +26,12 @@
 extern "C" {
 #endif
 
+#if defined(__GNUC__)
+#define PROMOE_API __attribute__((visibility("default")))
+#else
+#define PROMOE_API
+#endif
+
 #define PROMOE_OK 0
 #define PROMOE_EINVAL (-1)   /* bad argument / unsupported shape */
 #define PROMOE_ENOMEM (-2)   /* device or host allocation failed */
@@ -121,51 +127,51 @@ typedef struct {
 #define PROMOE_TRACE_PREDLIST 7  /* int32 [n_moe, 1 + E]  n, list predicted BY the predictor at layer m (uncapped by G5) */
 #define PROMOE_TRACE_ZLOGITS 8   /* float [n_moe, T, E]   router logits */
 
-int promoe_create(const promoe_shape_t* shape, const promoe_opts_t* opts, promoe_t** out);
-void promoe_destroy(promoe_t* h);
-const char* promoe_last_error(const promoe_t* h); /* h may be NULL: last create error */
+PROMOE_API int promoe_create(const promoe_shape_t* shape, const promoe_opts_t* opts, promoe_t** out);
+PROMOE_API void promoe_destroy(promoe_t* h);
+PROMOE_API const char* promoe_last_error(const promoe_t* h); /* h may be NULL: last create error */
 
 /* Hand over the non-expert parameters (device pointers, borrowed). */
-int promoe_load_dense(promoe_t* h, const promoe_dense_t* w);
+PROMOE_API int promoe_load_dense(promoe_t* h, const promoe_dense_t* w);
 
 /* host_ptrs[m*E + e] = host image of routed expert e of MoE layer m: [Wgate (I x H) | Wup (I x H) | Wdown
  * (H x I)] contiguous, expert_bytes = 3*H*I*sizeof(w) (three linears).  Borrowed until destroy.
  * With PROMOE_F_WARM the first C experts of every layer are copied into their slots here. */
-int promoe_load_experts(promoe_t* h, const void* const* host_ptrs, size_t expert_bytes);
+PROMOE_API int promoe_load_experts(promoe_t* h, const void* const* host_ptrs, size_t expert_bytes);
 
 /* Prefill: ids_host = host ptr to n_tokens int32 ids; positions continue from the current sequence length.
  * logits_out = HOST ptr to vocab floats (last token) or NULL.  Synchronous: returns when logits are valid. */
-int promoe_prefill(promoe_t* h, const int32_t* ids_host, int32_t n_tokens, float* logits_out);
+PROMOE_API int promoe_prefill(promoe_t* h, const int32_t* ids_host, int32_t n_tokens, float* logits_out);
 /* Decode one token (caller samples; tests teacher-force).  logits_out as above. */
-int promoe_decode(promoe_t* h, int32_t token_id, float* logits_out);
+PROMOE_API int promoe_decode(promoe_t* h, int32_t token_id, float* logits_out);
 
 /* predictor_mode TRACE: lists for the NEXT step call; pred[m*(1+E)] = n, then n expert ids = the list the
  * predictor at MoE layer m would emit for layer m+stride.  Host ptr, copied. */
-int promoe_set_prediction_trace(promoe_t* h, const int32_t* pred, size_t n_int32);
+PROMOE_API int promoe_set_prediction_trace(promoe_t* h, const int32_t* pred, size_t n_int32);
 
-int promoe_stats(promoe_t* h, promoe_stats_t* out);
-int promoe_get_trace(promoe_t* h, int which, const void** data, size_t* bytes);
-int promoe_reset(promoe_t* h);   /* clears KV cache, cache state (re-warms if F_WARM) and stats */
+PROMOE_API int promoe_stats(promoe_t* h, promoe_stats_t* out);
+PROMOE_API int promoe_get_trace(promoe_t* h, int which, const void** data, size_t* bytes);
+PROMOE_API int promoe_reset(promoe_t* h);   /* clears KV cache, cache state (re-warms if F_WARM) and stats */
 
 /* Current logical slot table of MoE layer m: slot_expert_out = host ptr to C int32 (-1 = empty). */
-int promoe_get_slots(promoe_t* h, int32_t moe_layer, int32_t* slot_expert_out);
+PROMOE_API int promoe_get_slots(promoe_t* h, int32_t moe_layer, int32_t* slot_expert_out);
 
 /* Measured pinned host->device bandwidth (GB/s) for `bytes`-sized copies at queue depth `depth`
  * (chunk size is chosen from this curve).  Allocates and frees its own buffers. */
-int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out);
+PROMOE_API int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out);
 
 /* Micro entry points: single hot-path steps on caller-provided DEVICE buffers (used by kernel-level parity
  * tests and bench.py's per-kernel roofline).  stream = cudaStream_t or NULL (default stream).
  * All are asynchronous on `stream`. */
 /* y[T,N] = x[T,K] . W[N,K]^T ; x,y fp32; W wdtype (0 fp32 / 1 bf16). path: 0 auto, 1 gemv, 2 simt gemm, 3 tcgen05 */
-int promoe_op_linear(const float* x, const void* w, float* y, int32_t T, int32_t N, int32_t K, int32_t wdtype,
+PROMOE_API int promoe_op_linear(const float* x, const void* w, float* y, int32_t T, int32_t N, int32_t K, int32_t wdtype,
                      int32_t path, void* stream);
 /* router row A4: z = u.R^T (+b); top-k (ties -> lower index); gates = softmax over selected. */
-int promoe_op_route(const float* u, const void* router, const float* bias, int32_t T, int32_t H, int32_t E,
+PROMOE_API int promoe_op_route(const float* u, const void* router, const float* bias, int32_t T, int32_t H, int32_t E,
                     int32_t k, int32_t wdtype, float* z_out, int32_t* sel_out, float* gates_out,
                     float* margin_out, void* stream);
 /* permutation row A8: sel [T,k] -> count[E], offset[E+1], perm[T*k], inv[T*k] */
-int promoe_op_permute(const int32_t* sel, int32_t T, int32_t k, int32_t E, int32_t* count, int32_t* offset,
+PROMOE_API int promoe_op_permute(const int32_t* sel, int32_t T, int32_t k, int32_t E, int32_t* count, int32_t* offset,
                       int32_t* perm, int32_t* inv, void* stream);
 
 #ifdef __cplusplus

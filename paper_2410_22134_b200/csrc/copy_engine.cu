@@ -1,0 +1,227 @@
+// copy_engine.cu — A7: chunked host→device prefetch on the dedicated copy stream (§5.1 chunked
+// prefetching P:185-193, §5.2 early preemption P:197-227, Alg. 1, two-priority queue P:179).
+//
+// Re-design for B200: there is no worker thread and no software queue for HIGH tasks.
+// The slot-table kernel (A6) publishes, per MoE layer, one command record in mapped pinned memory; the step
+// thread reads it and
+//   * HIGH (precise) fills: every missing chunk is enqueued on the copy stream at once, in launch order — nothing
+//     may overtake them, so the stream itself is the queue;
+//   * LOW (predicted) fills: kept in a host deque and fed to the stream only `max_inflight` chunks at a time, so a
+//     HIGH chunk waits for at most that many LOW chunks (bounded preemption delay); the un-issued LOW
+//     chunks of a layer are dropped at that layer's gate (Alg. 2 l.12);
+//   * every chunk is followed, on the same stream, by a 32-bit write of the slot's allocation generation into
+//     flags[slot][chunk] (Alg. 1 l.10 `ready_chunk`); expert kernels gate on exactly the chunks they read.
+// Nothing here changes the logical slot table: it lives on the device and advances in program order.
+#include "engine.h"
+
+#include <cuda.h>
+
+#include <atomic>
+#include <chrono>
+#include <cstring>
+
+using namespace pmk;
+
+#define CKC(call)                                                                                  \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      h->err = std::string(#call) + ": " + cudaGetErrorString(e_);                                 \
+      return PROMOE_ECUDA;                                                                         \
+    }                                                                                              \
+  } while (0)
+
+typedef CUresult (*write32_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+
+// retire finished timing slots of the ring; `all` = wait for every one (step end)
+int ce_retire(promoe_t* h, bool all) {
+  while (h->ev_tail != h->ev_head) {
+    const size_t i = h->ev_tail % h->ev_ring.size();
+    cudaError_t q = all ? cudaEventSynchronize(h->ev_ring[i]) : cudaEventQuery(h->ev_ring[i]);
+    if (q == cudaErrorNotReady) break;
+    if (q != cudaSuccess) { h->err = std::string("copy event: ") + cudaGetErrorString(q); return PROMOE_ECUDA; }
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, h->ev_ring_start[i], h->ev_ring[i]) == cudaSuccess) h->st.copy_busy_ms += ms;
+    if (h->ev_is_low[i]) h->low_inflight--;
+    h->ev_tail++;
+  }
+  return PROMOE_OK;
+}
+
+static int ring_slot(promoe_t* h, size_t* idx) {
+  if (h->ev_head - h->ev_tail >= h->ev_ring.size()) {   // full: wait for the oldest
+    const size_t i = h->ev_tail % h->ev_ring.size();
+    CKC(cudaEventSynchronize(h->ev_ring[i]));
+    int rc = ce_retire(h, false);
+    if (rc) return rc;
+  }
+  *idx = h->ev_head % h->ev_ring.size();
+  return PROMOE_OK;
+}
+
+// Enqueue chunks [c0, c1) of the fill (layer m, slot s) on the copy stream, each followed by its flag write.
+// One timing slot brackets the whole range.
+static int issue_chunks(promoe_t* h, int m, int s, int c0, int c1, bool low) {
+  SlotPhys& p = h->phys[(size_t)m * h->C + s];
+  const uint8_t* src = (const uint8_t*)h->expert_host[(size_t)m * h->s.n_experts + p.expert];
+  uint8_t* dst = h->slots + ((size_t)m * h->C + s) * h->Be;
+  uint32_t* fl = h->flags + ((size_t)m * h->C + s) * h->n_chunks;
+  size_t ri = 0;
+  int rc = ring_slot(h, &ri);
+  if (rc) return rc;
+  CKC(cudaEventRecord(h->ev_ring_start[ri], h->ps));
+  for (int c = c0; c < c1; ++c) {
+    const size_t off = (size_t)c * h->chunk_bytes;
+    const size_t len = std::min(h->chunk_bytes, h->Be - off);
+    CKC(cudaMemcpyAsync(dst + off, src + off, len, cudaMemcpyHostToDevice, h->ps));
+    if (h->fn_write32) {
+      CUresult r = ((write32_fn)h->fn_write32)((CUstream)h->ps, (CUdeviceptr)(uintptr_t)(fl + c), p.gen, 0);
+      if (r != CUDA_SUCCESS) { h->err = "cuStreamWriteValue32 failed"; return PROMOE_ECUDA; }
+    } else {
+      uint32_t* v = h->flagsrc_host + (h->flagsrc_pos++ % 65536);
+      *v = p.gen;
+      CKC(cudaMemcpyAsync(fl + c, v, 4, cudaMemcpyHostToDevice, h->ps));
+    }
+    h->st.h2d_bytes += len;
+    h->st.chunks_issued++;
+    if (low) h->st.chunks_low++; else h->st.chunks_high++;
+  }
+  CKC(cudaEventRecord(h->ev_ring[ri], h->ps));
+  h->ev_is_low[ri] = low ? 1 : 0;
+  if (low) h->low_inflight++;
+  h->ev_head++;
+  p.issued = c1;
+  if (c1 == h->n_chunks) { CKC(cudaEventRecord(p.done, h->ps)); p.done_valid = true; }
+  return PROMOE_OK;
+}
+
+// LOW queue: feed the copy stream while fewer than max_inflight LOW chunks are in flight.
+int ce_pump_low(promoe_t* h) {
+  int rc = ce_retire(h, false);
+  if (rc) return rc;
+  while (!h->low.empty() && h->low_inflight < h->max_inflight) {
+    FillJob j = h->low.front();
+    SlotPhys& p = h->phys[(size_t)j.layer * h->C + j.slot];
+    if (p.gen != j.gen || p.expert != j.expert || p.issued >= h->n_chunks) { h->low.pop_front(); continue; }  // stale / done
+    rc = issue_chunks(h, j.layer, j.slot, p.issued, p.issued + 1, true);
+    if (rc) return rc;
+    if (p.issued >= h->n_chunks) h->low.pop_front();
+  }
+  return PROMOE_OK;
+}
+
+// Early preemption (Alg. 2 l.12): drop the un-issued LOW chunks that target layer m.
+void ce_cancel_low(promoe_t* h, int m) {
+  for (auto it = h->low.begin(); it != h->low.end();) {
+    if (it->layer == m) {
+      const SlotPhys& p = h->phys[(size_t)m * h->C + it->slot];
+      if (p.gen == it->gen && p.issued < h->n_chunks) h->st.chunks_cancelled += (uint64_t)(h->n_chunks - p.issued);
+      it = h->low.erase(it);
+    } else ++it;
+  }
+}
+
+// Wait (host) for the command of MoE layer m of step `seq`, pumping LOW chunks meanwhile.
+int ce_wait_cmd(promoe_t* h, int m, uint32_t seq) {
+  volatile uint32_t* w = &h->cmd_host[m].seq;
+  const auto t0 = std::chrono::steady_clock::now();
+  unsigned spins = 0;
+  while (*w != seq) {
+    if (!h->low.empty() || h->ev_tail != h->ev_head) {
+      int rc = ce_pump_low(h);
+      if (rc) return rc;
+    }
+    if ((++spins & 0x3ff) == 0) {
+      if (std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count() > 20.0) {
+        cudaError_t e = cudaStreamQuery(h->cs);
+        h->err = std::string("timeout waiting for the slot-table command: ") + cudaGetErrorString(e);
+        return PROMOE_ETIMEOUT;
+      }
+    }
+  }
+  std::atomic_thread_fence(std::memory_order_acquire);
+  return PROMOE_OK;
+}
+
+// Enqueue (HIGH) whatever is still missing of the fill behind needed record i of layer m; `after` = event the copy
+// stream must wait for first (the compute that last read the slot's previous occupant, reading G2) or nullptr.
+int ce_issue_needed(promoe_t* h, int m, int i, cudaEvent_t after) {
+  const int32_t* r = (const int32_t*)h->cmd_host[m].need + 7 * i;
+  SlotPhys& p = h->phys[(size_t)m * h->C + r[2]];
+  if (p.issued >= h->n_chunks) return PROMOE_OK;
+  if (after) CKC(cudaStreamWaitEvent(h->ps, after, 0));
+  return issue_chunks(h, m, r[2], p.issued, h->n_chunks, false);
+}
+
+// Process the command of MoE layer m: statistics, cancellation, HIGH fills (launch order), LOW jobs.
+// Class-C fills whose slot is recycled inside the layer (dep >= 0: prefill with |needed| > C) are NOT
+// issued here: their indices are appended to `deferred` and the step scheduler issues them with
+// ce_issue_needed once the compute of launch position `dep` has been enqueued.
+int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
+  const LayerCmd& c = h->cmd_host[m];
+  const int n = c.n_needed, E = h->s.n_experts, C = h->C;
+  promoe_stats_t& st = h->st;
+  if (h->o.flags & PROMOE_F_PREEMPT) ce_cancel_low(h, m);
+  // prediction accuracy: |pred ∩ needed| / |pred| for the list pushed into this layer
+  std::vector<int32_t>& pend = h->pending_pred[m];
+  if (!pend.empty()) {
+    st.predicted += pend.size();
+    for (int32_t e : pend)
+      for (int i = 0; i < n; ++i) if (c.need[7 * i] == e) { st.predicted_correct++; break; }
+    pend.clear();
+  }
+  st.accesses += n;
+  for (int i = 0; i < n; ++i) {
+    const int32_t* r = (const int32_t*)c.need + 7 * i;
+    const int e = r[0], cls = r[1], s = r[2], victim = r[3], dep = r[4];
+    const uint32_t gen = (uint32_t)r[5];
+    SlotPhys& p = h->phys[(size_t)m * C + s];
+    if (!h->start_resident[(size_t)m * E + e]) st.need_experts++;
+    if (cls == 0) st.hits_resident++;
+    else if (cls == 1) {
+      st.hits_prefetch++;
+      st.fetched_at_gate_of++;
+      if (p.gen == gen && p.issued >= h->n_chunks && p.done_valid && cudaEventQuery(p.done) == cudaSuccess) st.fetched_at_gate++;
+    } else {
+      st.misses++;
+      if (victim >= 0) st.evictions++;
+      h->mirror[(size_t)m * C + s] = e;
+    }
+    if (dep >= 0 && deferred) { deferred->push_back(i); continue; }   // slot still in use by launch position dep
+    if (p.gen != gen || p.expert != e) {   // new allocation of this slot
+      p.gen = gen; p.expert = e; p.issued = 0; p.done_valid = false;
+    }
+    int rc = ce_issue_needed(h, m, i, nullptr);
+    if (rc) return rc;
+  }
+  // PushPredicted(m + stride): LOW jobs (Alg. 2 l.1-10)
+  const int mt = c.pred_target;
+  if (c.n_pred > 0 && mt < h->Lm) {
+    std::vector<int32_t>& pd = h->pending_pred[mt];
+    pd.clear();
+    for (int i = 0; i < c.n_pred; ++i) {
+      const int32_t* r = (const int32_t*)c.pred + 5 * i;
+      const int e = r[0], action = r[1], s = r[2], victim = r[3];
+      const uint32_t gen = (uint32_t)r[4];
+      pd.push_back(e);
+      if (action == 2) continue;           // SKIP: no victim available
+      SlotPhys& p = h->phys[(size_t)mt * C + s];
+      if (action == 1) {
+        st.pred_allocs++;
+        if (victim >= 0) st.evictions++;
+        h->mirror[(size_t)mt * C + s] = e;
+        p.gen = gen; p.expert = e; p.issued = 0; p.done_valid = false;
+      }
+      if (p.issued < h->n_chunks) h->low.push_back(FillJob{mt, s, e, gen, 1});   // alloc, or touch of a cancelled fill (G3)
+    }
+  }
+  return ce_pump_low(h);
+}
+
+// Deferred class-C fill: take over the slot physically (the previous occupant's compute is ordered by `after`).
+int ce_issue_deferred(promoe_t* h, int m, int i, cudaEvent_t after) {
+  const int32_t* r = (const int32_t*)h->cmd_host[m].need + 7 * i;
+  SlotPhys& p = h->phys[(size_t)m * h->C + r[2]];
+  p.gen = (uint32_t)r[5]; p.expert = r[0]; p.issued = 0; p.done_valid = false;
+  return ce_issue_needed(h, m, i, after);
+}

@@ -1,0 +1,224 @@
+// step.cu — the step scheduler: promoe_prefill / promoe_decode.  One host call per step; every arithmetic step
+// of the path runs in the kernels of kernels_*.cu on the compute stream `cs`, copies on the copy stream `ps`.
+//
+// Per layer:
+//   A1 rmsnorm → A2 qkv + rope + kv append → A3 attention + o-proj + residual → A1 rmsnorm
+//   dense layer: SwiGLU FFN + residual
+//   MoE layer m: A4 router + top-k + gates ‖ A5 predictor scores → list ‖ A8 permutation (T > 1)
+//                A6 slot-table kernel: PushPrecise(m) then PushPredicted(m+stride) (Alg. 2) → problem
+//                   table in launch order (cached → being prefetched → missing) + host command
+//                shared expert (always resident) is launched BEFORE the host looks at the command: it covers the
+//                   device→host hand-over and the first copy
+//                A7 host: cancel stale LOW chunks, enqueue HIGH fills, queue LOW fills
+//                A9 routed experts in launch order; decode: GEMV kernels gating on chunk flags; prefill: grouped
+//                   GEMMs, ready groups first, slots recycled in launch order when |needed| > C
+//                A10 combine in fixed j order + shared + residual
+//   final norm + lm_head on the last token.
+#include "engine.h"
+
+#include <cstring>
+
+using namespace pmk;
+
+int ce_retire(promoe_t* h, bool all);
+int ce_pump_low(promoe_t* h);
+int ce_wait_cmd(promoe_t* h, int m, uint32_t seq);
+int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred);
+int ce_issue_deferred(promoe_t* h, int m, int i, cudaEvent_t after);
+
+#define CKS(call)                                                                                  \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      h->err = std::string(#call) + ": " + cudaGetErrorString(e_);                                 \
+      return PROMOE_ECUDA;                                                                         \
+    }                                                                                              \
+  } while (0)
+
+// y[T,N] (+)= x[T,K]·W^T on the compute stream: GEMV for one token, GEMM otherwise.
+static void linear(promoe_t* h, const float* x, const void* w, float* y, int T, int N, int K, int flags) {
+  if (T == 1) launch_gemv(x, w, y, N, K, h->s.wdtype, flags, h->cs);
+  else launch_linear_gemm(x, w, y, T, N, K, h->s.wdtype, flags, (h->o.flags & PROMOE_F_TENSOR) != 0, h->cs);
+}
+
+// SwiGLU FFN of an always-resident MLP (shared expert / dense layer) for all T rows of u → h->sy.
+static void resident_ffn(promoe_t* h, int l, int inter, int T) {
+  const int H = h->s.hidden, wd = h->s.wdtype;
+  if (T == 1) {
+    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs);
+    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs);
+  } else {
+    launch_ffn_gateup_gemm(h->u, nullptr, 1, h->shared_prob, l, 1, T, T, inter, H, h->sact, h->ffn_w, wd,
+                           (h->o.flags & PROMOE_F_TENSOR) != 0, h->cs);
+    launch_ffn_down_gemm(h->sact, h->ffn_w, h->shared_prob, l, 1, T, T, inter, H, h->sy, wd,
+                         (h->o.flags & PROMOE_F_TENSOR) != 0, h->cs);
+  }
+}
+
+static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_out) {
+  const promoe_shape_t& s = h->s;
+  const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter;
+  const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = s.wdtype;
+  const bool tensor = (h->o.flags & PROMOE_F_TENSOR) != 0;
+  if (!h->dense_loaded || !h->experts_loaded) { h->err = "step before load_dense / load_experts"; return PROMOE_ESTATE; }
+  if (T < 1 || !ids_host) { h->err = "step: no tokens"; return PROMOE_EINVAL; }
+  if (h->pos + T > s.max_seq) { h->err = "step: sequence exceeds max_seq"; return PROMOE_ESTATE; }
+  for (int t = 0; t < T; ++t)
+    if (ids_host[t] < 0 || ids_host[t] >= s.vocab) { h->err = "step: token id out of range"; return PROMOE_EINVAL; }
+  cudaStream_t cs = h->cs;
+  const uint32_t step_seq = ++h->step_seq;
+  const int pos0 = h->pos;
+  // residency at step start, for B_need: needed \ resident-at-step-start
+  std::fill(h->start_resident.begin(), h->start_resident.end(), 0);
+  for (int m = 0; m < Lm; ++m)
+    for (int i = 0; i < C; ++i) {
+      const int e = h->mirror[(size_t)m * C + i];
+      if (e >= 0) h->start_resident[(size_t)m * E + e] = 1;
+    }
+  for (auto& v : h->pending_pred) v.clear();
+
+  CKS(cudaMemcpyAsync(h->ids, ids_host, (size_t)T * 4, cudaMemcpyHostToDevice, cs));
+  CKS(cudaEventRecord(h->step_start, cs));
+  if (h->o.flags & PROMOE_F_TRACE) {
+    CKS(cudaMemsetAsync(h->trace_pred, 0, (size_t)Lm * (1 + 4 * E) * 4, cs));
+    if (h->o.predictor_mode == PROMOE_PRED_NONE) CKS(cudaMemsetAsync(h->pred_list, 0, (size_t)Lm * (1 + E) * 4, cs));
+  }
+  launch_embed(h->ids, h->emb, h->x, T, H, wd, cs);
+  const size_t kv_layer = (size_t)nkv * s.max_seq * d;
+  std::vector<int> deferred;
+  for (int l = 0; l < s.n_layers; ++l) {
+    // ---- attention block (A1-A3)
+    launch_rmsnorm(h->x, h->ln1[l], h->u1, T, H, s.rms_eps, cs);
+    linear(h, h->u1, h->wqkv[l], h->qkv, T, h->qkv_w, H, 0);
+    float* kc = h->kcache + (size_t)l * kv_layer;
+    float* vc = h->vcache + (size_t)l * kv_layer;
+    launch_rope_append(h->qkv, h->cos_t, h->sin_t, kc, vc, T, pos0, nq, nkv, d, s.max_seq, cs);
+    if (T == 1) launch_attn_decode(h->qkv, kc, vc, h->attn, h->attn_ws, pos0 + 1, nq, nkv, d, s.max_seq, h->nsplit, cs);
+    else launch_attn_prefill(h->qkv, kc, vc, h->attn, T, pos0, nq, nkv, d, s.max_seq, cs);
+    linear(h, h->attn, h->wo[l], h->x, T, H, nq * d, LIN_ACC);
+    launch_rmsnorm(h->x, h->ln2[l], h->u, T, H, s.rms_eps, cs);
+    if (l < s.n_dense_layers) {
+      resident_ffn(h, l, s.dense_inter, T);
+      launch_add(h->x, h->sy, h->x, (size_t)T * H, cs);
+      continue;
+    }
+    // ---- MoE block
+    const int m = l - s.n_dense_layers;
+    const uint32_t seq = step_seq * 4096u + (uint32_t)m + 1u;
+    int32_t* sel = h->sel + (size_t)m * h->maxT * k;
+    float* gates = h->gates + (size_t)m * h->maxT * k;
+    int32_t* perm = h->perm + (size_t)m * h->maxT * k;
+    int32_t* inv = h->inv + (size_t)m * h->maxT * k;
+    int32_t* offset = h->offset + (size_t)m * (E + 1);
+    linear(h, h->u, h->router[l], h->zraw, T, E, H, 0);                               // A4
+    launch_topk_gate(h->zraw, s.router_bias ? h->router_bias[l] : nullptr, T, E, k, h->z + (size_t)m * h->maxT * E, sel,
+                     gates, h->margin + (size_t)m * h->maxT, cs);
+    int32_t* plist = nullptr;
+    if (h->o.predictor_mode == PROMOE_PRED_MLP) {                                      // A5
+      linear(h, h->u, h->pred_w1[l], h->p1, T, s.pred_hidden, H, LIN_RELU);
+      linear(h, h->p1, h->pred_w2[l], h->p2, T, E, s.pred_hidden, 0);
+      plist = h->pred_list + (size_t)m * (1 + E);
+      launch_pred_list(h->p2, T, E, k, C, plist, cs);
+    } else if (h->o.predictor_mode == PROMOE_PRED_TRACE) {
+      plist = h->pred_list + (size_t)m * (1 + E);
+    }
+    if (T > 1) launch_permute(sel, T, k, E, h->count + (size_t)m * E, offset, perm, inv, cs);   // A8
+    launch_slot_table(h->tbl, m, h->o.stride, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
+                      (h->o.flags & PROMOE_F_REORDER) != 0, h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb,
+                      h->problems, h->n_prob, h->row_of, h->cmd_dev + m, seq,
+                      h->trace_precise + (size_t)m * (1 + 5 * E),
+                      (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs);
+    const float* shared = nullptr;
+    const float* sgate = nullptr;
+    if (s.n_shared_inter) {                                                            // A10 shared expert first
+      resident_ffn(h, l, s.n_shared_inter, T);
+      shared = h->sy;
+      if (s.shared_gate) { linear(h, h->u, h->shared_gate_w[l], h->sgate, T, 1, H, 0); sgate = h->sgate; }
+    }
+    // ---- A7: hand-over to the copy engine
+    int rc = ce_wait_cmd(h, m, seq);
+    if (rc) return rc;
+    deferred.clear();
+    rc = ce_process_cmd(h, m, &deferred);
+    if (rc) return rc;
+    const LayerCmd& cmd = h->cmd_host[m];
+    const int n = cmd.n_needed;
+    // ---- A9 routed experts, launch order
+    if (T == 1) {
+      launch_ffn_gateup_gemv(h->u, h->problems, n, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);
+      launch_ffn_down_gemv(h->act, I, h->problems, n, I, H, h->yexp, wd, h->chunk_bytes, h->err_dev, cs);
+      launch_combine(h->x, h->yexp, h->row_of, gates, 1, k, H, shared, sgate, h->x, cs);
+    } else {
+      // batches: [all class A] [all class B] then every class C alone (its fill lands in copy order)
+      int i = 0;
+      size_t dnext = 0;
+      while (i < n) {
+        const int cls = cmd.need[7 * i + 1];
+        int j = i + 1;
+        if (cls != 2) while (j < n && cmd.need[7 * j + 1] == cls) ++j;
+        int max_rows = 0;
+        for (int q = i; q < j; ++q) {
+          max_rows = std::max(max_rows, (int)cmd.need[7 * q + 6]);
+          SlotPhys& p = h->phys[(size_t)m * C + cmd.need[7 * q + 2]];
+          if (p.done_valid) CKS(cudaStreamWaitEvent(cs, p.done, 0));      // dependency mechanism
+        }
+        launch_ffn_gateup_gemm(h->u, perm, k, h->problems, i, j - i, max_rows, 0, I, H, h->act, I, wd, tensor, cs);
+        launch_ffn_down_gemm(h->act, I, h->problems, i, j - i, max_rows, 0, I, H, h->yexp, wd, tensor, cs);
+        // slots recycled inside the layer: fills that wait for a launch position in [i, j)
+        bool need_ev = false;
+        for (size_t q = dnext; q < deferred.size(); ++q) {
+          const int dep = cmd.need[7 * deferred[q] + 4];
+          if (dep < j) need_ev = true;
+        }
+        if (need_ev) {
+          cudaEvent_t ev = h->done_ev[i % h->done_ev.size()];
+          CKS(cudaEventRecord(ev, cs));
+          while (dnext < deferred.size() && cmd.need[7 * deferred[dnext] + 4] < j) {
+            rc = ce_issue_deferred(h, m, deferred[dnext], ev);
+            if (rc) return rc;
+            ++dnext;
+          }
+        }
+        i = j;
+      }
+      launch_combine(h->x, h->yexp, inv, gates, T, k, H, shared, sgate, h->x, cs);
+    }
+  }
+  // ---- last token: final norm + lm_head
+  launch_rmsnorm(h->x + (size_t)(T - 1) * H, h->final_norm, h->xf, 1, H, s.rms_eps, cs);
+  launch_gemv(h->xf, h->lm_head, h->logits, s.vocab, H, wd, 0, cs);
+  CKS(cudaEventRecord(h->step_end, cs));
+  int err_host = 0;
+  if (logits_out) CKS(cudaMemcpyAsync(logits_out, h->logits, (size_t)s.vocab * 4, cudaMemcpyDeviceToHost, cs));
+  CKS(cudaMemcpyAsync(&err_host, h->err_dev, 4, cudaMemcpyDeviceToHost, cs));
+  // keep feeding LOW chunks while the tail of the step drains (no-preempt mode may leave some queued)
+  while (cudaStreamQuery(cs) == cudaErrorNotReady) {
+    int rc = ce_pump_low(h);
+    if (rc) return rc;
+  }
+  CKS(cudaStreamSynchronize(cs));
+  float ms = 0.f;
+  CKS(cudaEventElapsedTime(&ms, h->step_start, h->step_end));
+  int rc = ce_retire(h, false);
+  if (rc) return rc;
+  h->st.steps++; h->st.tokens += (uint64_t)T;
+  h->st.step_ms += ms; h->st.last_step_ms = ms;
+  h->pos += T;
+  h->last_T = T;
+  if (err_host) {
+    h->st.timeouts++;
+    CKS(cudaMemsetAsync(h->err_dev, 0, 4, cs));
+    h->err = "an expert kernel timed out waiting for a chunk-ready flag";
+    return PROMOE_ETIMEOUT;
+  }
+  return PROMOE_OK;
+}
+
+extern "C" int promoe_prefill(promoe_t* h, const int32_t* ids_host, int32_t n_tokens, float* logits_out) {
+  if (!h) return PROMOE_EINVAL;
+  return run_step(h, ids_host, n_tokens, logits_out);
+}
+extern "C" int promoe_decode(promoe_t* h, int32_t token_id, float* logits_out) {
+  if (!h) return PROMOE_EINVAL;
+  return run_step(h, &token_id, 1, logits_out);
+}
