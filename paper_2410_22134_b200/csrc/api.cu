@@ -129,3 +129,26 @@ extern "C" int promoe_op_permute(const int32_t* sel, int32_t T, int32_t k, int32
   launch_permute(sel, T, k, E, count, offset, perm, inv, (cudaStream_t)stream);
   return launch_status();
 }
+
+extern "C" int promoe_op_expert_ffn(const float* x, const void* wg, const void* wu, const void* wd, float* act_ws,
+                                    float* y, void* prob_ws, int32_t T, int32_t H, int32_t I, int32_t wdtype,
+                                    int32_t path, int32_t reserved, void* stream) {
+  (void)reserved;
+  if (!x || !wg || !wu || !wd || !act_ws || !y || !prob_ws || T < 1 || H % 16 || I % 16 || (wdtype != 0 && wdtype != 1)) return PROMOE_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  FfnProblem pb{};
+  pb.wg = wg; pb.wu = wu; pb.wd = wd; pb.flags = nullptr; pb.gen = 0; pb.inter = I; pb.row0 = 0; pb.nrows = T; pb.expert = -1;
+  if (cudaMemcpyAsync(prob_ws, &pb, sizeof(pb), cudaMemcpyHostToDevice, st) != cudaSuccess) return PROMOE_ECUDA;
+  const FfnProblem* dp = (const FfnProblem*)prob_ws;
+  if (path == 0) path = (T == 1) ? 1 : 2;
+  if (path == 1) {
+    if (T != 1) return PROMOE_EINVAL;
+    launch_ffn_gateup_gemv(x, dp, 1, I, H, act_ws, I, wdtype, (size_t)1 << 20, nullptr, st);
+    launch_ffn_down_gemv(act_ws, I, dp, 1, I, H, y, wdtype, (size_t)1 << 20, nullptr, st);
+  } else if (path == 2 || path == 3) {
+    if (path == 3 && wdtype != 1) return PROMOE_EINVAL;
+    launch_ffn_gateup_gemm(x, nullptr, 1, dp, 0, 1, T, 0, I, H, act_ws, I, wdtype, path == 3, st);
+    launch_ffn_down_gemm(act_ws, I, dp, 0, 1, T, 0, I, H, y, wdtype, path == 3, st);
+  } else return PROMOE_EINVAL;
+  return launch_status();
+}

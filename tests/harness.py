@@ -1,0 +1,80 @@
+"""Side-by-side driver: the CUDA path (through the C-ABI binding) against the CPU oracle on the same seeded inputs.
+
+Used by the `-m gpu` parity tests, `__graft_entry__.smoke()` and nothing in the product.  Decode is teacher-forced
+with the ORACLE's greedy tokens (P1), or with seeded random ids.
+"""
+from __future__ import annotations
+
+from typing import Dict, List, Optional
+
+import numpy as np
+
+from oracle.cache_sim import ProMoECacheSim
+from oracle.compare import ParityReport, compare_cache, compare_stats, compare_step, oracle_step_matching
+from oracle.forward import OracleModel
+
+
+def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional[int] = None,
+               stride: Optional[int] = None, chunk_bytes: int = 0, predictor_mode: int = 1, flags: Optional[int] = None,
+               decode_ids: Optional[List[int]] = None, max_inflight: int = 0, warm: bool = True) -> Dict:
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+
+    s = cfg.shape
+    cache_slots = cfg.cache_slots if cache_slots is None else cache_slots
+    stride = cfg.stride if stride is None else stride
+    if flags is None:
+        flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | (B.F_WARM if warm else 0)
+    n_moe = s.n_layers - s.n_dense_layers
+    C = cache_slots // n_moe
+    eng = ProMoE(weights, cache_slots=cache_slots, stride=stride, chunk_bytes=chunk_bytes,
+                 predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight)
+    use_pred = predictor_mode == B.PRED_MLP
+    ora = OracleModel(weights, stride=stride, slots_per_layer=C, use_predictor=use_pred)
+    sim = ProMoECacheSim(n_moe, s.n_experts, C, warm=bool(flags & B.F_WARM))
+    rep = ParityReport()
+    all_logits = []
+    try:
+        ids = [int(x) for x in prompt]
+        T = len(ids)
+        logits = eng.prefill(ids)
+        tr = eng.trace(T)
+        st = oracle_step_matching(ora, ids, tr["sel"], rep)
+        compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred)
+        compare_cache(sim, tr, stride, use_pred)
+        all_logits.append(logits)
+        nxt = st.next_token
+        for i in range(decode_steps):
+            tok = int(decode_ids[i]) if decode_ids is not None else nxt
+            logits = eng.decode(tok)
+            tr = eng.trace(1)
+            st = oracle_step_matching(ora, [tok], tr["sel"], rep)
+            compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred)
+            compare_cache(sim, tr, stride, use_pred)
+            all_logits.append(logits)
+            nxt = st.next_token
+        stats = eng.stats()
+        compare_stats(sim, stats)
+        for m in range(n_moe):
+            assert eng.slots(m).tolist() == sim.slot_expert[m], f"final slot table of layer {m} differs"
+    finally:
+        eng.close()
+    return {"report": rep, "stats": stats, "logits": all_logits, "sim": sim}
+
+
+def run_gpu_only(cfg, weights, prompt, decode_ids, **kw) -> Dict:
+    """GPU-only run (no oracle): logits per step + stats, for the bitwise-invariance tests (P5)."""
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+
+    flags = kw.pop("flags", B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TRACE)
+    eng = ProMoE(weights, cache_slots=kw.pop("cache_slots", cfg.cache_slots), stride=kw.pop("stride", cfg.stride),
+                 flags=flags, **kw)
+    try:
+        out = [eng.prefill([int(x) for x in prompt])]
+        for t in decode_ids:
+            out.append(eng.decode(int(t)))
+        stats = eng.stats()
+    finally:
+        eng.close()
+    return {"logits": out, "stats": stats}

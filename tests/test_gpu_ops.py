@@ -1,0 +1,170 @@
+"""-m gpu: kernel-level parity of the micro entry points (C-ABI) against the oracle's pieces.
+
+Rows of SURVEY.md §8(a): A4 router/top-k/gates (bit-exact selections), A8 permutation (bit-exact), linear and
+A9 expert FFN (fp32 accumulate vs fp64: |err| <= 1e-4·scale, far inside north_star's 1e-2 tolerance).
+Sizes span several tiles and a ragged tail; edge cases: k = E, k = 1, exact ties, T = 1, empty expert groups.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2410_22134_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _w(shape, dtype, seed, std=None):
+    g = torch.Generator().manual_seed(seed)
+    t = torch.randn(shape, generator=g) * (std if std is not None else shape[-1] ** -0.5)
+    return t.to(dtype)
+
+
+@pytest.mark.parametrize("wdtype", [0, 1])
+@pytest.mark.parametrize("T,N,K,path", [(1, 60, 2048, 1), (1, 1000, 256, 1), (3, 77, 264, 1), (5, 60, 2048, 2),
+                                        (97, 200, 264, 2), (130, 64, 512, 2), (1, 8, 4096, 0), (64, 6144, 256, 0)])
+def test_op_linear(B, wdtype, T, N, K, path):
+    dt = torch.float32 if wdtype == 0 else torch.bfloat16
+    x = _w((T, K), torch.float32, 1, 1.0)
+    w = _w((N, K), dt, 2)
+    xd, wd = x.cuda(), w.cuda()
+    y = torch.full((T, N), float("nan"), device="cuda")
+    rc = B.lib().promoe_op_linear(xd.data_ptr(), wd.data_ptr(), y.data_ptr(), T, N, K, wdtype, path, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    ref = x.double() @ w.double().T
+    err = (y.cpu().double() - ref).abs().max().item()
+    assert err <= 1e-4 * max(1.0, ref.abs().max().item()), err
+
+
+@pytest.mark.parametrize("wdtype", [0, 1])
+@pytest.mark.parametrize("T,H,E,k,bias", [(1, 256, 8, 2, False), (33, 256, 8, 8, False), (1, 2048, 60, 4, False),
+                                          (130, 2048, 64, 6, True), (7, 512, 8, 1, False), (65, 264, 200, 16, True)])
+def test_op_route(B, wdtype, T, H, E, k, bias):
+    from oracle.forward import route
+    dt = torch.float32 if wdtype == 0 else torch.bfloat16
+    u = _w((T, H), torch.float32, 3, 1.0)
+    R = _w((E, H), dt, 4)
+    b = _w((E,), torch.float32, 5, 0.5) if bias else None
+    ud, Rd = u.cuda(), R.cuda()
+    bd = b.cuda() if bias else None
+    z = torch.empty((T, E), device="cuda")
+    sel = torch.empty((T, k), dtype=torch.int32, device="cuda")
+    gates = torch.empty((T, k), device="cuda")
+    margin = torch.empty((T,), device="cuda")
+    rc = B.lib().promoe_op_route(ud.data_ptr(), Rd.data_ptr(), bd.data_ptr() if bias else None, T, H, E, k, wdtype,
+                                 z.data_ptr(), sel.data_ptr(), gates.data_ptr(), margin.data_ptr(), None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    zo = u.double() @ R.double().T
+    if bias:
+        zo = zo + b.double()
+    assert (z.cpu().double() - zo).abs().max().item() <= 1e-4
+    near = 0
+    for t in range(T):
+        so, go, mo = route(zo[t], k)
+        sg = sel[t].tolist()
+        if sg != so:
+            assert mo < 1e-3 or min(abs(zo[t][a] - zo[t][b2]).item() for a, b2 in zip(so, so[1:])) < 1e-3
+            near += 1
+            continue
+        assert np.abs(np.asarray(go) - gates[t].cpu().numpy()).max() <= 1e-5
+        assert abs(gates[t].sum().item() - 1.0) <= 1e-5
+        if k < E:
+            assert abs(margin[t].item() - mo) <= 1e-4
+    assert near <= max(1, T // 20)
+
+
+def test_op_route_exact_ties(B):
+    """Constructed exact ties → lower expert index wins (north_star), on logits handed over through a one-hot u."""
+    E, H, k = 8, 16, 3
+    R = torch.zeros(E, H)
+    vals = [1.0, 2.0, 2.0, 0.5, 2.0, 1.0, 1.0, -1.0]       # three-way tie at 2.0, three-way at 1.0
+    for e, v in enumerate(vals):
+        R[e, 0] = v
+    u = torch.zeros(1, H); u[0, 0] = 1.0
+    z = torch.empty((1, E), device="cuda"); sel = torch.empty((1, k), dtype=torch.int32, device="cuda")
+    gates = torch.empty((1, k), device="cuda"); margin = torch.empty((1,), device="cuda")
+    ud, Rd = u.cuda(), R.cuda()
+    assert B.lib().promoe_op_route(ud.data_ptr(), Rd.data_ptr(), None, 1, H, E, k, 0, z.data_ptr(), sel.data_ptr(),
+                                   gates.data_ptr(), margin.data_ptr(), None) == 0
+    torch.cuda.synchronize()
+    assert sel[0].tolist() == [1, 2, 4]
+    assert margin[0].item() == pytest.approx(1.0)
+    k = 5
+    sel = torch.empty((1, k), dtype=torch.int32, device="cuda"); gates = torch.empty((1, k), device="cuda")
+    assert B.lib().promoe_op_route(ud.data_ptr(), Rd.data_ptr(), None, 1, H, E, k, 0, z.data_ptr(), sel.data_ptr(),
+                                   gates.data_ptr(), margin.data_ptr(), None) == 0
+    torch.cuda.synchronize()
+    assert sel[0].tolist() == [1, 2, 4, 0, 5]
+    assert margin[0].item() == 0.0
+
+
+@pytest.mark.parametrize("T,k,E,seed", [(1, 2, 8, 0), (32, 2, 8, 1), (96, 4, 60, 2), (1024, 6, 64, 3), (2048, 6, 64, 4),
+                                        (517, 2, 8, 5), (333, 16, 256, 6), (1500, 1, 3, 7)])
+def test_op_permute(B, T, k, E, seed):
+    from oracle.permute import permutation
+    g = torch.Generator().manual_seed(seed)
+    # distinct experts per token; skewed so that some groups are empty and some are large
+    scores = torch.rand(T, E, generator=g) + (torch.arange(E) % 5 == 0).float() * 0.5
+    if E > 4:
+        scores[:, 3] = -1.0        # expert 3 never selected → empty group
+    sel = torch.topk(scores, k, dim=1).indices.to(torch.int32)
+    sd = sel.cuda()
+    count = torch.empty(E, dtype=torch.int32, device="cuda"); offset = torch.empty(E + 1, dtype=torch.int32, device="cuda")
+    perm = torch.full((T * k,), -7, dtype=torch.int32, device="cuda"); inv = torch.full((T * k,), -7, dtype=torch.int32, device="cuda")
+    assert B.lib().promoe_op_permute(sd.data_ptr(), T, k, E, count.data_ptr(), offset.data_ptr(), perm.data_ptr(),
+                                     inv.data_ptr(), None) == 0
+    torch.cuda.synchronize()
+    c, o, p, i = permutation(sel.tolist(), E)
+    assert count.tolist() == c and offset.tolist() == o
+    assert perm.tolist() == p and inv.tolist() == i
+
+
+@pytest.mark.parametrize("wdtype", [0, 1])
+@pytest.mark.parametrize("T,H,I,path", [(1, 256, 512, 1), (1, 2048, 1408, 1), (37, 256, 512, 2), (130, 2048, 1408, 2),
+                                        (1, 4096, 14336, 1)])
+def test_op_expert_ffn(B, wdtype, T, H, I, path):
+    from oracle.forward import swiglu_ffn
+    dt = torch.float32 if wdtype == 0 else torch.bfloat16
+    x = _w((T, H), torch.float32, 7, 1.0)
+    wg, wu, wdn = _w((I, H), dt, 8), _w((I, H), dt, 9), _w((H, I), dt, 10)
+    xd, wgd, wud, wdd = x.cuda(), wg.cuda(), wu.cuda(), wdn.cuda()
+    act = torch.empty((T, I), device="cuda"); y = torch.full((T, H), float("nan"), device="cuda")
+    ws = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    rc = B.lib().promoe_op_expert_ffn(xd.data_ptr(), wgd.data_ptr(), wud.data_ptr(), wdd.data_ptr(), act.data_ptr(),
+                                      y.data_ptr(), ws.data_ptr(), T, H, I, wdtype, path, 0, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    ref = swiglu_ffn(x.double(), wg, wu, wdn)
+    err = (y.cpu().double() - ref).abs().max().item()
+    assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
+
+
+def test_bad_arguments(B):
+    L = B.lib()
+    assert L.promoe_op_linear(None, None, None, 1, 1, 8, 0, 0, None) == B.PROMOE_EINVAL
+    assert L.promoe_op_permute(None, 1, 1, 1, None, None, None, None, None) == B.PROMOE_EINVAL
+    sh = B.promoe_shape_t(n_layers=2, hidden=250, n_q_heads=4, n_kv_heads=4, head_dim=64, vocab=10, max_seq=8,
+                          n_experts=8, top_k=2, expert_inter=512, pred_hidden=128, wdtype=0)
+    with pytest.raises(B.PromoeError) as e:
+        B.promoe_create(sh, B.promoe_opts_t(cache_slots=8, stride=1))
+    assert e.value.code == B.PROMOE_EINVAL
+    sh.hidden = 256
+    with pytest.raises(B.PromoeError):
+        B.promoe_create(sh, B.promoe_opts_t(cache_slots=7, stride=1))      # not a multiple of n_moe_layers
+    with pytest.raises(B.PromoeError):
+        B.promoe_create(sh, B.promoe_opts_t(cache_slots=2, stride=1))      # fewer slots per layer than top_k
+    h = B.promoe_create(sh, B.promoe_opts_t(cache_slots=8, stride=1))
+    with pytest.raises(B.PromoeError) as e:
+        B.promoe_decode(h, 0, None)                                         # decode before load
+    assert e.value.code == B.PROMOE_ESTATE
+    B.promoe_destroy(h)

@@ -1,0 +1,28 @@
+"""CPU: the C-ABI library builds/loads and exports every symbol include/promoe.h declares (no compute calls)."""
+import os
+import re
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_header_symbols_are_exported():
+    from paper_2410_22134_b200.build import build
+    build()
+    from paper_2410_22134_b200 import binding
+    hdr = open(os.path.join(ROOT, "include", "promoe.h")).read()
+    declared = sorted(set(re.findall(r"PROMOE_API [\w\s\*]*?(promoe_\w+)\(", hdr)))
+    assert len(declared) >= 17
+    L = binding.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert sorted(binding.EXPORTS) == declared
+
+
+def test_struct_layouts_match_header():
+    import ctypes
+    from paper_2410_22134_b200 import binding as B
+    # sizes computed from the header's field lists (all int32/float/uint64/double/pointers, natural alignment)
+    assert ctypes.sizeof(B.promoe_shape_t) == 17 * 4 + 2 * 4
+    assert ctypes.sizeof(B.promoe_opts_t) == 40
+    assert ctypes.sizeof(B.promoe_dense_t) == 15 * 8
+    assert ctypes.sizeof(B.promoe_stats_t) == 19 * 8 + 3 * 8 + 8
