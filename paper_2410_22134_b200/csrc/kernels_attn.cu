@@ -58,18 +58,24 @@ __global__ void __launch_bounds__(128) attn_decode_kernel(const float* __restric
   float m = -INFINITY, l = 0.f, o[PER];
 #pragma unroll
   for (int i = 0; i < PER; ++i) o[i] = 0.f;
-  for (int p = p0 + grp; p < p1; p += 16) {
-    const float4* kr = reinterpret_cast<const float4*>(kb + (size_t)p * D + sub * PER);
+  // uniform trip count per CTA: the 8-lane shuffles below use the full-warp mask, so no lane may leave early
+  for (int pb = p0; pb < p1; pb += 16) {
+    const int p = pb + grp;
+    const bool valid = p < p1;
     float s = 0.f;
+    if (valid) {
+      const float4* kr = reinterpret_cast<const float4*>(kb + (size_t)p * D + sub * PER);
 #pragma unroll
-    for (int i = 0; i < PER / 4; ++i) {
-      float4 kv = __ldcs(kr + i);
-      s = fmaf(q[4 * i], kv.x, s); s = fmaf(q[4 * i + 1], kv.y, s);
-      s = fmaf(q[4 * i + 2], kv.z, s); s = fmaf(q[4 * i + 3], kv.w, s);
+      for (int i = 0; i < PER / 4; ++i) {
+        float4 kv = __ldcs(kr + i);
+        s = fmaf(q[4 * i], kv.x, s); s = fmaf(q[4 * i + 1], kv.y, s);
+        s = fmaf(q[4 * i + 2], kv.z, s); s = fmaf(q[4 * i + 3], kv.w, s);
+      }
     }
     s += __shfl_xor_sync(0xffffffffu, s, 1);
     s += __shfl_xor_sync(0xffffffffu, s, 2);
     s += __shfl_xor_sync(0xffffffffu, s, 4);
+    if (!valid) continue;
     const float mn = fmaxf(m, s);
     const float corr = expf(m - mn), pw = expf(s - mn);
     l = l * corr + pw;
