@@ -160,6 +160,12 @@ PROMOE_API int promoe_get_slots(promoe_t* h, int32_t moe_layer, int32_t* slot_ex
  * (chunk size is chosen from this curve).  Allocates and frees its own buffers. */
 PROMOE_API int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out);
 
+/* Live kernel timing for bench.py's roofline: runs `reps` launches of one hot kernel of the decode step on the
+ * compute stream, bracketed by CUDA events, over RESIDENT slots rotating through all layers (working set = the
+ * whole slot region, far larger than L2).  which: 0 = A9 gate/up SwiGLU GEMV over top_k experts, 1 = A9 down GEMV
+ * over top_k experts.  Outputs the average launch duration and the algorithmic weight bytes one launch streams. */
+PROMOE_API int promoe_kernel_time(promoe_t* h, int32_t which, int32_t reps, double* avg_ms_out, double* bytes_per_launch_out);
+
 /* Micro entry points: single hot-path steps on caller-provided DEVICE buffers (used by kernel-level parity
  * tests and bench.py's per-kernel roofline).  stream = cudaStream_t or NULL (default stream).
  * All are asynchronous on `stream`. */

@@ -24,7 +24,7 @@ EXPORTS = [
     "promoe_create", "promoe_destroy", "promoe_last_error", "promoe_load_dense", "promoe_load_experts",
     "promoe_prefill", "promoe_decode", "promoe_set_prediction_trace", "promoe_stats", "promoe_get_trace",
     "promoe_reset", "promoe_get_slots", "promoe_measure_h2d", "promoe_op_linear", "promoe_op_route",
-    "promoe_op_permute", "promoe_op_expert_ffn",
+    "promoe_op_permute", "promoe_op_expert_ffn", "promoe_kernel_time",
 ]
 
 
@@ -95,6 +95,7 @@ def lib() -> C.CDLL:
     L.promoe_op_route.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_permute.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_expert_ffn.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
+    L.promoe_kernel_time.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     for n in EXPORTS:
         f = getattr(L, n)
         if n not in ("promoe_destroy", "promoe_last_error"):
@@ -170,3 +171,10 @@ def promoe_measure_h2d(nbytes: int, depth: int = 2, reps: int = 5) -> float:
     g = C.c_double()
     _check(lib().promoe_measure_h2d(nbytes, depth, reps, C.byref(g)))
     return g.value
+
+
+def promoe_kernel_time(h, which: int, reps: int = 200):
+    """(average launch ms, algorithmic bytes per launch) of decode kernel `which` over resident slots."""
+    ms, nb = C.c_double(), C.c_double()
+    _check(lib().promoe_kernel_time(h, which, reps, C.byref(ms), C.byref(nb)), h)
+    return ms.value, nb.value
