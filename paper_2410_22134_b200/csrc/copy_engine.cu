@@ -42,7 +42,7 @@ int ce_retire(promoe_t* h, bool all) {
     if (q != cudaSuccess) { h->err = std::string("copy event: ") + cudaGetErrorString(q); return PROMOE_ECUDA; }
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, h->ev_ring_start[i], h->ev_ring[i]) == cudaSuccess) h->st.copy_busy_ms += ms;
-    if (h->ev_is_low[i]) h->low_inflight--;
+    if (h->ev_is_low[i]) h->low_inflight--; else h->high_inflight--;
     h->ev_tail++;
   }
   return PROMOE_OK;
@@ -88,18 +88,21 @@ static int issue_chunks(promoe_t* h, int m, int s, int c0, int c1, bool low) {
   }
   CKC(cudaEventRecord(h->ev_ring[ri], h->ps));
   h->ev_is_low[ri] = low ? 1 : 0;
-  if (low) h->low_inflight++;
+  if (low) h->low_inflight++; else h->high_inflight++;
   h->ev_head++;
   p.issued = c1;
   if (c1 == h->n_chunks) { CKC(cudaEventRecord(p.done, h->ps)); p.done_valid = true; }
   return PROMOE_OK;
 }
 
-// LOW queue: feed the copy stream while fewer than max_inflight LOW chunks are in flight.
+// LOW queue ("low-priority tasks are only executed when there are no high-priority tasks"): feed the copy
+// stream only while no HIGH fill is outstanding on it, and keep at most max_inflight LOW chunks in flight so that a
+// HIGH chunk arriving later waits for at most that many (bounded preemption delay).  On a B200 every bf16
+// config is H2D-bound, so a LOW byte may only ever use link time that would otherwise idle.
 int ce_pump_low(promoe_t* h) {
   int rc = ce_retire(h, false);
   if (rc) return rc;
-  while (!h->low.empty() && h->low_inflight < h->max_inflight) {
+  while (!h->low.empty() && h->low_inflight < h->max_inflight && (h->high_inflight == 0 || !h->low_yields)) {
     FillJob j = h->low.front();
     SlotPhys& p = h->phys[(size_t)j.layer * h->C + j.slot];
     if (p.gen != j.gen || p.expert != j.expert || p.issued >= h->n_chunks) { h->low.pop_front(); continue; }  // stale / done

@@ -29,6 +29,7 @@ static cudaError_t dalloc(T** p, size_t n) {
 }
 
 int promoe_init_cache_state(promoe_t* h, bool copy_warm);  // below
+int ce_retire(promoe_t* h, bool all);
 
 extern "C" const char* promoe_last_error(const promoe_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 
@@ -217,6 +218,7 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
   CK(cudaMemset(h->err_dev, 0, 4));
   h->mirror = se;
   h->low.clear();
+  if (ce_retire(h, true)) return PROMOE_ECUDA;
   for (size_t i = 0; i < h->phys.size(); ++i) {
     SlotPhys& p = h->phys[i];
     p.gen = 0; p.expert = se[i]; p.issued = warm ? h->n_chunks : 0; p.done_valid = false;

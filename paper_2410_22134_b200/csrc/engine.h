@@ -78,7 +78,8 @@ struct promoe {
   std::vector<cudaEvent_t> ev_ring_start;
   size_t ev_head = 0, ev_tail = 0;        // in flight = [tail, head)
   std::vector<int> ev_is_low;
-  int low_inflight = 0;
+  int low_inflight = 0, high_inflight = 0;
+  bool low_yields = true;             // LOW chunks wait while HIGH fills are outstanding
   std::vector<cudaEvent_t> done_ev;       // prefill: per launch position "expert finished" events
   cudaEvent_t step_start = nullptr, step_end = nullptr;
 
