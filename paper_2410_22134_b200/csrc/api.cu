@@ -1,5 +1,6 @@
 // api.cu — trace getters, injected prediction lists and the micro entry points of include/promoe.h.
 #include "engine.h"
+#include "gemm_tc.h"
 
 #include <cstring>
 
@@ -102,9 +103,22 @@ extern "C" int promoe_op_linear(const float* x, const void* w, float* y, int32_t
     for (int t = 0; t < T; ++t) launch_gemv(x + (size_t)t * K, w, y + (size_t)t * N, N, K, wdtype, 0, st);
   } else if (path == 2) {
     launch_gemm_simt(x, w, y, T, N, K, wdtype, 0, st);
-  } else if (path == 3) {
+  } else if (path == 3) {   // tcgen05 (test entry: allocates scratch and synchronises)
     if (wdtype != 1) return PROMOE_EINVAL;
-    launch_linear_gemm(x, w, y, T, N, K, wdtype, 0, true, st);
+    TcContext* tc = tc_create(nullptr);
+    if (!tc) return PROMOE_ECUDA;
+    __nv_bfloat16* sp = nullptr;
+    int rc = PROMOE_ECUDA;
+    if (cudaMalloc((void**)&sp, (size_t)2 * T * K * 2) == cudaSuccess) {
+      launch_split_rows(x, nullptr, 1, T, K, sp, (size_t)T * K, st);
+      TcGemm g;
+      g.a0 = w; g.a_rows = N; g.b_hi = sp; g.b_lo_off = (size_t)T * K; g.b_rows_cap = T; g.K = K; g.N = N; g.rows = T;
+      g.y = y; g.ldy = N;
+      if (tc_launch(tc, g, st, nullptr) && cudaStreamSynchronize(st) == cudaSuccess) rc = PROMOE_OK;
+      cudaFree(sp);
+    }
+    tc_destroy(tc);
+    return rc == PROMOE_OK ? launch_status() : rc;
   } else return PROMOE_EINVAL;
   return launch_status();
 }
@@ -145,10 +159,29 @@ extern "C" int promoe_op_expert_ffn(const float* x, const void* wg, const void* 
     if (T != 1) return PROMOE_EINVAL;
     launch_ffn_gateup_gemv(x, dp, 1, I, H, act_ws, I, wdtype, (size_t)1 << 20, nullptr, st);
     launch_ffn_down_gemv(act_ws, I, dp, 1, I, H, y, wdtype, (size_t)1 << 20, nullptr, st);
-  } else if (path == 2 || path == 3) {
-    if (path == 3 && wdtype != 1) return PROMOE_EINVAL;
-    launch_ffn_gateup_gemm(x, nullptr, 1, dp, 0, 1, T, 0, I, H, act_ws, I, wdtype, path == 3, st);
-    launch_ffn_down_gemm(act_ws, I, dp, 0, 1, T, 0, I, H, y, wdtype, path == 3, st);
+  } else if (path == 2) {
+    launch_ffn_gateup_gemm_simt(x, nullptr, 1, dp, 0, 1, T, 0, I, H, act_ws, I, wdtype, st);
+    launch_ffn_down_gemm_simt(act_ws, I, dp, 0, 1, T, 0, I, H, y, wdtype, st);
+  } else if (path == 3) {   // tcgen05 (test entry: allocates scratch and synchronises)
+    if (wdtype != 1) return PROMOE_EINVAL;
+    TcContext* tc = tc_create(nullptr);
+    if (!tc) return PROMOE_ECUDA;
+    __nv_bfloat16 *s1 = nullptr, *s2 = nullptr;
+    int rc = PROMOE_ECUDA;
+    if (cudaMalloc((void**)&s1, (size_t)2 * T * H * 2) == cudaSuccess && cudaMalloc((void**)&s2, (size_t)2 * T * I * 2) == cudaSuccess) {
+      launch_split_rows(x, nullptr, 1, T, H, s1, (size_t)T * H, st);
+      TcGemm g;
+      g.a0 = wg; g.a1 = wu; g.a_rows = I; g.b_hi = s1; g.b_lo_off = (size_t)T * H; g.b_rows_cap = T; g.K = H; g.N = I; g.rows = T;
+      g.swiglu = true; g.o_hi = s2; g.o_lo_off = (size_t)T * I; g.ldo = I;
+      TcGemm d;
+      d.a0 = wd; d.a_rows = H; d.b_hi = s2; d.b_lo_off = (size_t)T * I; d.b_rows_cap = T; d.K = I; d.N = H; d.rows = T;
+      d.y = y; d.ldy = H;
+      if (tc_launch(tc, g, st, nullptr) && tc_launch(tc, d, st, nullptr) && cudaStreamSynchronize(st) == cudaSuccess) rc = PROMOE_OK;
+    }
+    if (s1) cudaFree(s1);
+    if (s2) cudaFree(s2);
+    tc_destroy(tc);
+    return rc == PROMOE_OK ? launch_status() : rc;
   } else return PROMOE_EINVAL;
   return launch_status();
 }

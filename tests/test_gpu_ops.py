@@ -168,3 +168,37 @@ def test_bad_arguments(B):
         B.promoe_decode(h, 0, None)                                         # decode before load
     assert e.value.code == B.PROMOE_ESTATE
     B.promoe_destroy(h)
+
+
+# ---- tcgen05 / TMEM / TMA path (bf16 weights, activations as a bf16 hi/lo pair; G1) ---------------------
+@pytest.mark.parametrize("T,N,K", [(64, 128, 64), (1, 128, 128), (5, 60, 2048), (130, 6144, 2048), (97, 200, 264),
+                                   (512, 2048, 1408), (63, 512, 2048)])
+def test_op_linear_tcgen05(B, T, N, K):
+    x = _w((T, K), torch.float32, 11, 1.0)
+    w = _w((N, K), torch.bfloat16, 12)
+    xd, wd = x.cuda(), w.cuda()
+    y = torch.full((T, N), float("nan"), device="cuda")
+    rc = B.lib().promoe_op_linear(xd.data_ptr(), wd.data_ptr(), y.data_ptr(), T, N, K, 1, 3, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    ref = x.double() @ w.double().T
+    err = (y.cpu().double() - ref).abs().max().item()
+    # hi/lo split: |x - hi - lo| <= 2^-17 |x| per element → ~1e-5 relative on the dot product
+    assert err <= 1e-4 * max(1.0, ref.abs().max().item()), err
+
+
+@pytest.mark.parametrize("T,H,I", [(37, 256, 512), (130, 2048, 1408), (64, 4096, 14336), (1, 256, 512)])
+def test_op_expert_ffn_tcgen05(B, T, H, I):
+    from oracle.forward import swiglu_ffn
+    x = _w((T, H), torch.float32, 7, 1.0)
+    wg, wu, wdn = _w((I, H), torch.bfloat16, 8), _w((I, H), torch.bfloat16, 9), _w((H, I), torch.bfloat16, 10)
+    xd, wgd, wud, wdd = x.cuda(), wg.cuda(), wu.cuda(), wdn.cuda()
+    act = torch.empty((T, I), device="cuda"); y = torch.full((T, H), float("nan"), device="cuda")
+    ws = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    rc = B.lib().promoe_op_expert_ffn(xd.data_ptr(), wgd.data_ptr(), wud.data_ptr(), wdd.data_ptr(), act.data_ptr(),
+                                      y.data_ptr(), ws.data_ptr(), T, H, I, 1, 3, 0, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    ref = swiglu_ffn(x.double(), wg, wu, wdn)
+    err = (y.cpu().double() - ref).abs().max().item()
+    assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
