@@ -1,9 +1,11 @@
 // engine.cu — promoe_create / load / reset / destroy: shapes, buffers, the contiguous slot region,
 // slot-table state, streams.  The step scheduler is in step.cu, the copy engine in copy_engine.cu.
 #include "engine.h"
+#include "gemm_tc.h"
 
 #include <cuda.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -85,6 +87,16 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->pred_list, (size_t)Lm * (1 + E))); CK(dalloc(&h->trace_precise, (size_t)Lm * (1 + 5 * E)));
     CK(dalloc(&h->trace_pred, (size_t)Lm * (1 + 4 * E))); CK(dalloc(&h->row_of, (size_t)k)); CK(dalloc(&h->n_prob, (size_t)1));
     CK(dalloc(&h->problems, (size_t)E)); CK(dalloc(&h->shared_prob, (size_t)L)); CK(dalloc(&h->err_dev, (size_t)1));
+    if ((op->flags & PROMOE_F_TENSOR) && s.wdtype == 1) {
+      h->tc = tc_create(&h->err);
+      if (!h->tc) return PROMOE_ECUDA;
+      auto up8 = [](size_t v) { return (v + 7) & ~(size_t)7; };
+      const size_t ka = (size_t)std::max(std::max(H, s.n_q_heads * s.head_dim), s.pred_hidden);
+      h->xsA_half = up8((size_t)T * ka);
+      h->xsG_half = up8((size_t)T * k * H);
+      h->xsB_half = up8(std::max((size_t)T * k * s.expert_inter, (size_t)T * h->ffn_w));
+      CK(dalloc(&h->xsA, 2 * h->xsA_half)); CK(dalloc(&h->xsG, 2 * h->xsG_half)); CK(dalloc(&h->xsB, 2 * h->xsB_half));
+    }
     // RoPE tables in double (reading G11): angle = pos * theta^(-2i/d)
     {
       const int half = s.head_dim / 2;
@@ -146,6 +158,10 @@ extern "C" void promoe_destroy(promoe_t* h) {
                   h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->slots, h->flags,
                   h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock};
   for (void* b : bufs) if (b) cudaFree(b);
+  if (h->xsA) cudaFree(h->xsA);
+  if (h->xsG) cudaFree(h->xsG);
+  if (h->xsB) cudaFree(h->xsB);
+  if (h->tc) tc_destroy(h->tc);
   if (h->cmd_host) cudaFreeHost((void*)h->cmd_host);
   if (h->flagsrc_host) cudaFreeHost(h->flagsrc_host);
   for (auto& p : h->phys) if (p.done) cudaEventDestroy(p.done);

@@ -1,5 +1,6 @@
 // engine.h — the promoe handle: device buffers, slot region, copy engine state.  Internal to the library.
 #pragma once
+#include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
 #include <deque>
@@ -10,6 +11,7 @@
 #include "kernels.h"
 
 namespace pmk {
+struct TcContext;
 
 // One expert fill = all chunks of one expert image into one slot (Alg. 1: tasks of one expert, in chunk order).
 struct FillJob {
@@ -60,6 +62,11 @@ struct promoe {
           *n_prob = nullptr;
   pmk::FfnProblem *problems = nullptr, *shared_prob = nullptr;
   int* err_dev = nullptr;
+  // tcgen05 path (PROMOE_F_TENSOR, bf16 weights): activation operands as bf16 hi/lo planes; the lo plane of each
+  // buffer starts *_half elements after the hi plane
+  pmk::TcContext* tc = nullptr;
+  __nv_bfloat16 *xsA = nullptr, *xsG = nullptr, *xsB = nullptr;   // direct rows | gathered rows | SwiGLU outputs
+  size_t xsA_half = 0, xsG_half = 0, xsB_half = 0;
 
   // expert cache
   uint8_t* slots = nullptr;       // ONE contiguous region [Lm, C, Be]

@@ -89,17 +89,6 @@ void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src
 void launch_ffn_down_gemm_simt(const float* act, int act_stride, const FfnProblem* probs, int p0, int np,
                                int max_rows, int rows_override, int max_inter, int H, float* y, int wdtype, cudaStream_t st);
 
-// Dispatchers used by the step scheduler: tcgen05 tensor-core path (bf16 weights, `tensor` set, shape supported)
-// or the SIMT fp32 path.
-void launch_linear_gemm(const float* x, const void* w, float* y, int T, int N, int K, int wdtype, int flags,
-                        bool tensor, cudaStream_t st);
-void launch_ffn_gateup_gemm(const float* x, const int32_t* row_src, int src_div, const FfnProblem* probs, int p0,
-                            int np, int max_rows, int rows_override, int max_inter, int H, float* act,
-                            int act_stride, int wdtype, bool tensor, cudaStream_t st);
-void launch_ffn_down_gemm(const float* act, int act_stride, const FfnProblem* probs, int p0, int np, int max_rows,
-                          int rows_override, int max_inter, int H, float* y, int wdtype, bool tensor,
-                          cudaStream_t st);
-
 // A10 combine: out[t,:] = hres[t,:] + sum_j (fixed j order) g[t,j] * yexp[row(t,j),:] (+ sgate[t]*shared[t,:]).
 //  row(t,j) = inv[t*k+j] (prefill) or pos_of_j[j] (decode).  shared may be nullptr; sgate nullptr => 1.
 void launch_combine(const float* hres, const float* yexp, const int32_t* row_of, const float* gates, int T, int k,

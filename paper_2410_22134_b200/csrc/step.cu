@@ -15,6 +15,7 @@
 //                A10 combine in fixed j order + shared + residual
 //   final norm + lm_head on the last token.
 #include "engine.h"
+#include "gemm_tc.h"
 
 #include <cstring>
 
@@ -35,31 +36,79 @@ int ce_issue_deferred(promoe_t* h, int m, int i, cudaEvent_t after);
     }                                                                                              \
   } while (0)
 
-// y[T,N] (+)= x[T,K]·W^T on the compute stream: GEMV for one token, GEMM otherwise.
-static void linear(promoe_t* h, const float* x, const void* w, float* y, int T, int N, int K, int flags) {
-  if (T == 1) launch_gemv(x, w, y, N, K, h->s.wdtype, flags, h->cs);
-  else launch_linear_gemm(x, w, y, T, N, K, h->s.wdtype, flags, (h->o.flags & PROMOE_F_TENSOR) != 0, h->cs);
+static bool use_tc(const promoe_t* h, int T) { return T > 1 && h->tc != nullptr && h->s.wdtype == 1; }
+
+// fp32 rows of x → bf16 hi/lo planes in xsA (the activation operand of the tcgen05 GEMMs, reading G1)
+static void split_A(promoe_t* h, const float* x, int T, int K) {
+  launch_split_rows(x, nullptr, 1, T, K, h->xsA, h->xsA_half, h->cs);
+}
+
+// y[T,N] (+)= x[T,K]·W^T on the compute stream: GEMV for one token; T > 1: tcgen05 GEMM (bf16 weights) or SIMT.
+// presplit: xsA already holds the hi/lo split of x.
+static int linear(promoe_t* h, const float* x, const void* w, float* y, int T, int N, int K, int flags, bool presplit = false) {
+  if (T == 1) { launch_gemv(x, w, y, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
+  if (!use_tc(h, T) || N < 16) { launch_gemm_simt(x, w, y, T, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
+  if (!presplit) split_A(h, x, T, K);
+  TcGemm g;
+  g.a0 = w; g.a_rows = N; g.b_hi = h->xsA; g.b_lo_off = h->xsA_half; g.b_rows_cap = (int)(h->xsA_half / K);
+  g.K = K; g.N = N; g.rows = T; g.y = y; g.ldy = N; g.flags = flags;
+  return tc_launch(h->tc, g, h->cs, &h->err) ? PROMOE_OK : PROMOE_ECUDA;
 }
 
 // SwiGLU FFN of an always-resident MLP (shared expert / dense layer) for all T rows of u → h->sy.
-static void resident_ffn(promoe_t* h, int l, int inter, int T) {
+// T > 1 with tensor cores: expects the split of u in xsA.
+static int resident_ffn(promoe_t* h, int l, int inter, int T) {
   const int H = h->s.hidden, wd = h->s.wdtype;
   if (T == 1) {
     launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs);
     launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs);
+  } else if (!use_tc(h, T)) {
+    launch_ffn_gateup_gemm_simt(h->u, nullptr, 1, h->shared_prob, l, 1, T, T, inter, H, h->sact, h->ffn_w, wd, h->cs);
+    launch_ffn_down_gemm_simt(h->sact, h->ffn_w, h->shared_prob, l, 1, T, T, inter, H, h->sy, wd, h->cs);
   } else {
-    launch_ffn_gateup_gemm(h->u, nullptr, 1, h->shared_prob, l, 1, T, T, inter, H, h->sact, h->ffn_w, wd,
-                           (h->o.flags & PROMOE_F_TENSOR) != 0, h->cs);
-    launch_ffn_down_gemm(h->sact, h->ffn_w, h->shared_prob, l, 1, T, T, inter, H, h->sy, wd,
-                         (h->o.flags & PROMOE_F_TENSOR) != 0, h->cs);
+    TcGemm g;
+    g.a0 = h->ffn_gate[l]; g.a1 = h->ffn_up[l]; g.a_rows = inter;
+    g.b_hi = h->xsA; g.b_lo_off = h->xsA_half; g.b_rows_cap = (int)(h->xsA_half / H);
+    g.K = H; g.N = inter; g.rows = T; g.swiglu = true;
+    g.o_hi = h->xsB; g.o_lo_off = h->xsB_half; g.ldo = inter;
+    TcGemm d;
+    d.a0 = h->ffn_down[l]; d.a_rows = H; d.b_hi = h->xsB; d.b_lo_off = h->xsB_half; d.b_rows_cap = (int)(h->xsB_half / inter);
+    d.K = inter; d.N = H; d.rows = T; d.y = h->sy; d.ldy = H;
+    if (!tc_launch(h->tc, g, h->cs, &h->err) || !tc_launch(h->tc, d, h->cs, &h->err)) return PROMOE_ECUDA;
   }
+  return PROMOE_OK;
 }
+
+// Routed experts [i, j) of the problem table (prefill): grouped SwiGLU FFN over their row ranges → yexp.
+static int expert_batch(promoe_t* h, const int32_t* perm, int i, int j, int max_rows) {
+  const promoe_shape_t& s = h->s;
+  const int H = s.hidden, I = s.expert_inter, k = s.top_k;
+  if (!use_tc(h, 2)) {
+    launch_ffn_gateup_gemm_simt(h->u, perm, k, h->problems, i, j - i, max_rows, 0, I, H, h->act, I, s.wdtype, h->cs);
+    launch_ffn_down_gemm_simt(h->act, I, h->problems, i, j - i, max_rows, 0, I, H, h->yexp, s.wdtype, h->cs);
+    return PROMOE_OK;
+  }
+  const int n_slots = h->Lm * h->C;
+  TcGemm g;   // gate | up rows of the slot images: one 3-D tensor map over the whole slot region
+  g.a0 = h->slots; g.a1 = h->slots; g.a_rows = 2 * I; g.a1_row_off = I; g.a_batches = n_slots; g.a_batch_stride = h->Be;
+  g.b_hi = h->xsG; g.b_lo_off = h->xsG_half; g.b_rows_cap = (int)(h->xsG_half / H);
+  g.K = H; g.N = I; g.probs = h->problems; g.p0 = i; g.np = j - i; g.max_rows = max_rows; g.slot_base = h->slots;
+  g.swiglu = true; g.o_hi = h->xsB; g.o_lo_off = h->xsB_half; g.ldo = I;
+  TcGemm d;   // down rows
+  d.a0 = h->slots + (size_t)2 * H * I * h->wb; d.a_rows = H; d.a_batches = n_slots; d.a_batch_stride = h->Be;
+  d.b_hi = h->xsB; d.b_lo_off = h->xsB_half; d.b_rows_cap = (int)(h->xsB_half / I);
+  d.K = I; d.N = H; d.probs = h->problems; d.p0 = i; d.np = j - i; d.max_rows = max_rows; d.slot_base = h->slots;
+  d.y = h->yexp; d.ldy = H;
+  if (!tc_launch(h->tc, g, h->cs, &h->err) || !tc_launch(h->tc, d, h->cs, &h->err)) return PROMOE_ECUDA;
+  return PROMOE_OK;
+}
+
+#define RC(expr) do { int rc_ = (expr); if (rc_ != PROMOE_OK) return rc_; } while (0)
 
 static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_out) {
   const promoe_shape_t& s = h->s;
   const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter;
   const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = s.wdtype;
-  const bool tensor = (h->o.flags & PROMOE_F_TENSOR) != 0;
   if (!h->dense_loaded || !h->experts_loaded) { h->err = "step before load_dense / load_experts"; return PROMOE_ESTATE; }
   if (T < 1 || !ids_host) { h->err = "step: no tokens"; return PROMOE_EINVAL; }
   if (h->pos + T > s.max_seq) { h->err = "step: sequence exceeds max_seq"; return PROMOE_ESTATE; }
@@ -89,16 +138,18 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
   for (int l = 0; l < s.n_layers; ++l) {
     // ---- attention block (A1-A3)
     launch_rmsnorm(h->x, h->ln1[l], h->u1, T, H, s.rms_eps, cs);
-    linear(h, h->u1, h->wqkv[l], h->qkv, T, h->qkv_w, H, 0);
+    RC(linear(h, h->u1, h->wqkv[l], h->qkv, T, h->qkv_w, H, 0));
     float* kc = h->kcache + (size_t)l * kv_layer;
     float* vc = h->vcache + (size_t)l * kv_layer;
     launch_rope_append(h->qkv, h->cos_t, h->sin_t, kc, vc, T, pos0, nq, nkv, d, s.max_seq, cs);
     if (T == 1) launch_attn_decode(h->qkv, kc, vc, h->attn, h->attn_ws, pos0 + 1, nq, nkv, d, s.max_seq, h->nsplit, cs);
     else launch_attn_prefill(h->qkv, kc, vc, h->attn, T, pos0, nq, nkv, d, s.max_seq, cs);
-    linear(h, h->attn, h->wo[l], h->x, T, H, nq * d, LIN_ACC);
+    RC(linear(h, h->attn, h->wo[l], h->x, T, H, nq * d, LIN_ACC));
     launch_rmsnorm(h->x, h->ln2[l], h->u, T, H, s.rms_eps, cs);
+    const bool tc = use_tc(h, T);
+    if (tc) split_A(h, h->u, T, H);   // u feeds the router, predictor, shared-expert and dense GEMMs
     if (l < s.n_dense_layers) {
-      resident_ffn(h, l, s.dense_inter, T);
+      RC(resident_ffn(h, l, s.dense_inter, T));
       launch_add(h->x, h->sy, h->x, (size_t)T * H, cs);
       continue;
     }
@@ -110,13 +161,15 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     int32_t* perm = h->perm + (size_t)m * h->maxT * k;
     int32_t* inv = h->inv + (size_t)m * h->maxT * k;
     int32_t* offset = h->offset + (size_t)m * (E + 1);
-    linear(h, h->u, h->router[l], h->zraw, T, E, H, 0);                               // A4
+    RC(linear(h, h->u, h->router[l], h->zraw, T, E, H, 0, tc));                             // A4
     launch_topk_gate(h->zraw, s.router_bias ? h->router_bias[l] : nullptr, T, E, k, h->z + (size_t)m * h->maxT * E, sel,
                      gates, h->margin + (size_t)m * h->maxT, cs);
     int32_t* plist = nullptr;
     if (h->o.predictor_mode == PROMOE_PRED_MLP) {                                      // A5
-      linear(h, h->u, h->pred_w1[l], h->p1, T, s.pred_hidden, H, LIN_RELU);
-      linear(h, h->p1, h->pred_w2[l], h->p2, T, E, s.pred_hidden, 0);
+      RC(linear(h, h->u, h->pred_w1[l], h->p1, T, s.pred_hidden, H, LIN_RELU, tc));
+      // W2 is tiny (E x ph): SIMT for T > 1, which also leaves the split of u in xsA for the shared expert
+      if (T == 1) launch_gemv(h->p1, h->pred_w2[l], h->p2, E, s.pred_hidden, wd, 0, cs);
+      else launch_gemm_simt(h->p1, h->pred_w2[l], h->p2, T, E, s.pred_hidden, wd, 0, cs);
       plist = h->pred_list + (size_t)m * (1 + E);
       launch_pred_list(h->p2, T, E, k, C, plist, cs);
     } else if (h->o.predictor_mode == PROMOE_PRED_TRACE) {
@@ -131,9 +184,9 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     const float* shared = nullptr;
     const float* sgate = nullptr;
     if (s.n_shared_inter) {                                                            // A10 shared expert first
-      resident_ffn(h, l, s.n_shared_inter, T);
+      RC(resident_ffn(h, l, s.n_shared_inter, T));
       shared = h->sy;
-      if (s.shared_gate) { linear(h, h->u, h->shared_gate_w[l], h->sgate, T, 1, H, 0); sgate = h->sgate; }
+      if (s.shared_gate) { RC(linear(h, h->u, h->shared_gate_w[l], h->sgate, T, 1, H, 0)); sgate = h->sgate; }
     }
     // ---- A7: hand-over to the copy engine
     int rc = ce_wait_cmd(h, m, seq);
@@ -149,6 +202,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
       launch_ffn_down_gemv(h->act, I, h->problems, n, I, H, h->yexp, wd, h->chunk_bytes, h->err_dev, cs);
       launch_combine(h->x, h->yexp, h->row_of, gates, 1, k, H, shared, sgate, h->x, cs);
     } else {
+      if (tc) launch_split_rows(h->u, perm, k, T * k, H, h->xsG, h->xsG_half, cs);   // gathered rows, permuted order
       // batches: [all class A] [all class B] then every class C alone (its fill lands in copy order)
       int i = 0;
       size_t dnext = 0;
@@ -162,8 +216,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
           SlotPhys& p = h->phys[(size_t)m * C + cmd.need[7 * q + 2]];
           if (p.done_valid) CKS(cudaStreamWaitEvent(cs, p.done, 0));      // dependency mechanism
         }
-        launch_ffn_gateup_gemm(h->u, perm, k, h->problems, i, j - i, max_rows, 0, I, H, h->act, I, wd, tensor, cs);
-        launch_ffn_down_gemm(h->act, I, h->problems, i, j - i, max_rows, 0, I, H, h->yexp, wd, tensor, cs);
+        RC(expert_batch(h, perm, i, j, max_rows));
         // slots recycled inside the layer: fills that wait for a launch position in [i, j)
         bool need_ev = false;
         for (size_t q = dnext; q < deferred.size(); ++q) {

@@ -62,6 +62,17 @@ def test_config1_variants(chunk, mode, stride, slots, warm):
         assert out["stats"]["misses"] == 0 and out["stats"]["h2d_bytes"] == 0
 
 
+def test_config1b_tcgen05():
+    """c1 with bf16 weights through the tcgen05 prefill path (c1b exercises the tensor-core path)."""
+    from paper_2410_22134_b200 import binding as B
+    cfg = synth.get_config("c1b")
+    w = synth.make_weights(cfg, predictor="skip")
+    out = run_parity(cfg, w, synth.make_prompt(cfg), cfg.decode_steps,
+                     flags=B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR)
+    _report("c1b/tcgen05", out)
+    assert out["report"].max_hidden_ratio <= 1.0
+
+
 def test_injected_prediction_trace():
     """predictor_mode TRACE with the true routing of layer m+stride (oracle-routing upper bound): no class-C
     miss in layers >= stride during decode when C >= k."""
@@ -98,7 +109,8 @@ def test_injected_prediction_trace():
 
 
 @pytest.mark.parametrize("name", ["c2", "c3", "c4"])
-def test_mini_configs(name):
+@pytest.mark.parametrize("tensor", [0, 1])
+def test_mini_configs(name, tensor):
     """Per-layer shapes of BASELINE.json configs[1..3] (reduced depth / vocab so the oracle finishes in seconds):
     shared expert + sigmoid gate (c2), dense layer 0 + router bias + always-on shared experts (c3), GQA + 352 MB
     experts with |needed| > slots in prefill, i.e. in-layer slot recycling (c4)."""
@@ -106,8 +118,10 @@ def test_mini_configs(name):
     cfg = mini(name)
     w = synth.make_weights(cfg, predictor="skip")
     T = {"c2": 96, "c3": 96, "c4": 40}[name]
-    out = run_parity(cfg, w, synth.make_prompt(cfg, T), 6)
-    _report(name + "-mini", out)
+    from paper_2410_22134_b200 import binding as B
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | (B.F_TENSOR if tensor else 0)
+    out = run_parity(cfg, w, synth.make_prompt(cfg, T), 6, flags=flags)
+    _report(name + "-mini" + ("/tcgen05" if tensor else "/simt"), out)
     assert out["report"].max_hidden_ratio <= 1.0
 
 
@@ -119,8 +133,15 @@ def test_outputs_independent_of_cache_parameters():
     w = synth.make_weights(cfg, predictor="skip")
     prompt = synth.make_prompt(cfg, 27)
     ids = synth.make_decode_ids(cfg, 10).tolist()
+    TF = B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TRACE | B.F_TENSOR
     base = run_gpu_only(cfg, w, prompt, ids, cache_slots=16)
     assert base["stats"]["misses"] == 0
+    # tcgen05 prefill: same invariance among tensor-path runs
+    tb = run_gpu_only(cfg, w, prompt, ids, cache_slots=16, flags=TF)
+    for kw in (dict(cache_slots=4, flags=TF), dict(cache_slots=8, stride=2, chunk_bytes=1 << 14, flags=TF)):
+        out = run_gpu_only(cfg, w, prompt, ids, **kw)
+        for a, b in zip(tb["logits"], out["logits"]):
+            assert np.array_equal(a, b), f"tcgen05 path: logits differ bitwise for {kw}"
     variants = [dict(cache_slots=4), dict(cache_slots=8, stride=2), dict(cache_slots=8, chunk_bytes=1 << 14),
                 dict(cache_slots=12, predictor_mode=B.PRED_NONE), dict(cache_slots=8, flags=B.F_REORDER | B.F_TRACE),
                 dict(cache_slots=4, chunk_bytes=1 << 18, max_inflight=1)]
