@@ -73,7 +73,8 @@ typedef struct {
   int32_t predictor_mode;
   int32_t flags;
   int32_t max_inflight;    /* chunks kept in flight on the copy stream (P:191 bounded delay); 0 = default 2 */
-  int32_t reserved;
+  int32_t high_group;      /* chunks per HIGH (precise) copy operation; 0 = the whole remaining fill in ONE copy (measured
+                              fastest); ready flags are written behind every operation */
   void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
 } promoe_opts_t;
 
@@ -159,6 +160,13 @@ PROMOE_API int promoe_get_slots(promoe_t* h, int32_t moe_layer, int32_t* slot_ex
 /* Measured pinned host->device bandwidth (GB/s) for `bytes`-sized copies at queue depth `depth`
  * (chunk size is chosen from this curve).  Allocates and frees its own buffers. */
 PROMOE_API int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out);
+
+/* Measured cost of the fill protocol itself:
+ * n_fills expert images of expert_bytes each, pinned host -> device, back to back on one stream, every fill bracketed
+ * by events as in the engine.  mode 0: one copy + one 32-bit stream write per chunk; 1: ONE copy per fill, then one
+ * 32-bit stream write per chunk; 2: one copy per fill + ONE small copy for all its flags; 3: one copy, no flags;
+ * 4: one copy + one 4-byte copy per chunk.  Result: sustained GB/s over the whole sequence. */
+PROMOE_API int promoe_measure_fill(size_t expert_bytes, size_t chunk_bytes, int32_t mode, int32_t n_fills, double* gbs_out);
 
 /* Live kernel timing for bench.py's roofline: runs `reps` launches of one hot kernel of the decode step on the
  * compute stream, bracketed by CUDA events, over RESIDENT slots rotating through all layers (working set = the

@@ -24,7 +24,7 @@ EXPORTS = [
     "promoe_create", "promoe_destroy", "promoe_last_error", "promoe_load_dense", "promoe_load_experts",
     "promoe_prefill", "promoe_decode", "promoe_set_prediction_trace", "promoe_stats", "promoe_get_trace",
     "promoe_reset", "promoe_get_slots", "promoe_measure_h2d", "promoe_op_linear", "promoe_op_route",
-    "promoe_op_permute", "promoe_op_expert_ffn", "promoe_kernel_time",
+    "promoe_op_permute", "promoe_op_expert_ffn", "promoe_kernel_time", "promoe_measure_fill",
 ]
 
 
@@ -38,7 +38,7 @@ class promoe_shape_t(C.Structure):
 class promoe_opts_t(C.Structure):
     _fields_ = [("cache_slots", C.c_int32), ("stride", C.c_int32), ("chunk_bytes", C.c_uint64),
                 ("predictor_mode", C.c_int32), ("flags", C.c_int32), ("max_inflight", C.c_int32),
-                ("reserved", C.c_int32), ("compute_stream", C.c_void_p)]
+                ("high_group", C.c_int32), ("compute_stream", C.c_void_p)]
 
 
 class promoe_dense_t(C.Structure):
@@ -95,6 +95,7 @@ def lib() -> C.CDLL:
     L.promoe_op_route.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_permute.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_expert_ffn.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
+    L.promoe_measure_fill.argtypes = [sz, sz, i32, i32, C.POINTER(C.c_double)]
     L.promoe_kernel_time.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     for n in EXPORTS:
         f = getattr(L, n)
@@ -178,3 +179,9 @@ def promoe_kernel_time(h, which: int, reps: int = 200):
     ms, nb = C.c_double(), C.c_double()
     _check(lib().promoe_kernel_time(h, which, reps, C.byref(ms), C.byref(nb)), h)
     return ms.value, nb.value
+
+
+def promoe_measure_fill(expert_bytes: int, chunk_bytes: int, mode: int, n_fills: int = 32) -> float:
+    g = C.c_double()
+    _check(lib().promoe_measure_fill(expert_bytes, chunk_bytes, mode, n_fills, C.byref(g)))
+    return g.value

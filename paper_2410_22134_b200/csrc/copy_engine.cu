@@ -59,39 +59,51 @@ static int ring_slot(promoe_t* h, size_t* idx) {
   return PROMOE_OK;
 }
 
-// Enqueue chunks [c0, c1) of the fill (layer m, slot s) on the copy stream, each followed by its flag write.
-// One timing slot brackets the whole range.
+// Flags of chunks [p.flagged, p.issued) ← generation, as ONE small copy behind the data copies (measured: a 32-bit
+// stream write or a 4-byte copy behind EVERY chunk costs 8-30 % of the link, profiles/r01_fill_protocol.md).
+static int write_flags(promoe_t* h, int m, int s) {
+  SlotPhys& p = h->phys[(size_t)m * h->C + s];
+  const int n = p.issued - p.flagged;
+  if (n <= 0) return PROMOE_OK;
+  if (h->flagsrc_pos + (size_t)n > 65536) h->flagsrc_pos = 0;
+  uint32_t* v = h->flagsrc_host + h->flagsrc_pos;
+  h->flagsrc_pos += (size_t)n;
+  for (int i = 0; i < n; ++i) v[i] = p.gen;
+  uint32_t* fl = h->flags + ((size_t)m * h->C + s) * h->n_chunks + p.flagged;
+  CKC(cudaMemcpyAsync(fl, v, (size_t)n * 4, cudaMemcpyHostToDevice, h->ps));
+  p.flagged = p.issued;
+  return PROMOE_OK;
+}
+
+// Enqueue chunks [c0, c1) of the fill (layer m, slot s) on the copy stream.  HIGH: `group` chunks per copy
+// operation (0 = all of them in one), flags written behind every operation; LOW: one chunk per call, flags deferred
+// until the fill completes or a HIGH operation takes it over.  One timing slot brackets the whole call.
 static int issue_chunks(promoe_t* h, int m, int s, int c0, int c1, bool low) {
   SlotPhys& p = h->phys[(size_t)m * h->C + s];
   const uint8_t* src = (const uint8_t*)h->expert_host[(size_t)m * h->s.n_experts + p.expert];
   uint8_t* dst = h->slots + ((size_t)m * h->C + s) * h->Be;
-  uint32_t* fl = h->flags + ((size_t)m * h->C + s) * h->n_chunks;
   size_t ri = 0;
   int rc = ring_slot(h, &ri);
   if (rc) return rc;
   CKC(cudaEventRecord(h->ev_ring_start[ri], h->ps));
-  for (int c = c0; c < c1; ++c) {
+  const int group = low ? 1 : (h->high_group > 0 ? h->high_group : h->n_chunks);
+  for (int c = c0; c < c1; c += group) {
+    const int ce = std::min(c1, c + group);
     const size_t off = (size_t)c * h->chunk_bytes;
-    const size_t len = std::min(h->chunk_bytes, h->Be - off);
+    const size_t len = std::min((size_t)ce * h->chunk_bytes, h->Be) - off;
     CKC(cudaMemcpyAsync(dst + off, src + off, len, cudaMemcpyHostToDevice, h->ps));
-    if (h->fn_write32) {
-      CUresult r = ((write32_fn)h->fn_write32)((CUstream)h->ps, (CUdeviceptr)(uintptr_t)(fl + c), p.gen, 0);
-      if (r != CUDA_SUCCESS) { h->err = "cuStreamWriteValue32 failed"; return PROMOE_ECUDA; }
-    } else {
-      uint32_t* v = h->flagsrc_host + (h->flagsrc_pos++ % 65536);
-      *v = p.gen;
-      CKC(cudaMemcpyAsync(fl + c, v, 4, cudaMemcpyHostToDevice, h->ps));
-    }
+    p.issued = ce;
     h->st.h2d_bytes += len;
-    h->st.chunks_issued++;
-    if (low) h->st.chunks_low++; else h->st.chunks_high++;
+    h->st.chunks_issued += (uint64_t)(ce - c);
+    if (low) h->st.chunks_low += (uint64_t)(ce - c); else h->st.chunks_high += (uint64_t)(ce - c);
+    if (!low || ce == h->n_chunks) { rc = write_flags(h, m, s); if (rc) return rc; }
   }
   CKC(cudaEventRecord(h->ev_ring[ri], h->ps));
   h->ev_is_low[ri] = low ? 1 : 0;
   if (low) h->low_inflight++; else h->high_inflight++;
+  p.fill_seq = h->ev_head;           // complete once the ring tail has passed this slot
   h->ev_head++;
-  p.issued = c1;
-  if (c1 == h->n_chunks) { CKC(cudaEventRecord(p.done, h->ps)); p.done_valid = true; }
+  if (c1 == h->n_chunks && h->want_done_events) { CKC(cudaEventRecord(p.done, h->ps)); p.done_valid = true; }
   return PROMOE_OK;
 }
 
@@ -164,6 +176,7 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
   const LayerCmd& c = h->cmd_host[m];
   const int n = c.n_needed, E = h->s.n_experts, C = h->C;
   promoe_stats_t& st = h->st;
+  { int rc0 = ce_retire(h, false); if (rc0) return rc0; }
   if (h->o.flags & PROMOE_F_PREEMPT) ce_cancel_low(h, m);
   // prediction accuracy: |pred ∩ needed| / |pred| for the list pushed into this layer
   std::vector<int32_t>& pend = h->pending_pred[m];
@@ -184,7 +197,7 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
     else if (cls == 1) {
       st.hits_prefetch++;
       st.fetched_at_gate_of++;
-      if (p.gen == gen && p.issued >= h->n_chunks && p.done_valid && cudaEventQuery(p.done) == cudaSuccess) st.fetched_at_gate++;
+      if (p.gen == gen && p.issued >= h->n_chunks && h->ev_tail > p.fill_seq) st.fetched_at_gate++;
     } else {
       st.misses++;
       if (victim >= 0) st.evictions++;
@@ -192,7 +205,7 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
     }
     if (dep >= 0 && deferred) { deferred->push_back(i); continue; }   // slot still in use by launch position dep
     if (p.gen != gen || p.expert != e) {   // new allocation of this slot
-      p.gen = gen; p.expert = e; p.issued = 0; p.done_valid = false;
+      p.gen = gen; p.expert = e; p.issued = 0; p.flagged = 0; p.done_valid = false;
     }
     int rc = ce_issue_needed(h, m, i, nullptr);
     if (rc) return rc;
@@ -213,7 +226,7 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
         st.pred_allocs++;
         if (victim >= 0) st.evictions++;
         h->mirror[(size_t)mt * C + s] = e;
-        p.gen = gen; p.expert = e; p.issued = 0; p.done_valid = false;
+        p.gen = gen; p.expert = e; p.issued = 0; p.flagged = 0; p.done_valid = false;
       }
       if (p.issued < h->n_chunks) h->low.push_back(FillJob{mt, s, e, gen, 1});   // alloc, or touch of a cancelled fill (G3)
     }
@@ -225,6 +238,6 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
 int ce_issue_deferred(promoe_t* h, int m, int i, cudaEvent_t after) {
   const int32_t* r = (const int32_t*)h->cmd_host[m].need + 7 * i;
   SlotPhys& p = h->phys[(size_t)m * h->C + r[2]];
-  p.gen = (uint32_t)r[5]; p.expert = r[0]; p.issued = 0; p.done_valid = false;
+  p.gen = (uint32_t)r[5]; p.expert = r[0]; p.issued = 0; p.flagged = 0; p.done_valid = false;
   return ce_issue_needed(h, m, i, after);
 }

@@ -61,6 +61,7 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   if (h->chunk_bytes % 256) { delete h; return bad("chunk_bytes must be a multiple of 256"); }
   h->n_chunks = (int)((h->Be + h->chunk_bytes - 1) / h->chunk_bytes);
   h->max_inflight = op->max_inflight > 0 ? op->max_inflight : 2;
+  h->high_group = op->high_group > 0 ? op->high_group : 0;
   h->maxT = s.max_seq;
   h->qkv_w = (s.n_q_heads + 2 * s.n_kv_heads) * s.head_dim;
   h->ffn_w = s.n_shared_inter > s.dense_inter ? s.n_shared_inter : s.dense_inter;
@@ -237,7 +238,7 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
   if (ce_retire(h, true)) return PROMOE_ECUDA;
   for (size_t i = 0; i < h->phys.size(); ++i) {
     SlotPhys& p = h->phys[i];
-    p.gen = 0; p.expert = se[i]; p.issued = warm ? h->n_chunks : 0; p.done_valid = false;
+    p.gen = 0; p.expert = se[i]; p.issued = warm ? h->n_chunks : 0; p.flagged = p.issued; p.fill_seq = 0; p.done_valid = false;
   }
   if (warm && copy_warm && h->experts_loaded)
     for (int m = 0; m < Lm; ++m)
@@ -321,5 +322,68 @@ extern "C" int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, dou
   if (st) cudaStreamDestroy(st);
   if (dbuf) cudaFree(dbuf);
   if (hbuf) cudaFreeHost(hbuf);
+  return rc;
+}
+
+typedef CUresult (*mf_write32_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+extern "C" int promoe_measure_fill(size_t Be, size_t chunk, int32_t mode, int32_t n_fills, double* gbs_out) {
+  if (!Be || !chunk || n_fills < 1 || mode < 0 || mode > 4 || !gbs_out) return PROMOE_EINVAL;
+  const int nslot = 8, nch = (int)((Be + chunk - 1) / chunk);
+  void *hbuf = nullptr, *dbuf = nullptr;
+  uint32_t *flags = nullptr, *fsrc = nullptr;
+  cudaStream_t st = nullptr;
+  std::vector<cudaEvent_t> ev(3 * (size_t)n_fills + 2, nullptr);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &fn, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess) fn = nullptr;
+  int rc = PROMOE_ECUDA;
+  bool ok = cudaHostAlloc(&hbuf, Be * nslot, cudaHostAllocDefault) == cudaSuccess && cudaMalloc(&dbuf, Be * nslot) == cudaSuccess &&
+            cudaMalloc((void**)&flags, (size_t)nslot * nch * 4) == cudaSuccess &&
+            cudaHostAlloc((void**)&fsrc, (size_t)nch * 4, cudaHostAllocDefault) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess;
+  for (auto& e : ev) ok = ok && cudaEventCreate(&e) == cudaSuccess;
+  if (ok && ((mode == 0 || mode == 1) && !fn)) ok = false;
+  if (ok) {
+    memset(hbuf, 1, Be * nslot);
+    for (int c = 0; c < nch; ++c) fsrc[c] = 7;
+    double best = 0.0;
+    for (int rep = 0; rep < 2; ++rep) {
+      cudaEventRecord(ev[3 * (size_t)n_fills], st);
+      for (int f = 0; f < n_fills; ++f) {
+        const int sl = f % nslot;
+        char* d = (char*)dbuf + (size_t)sl * Be;
+        const char* s = (const char*)hbuf + (size_t)sl * Be;
+        uint32_t* fl = flags + (size_t)sl * nch;
+        cudaEventRecord(ev[3 * (size_t)f], st);
+        if (mode == 0 || mode == 4) {
+          for (int c = 0; c < nch; ++c) {
+            const size_t off = (size_t)c * chunk, len = std::min(chunk, Be - off);
+            cudaMemcpyAsync(d + off, s + off, len, cudaMemcpyHostToDevice, st);
+            if (mode == 0) ((mf_write32_fn)fn)((CUstream)st, (CUdeviceptr)(uintptr_t)(fl + c), 7, 0);
+            else cudaMemcpyAsync(fl + c, fsrc + c, 4, cudaMemcpyHostToDevice, st);
+          }
+        } else {
+          cudaMemcpyAsync(d, s, Be, cudaMemcpyHostToDevice, st);
+          if (mode == 1) for (int c = 0; c < nch; ++c) ((mf_write32_fn)fn)((CUstream)st, (CUdeviceptr)(uintptr_t)(fl + c), 7, 0);
+          if (mode == 2) cudaMemcpyAsync(fl, fsrc, (size_t)nch * 4, cudaMemcpyHostToDevice, st);
+        }
+        cudaEventRecord(ev[3 * (size_t)f + 1], st);
+        cudaEventRecord(ev[3 * (size_t)f + 2], st);
+      }
+      cudaEventRecord(ev[3 * (size_t)n_fills + 1], st);
+      if (cudaStreamSynchronize(st) != cudaSuccess) break;
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, ev[3 * (size_t)n_fills], ev[3 * (size_t)n_fills + 1]);
+      if (ms > 0.f) best = std::max(best, (double)Be * n_fills / (ms * 1e6));
+    }
+    *gbs_out = best;
+    rc = best > 0.0 ? PROMOE_OK : PROMOE_ECUDA;
+  }
+  for (auto e : ev) if (e) cudaEventDestroy(e);
+  if (st) cudaStreamDestroy(st);
+  if (dbuf) cudaFree(dbuf);
+  if (flags) cudaFree(flags);
+  if (hbuf) cudaFreeHost(hbuf);
+  if (fsrc) cudaFreeHost(fsrc);
   return rc;
 }

@@ -25,6 +25,8 @@ struct SlotPhys {
   uint32_t gen = 0;
   int expert = -1;
   int issued = 0;
+  int flagged = 0;              // chunks whose ready flag write has been enqueued (<= issued)
+  size_t fill_seq = 0;          // ring sequence of the last copy operation of this slot
   cudaEvent_t done = nullptr;   // recorded after the last chunk of the current generation
   bool done_valid = false;
 };
@@ -86,6 +88,8 @@ struct promoe {
   size_t ev_head = 0, ev_tail = 0;        // in flight = [tail, head)
   std::vector<int> ev_is_low;
   int low_inflight = 0, high_inflight = 0;
+  int high_group = 0;                 // chunks per HIGH copy operation, 0 = whole remaining fill in one copy
+  bool want_done_events = false;      // prefill: per-fill completion events for cudaStreamWaitEvent
   bool low_yields = true;             // LOW chunks wait while HIGH fills are outstanding
   std::vector<cudaEvent_t> done_ev;       // prefill: per launch position "expert finished" events
   cudaEvent_t step_start = nullptr, step_end = nullptr;

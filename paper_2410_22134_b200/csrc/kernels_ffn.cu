@@ -43,6 +43,8 @@ __global__ void __launch_bounds__(256) ffn_gateup_gemv_kernel(const float* __res
   if (!ok) return;
   const int r = r0 + warp;
   if (r >= pb.inter) return;
+  // two passes (4 loads in flight per lane each): 48 registers keep 40 warps/SM resident, so the c2/c3 grid
+  // (5632 / 8448 warps) is a single wave; the fused two-row variant (row_dot2) needs 2 waves and measured slower
   const float g = row_dot<WT>((const WT*)pb.wg + (size_t)r * H, u, H, lane);
   const float v = row_dot<WT>((const WT*)pb.wu + (size_t)r * H, u, H, lane);
   if (lane == 0) act[(size_t)p * act_stride + r] = silu(g) * v;

@@ -10,7 +10,7 @@ constexpr int kMaxE = 256;
 
 struct SlotView {
   int32_t* slot_expert; int32_t* expert_slot; unsigned long long* stamp; uint32_t* gen; uint8_t* origin;
-  unsigned long long* clock; int C, E;
+  unsigned long long* clock; int C, E;   // all pointers: SHARED-memory copies of one layer's rows (+ a local clock)
   __device__ void touch(int s) { stamp[s] = ++(*clock); }
   // Alg. 1 l.4 cache.replace_with: lowest EMPTY slot, else smallest stamp among unprotected slots; -1 if none.
   __device__ int victim(const uint8_t* prot) const {
@@ -49,15 +49,39 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   __shared__ int32_t rec[7 * kMaxE];    // staged command records (mapped host memory is write-only here)
   __shared__ int32_t prec[5 * kMaxE];
   __shared__ int s_n, s_np;
+  // the table rows of layer m and of the prediction target are staged in shared memory (parallel loads), the
+  // serial state machine runs on them, and they are written back in parallel: the kernel sits on the critical
+  // path in front of every copy, so no dependent global load may be in the serial part
+  __shared__ int32_t t_se[2][kMaxE], t_es[2][kMaxE];
+  __shared__ unsigned long long t_stamp[2][kMaxE];
+  __shared__ uint32_t t_gen[2][kMaxE];
+  __shared__ uint8_t t_org[2][kMaxE];
+  __shared__ unsigned long long t_clock;
+  __shared__ int32_t s_pred[kMaxE + 1];
   const int E = tbl.E, C = tbl.C;
+  const int mt_ = m + stride;
+  const bool have_t = pred_list != nullptr && mt_ < tbl.Lm;
+  for (int i = threadIdx.x; i < C; i += blockDim.x) {
+    t_se[0][i] = tbl.slot_expert[(size_t)m * C + i]; t_stamp[0][i] = tbl.stamp[(size_t)m * C + i];
+    t_gen[0][i] = tbl.gen[(size_t)m * C + i]; t_org[0][i] = tbl.origin[(size_t)m * C + i];
+    if (have_t) {
+      t_se[1][i] = tbl.slot_expert[(size_t)mt_ * C + i]; t_stamp[1][i] = tbl.stamp[(size_t)mt_ * C + i];
+      t_gen[1][i] = tbl.gen[(size_t)mt_ * C + i]; t_org[1][i] = tbl.origin[(size_t)mt_ * C + i];
+    }
+  }
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    t_es[0][e] = tbl.expert_slot[(size_t)m * E + e];
+    if (have_t) t_es[1][e] = tbl.expert_slot[(size_t)mt_ * E + e];
+  }
+  if (have_t) for (int i = threadIdx.x; i <= E; i += blockDim.x) s_pred[i] = pred_list[i];
+  if (threadIdx.x == 0) t_clock = *tbl.clock;
   for (int e = threadIdx.x; e < kMaxE; e += blockDim.x) { needed[e] = 0; prot[e] = 0; }
   __syncthreads();
   for (int i = threadIdx.x; i < T * k; i += blockDim.x) needed[sel[i]] = 1;   // same-value writes
   __syncthreads();
   if (threadIdx.x == 0) {
 
-  SlotView v{tbl.slot_expert + (size_t)m * C, tbl.expert_slot + (size_t)m * E, tbl.stamp + (size_t)m * C,
-             tbl.gen + (size_t)m * C, tbl.origin + (size_t)m * C, tbl.clock, C, E};
+  SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
   // ---- PushPrecise(m): classes A (cached) → B (being prefetched) → C (not begun), ascending id inside
   int n = 0, nA = 0, nB = 0;
   for (int e = 0; e < E; ++e)
@@ -121,9 +145,9 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   // its own predictions; no victim → skip.
   int np = 0;
   const int mt = m + stride;
-  if (pred_list && mt < tbl.Lm) {
-    SlotView t{tbl.slot_expert + (size_t)mt * C, tbl.expert_slot + (size_t)mt * E, tbl.stamp + (size_t)mt * C,
-               tbl.gen + (size_t)mt * C, tbl.origin + (size_t)mt * C, tbl.clock, C, E};
+  if (have_t) {
+    SlotView t{t_se[1], t_es[1], t_stamp[1], t_gen[1], t_org[1], &t_clock, C, E};
+    const int32_t* pred_list = s_pred;
     np = pred_list[0];
     for (int e = 0; e < E; ++e) prot[e] = 0;
     for (int i = 0; i < np; ++i) prot[pred_list[1 + i]] = 1;
@@ -142,8 +166,23 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   }
   if (trace_pred) trace_pred[0] = np;
   s_n = n; s_np = np;
+  (void)mt;
   }  // thread 0
   __syncthreads();
+  // write the staged rows back
+  for (int i = threadIdx.x; i < C; i += blockDim.x) {
+    tbl.slot_expert[(size_t)m * C + i] = t_se[0][i]; tbl.stamp[(size_t)m * C + i] = t_stamp[0][i];
+    tbl.gen[(size_t)m * C + i] = t_gen[0][i]; tbl.origin[(size_t)m * C + i] = t_org[0][i];
+    if (have_t) {
+      tbl.slot_expert[(size_t)mt_ * C + i] = t_se[1][i]; tbl.stamp[(size_t)mt_ * C + i] = t_stamp[1][i];
+      tbl.gen[(size_t)mt_ * C + i] = t_gen[1][i]; tbl.origin[(size_t)mt_ * C + i] = t_org[1][i];
+    }
+  }
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    tbl.expert_slot[(size_t)m * E + e] = t_es[0][e];
+    if (have_t) tbl.expert_slot[(size_t)mt_ * E + e] = t_es[1][e];
+  }
+  if (threadIdx.x == 0) *tbl.clock = t_clock;
   // publish the command to the host issuer (posted writes to mapped pinned memory), seq last
   for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
   for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) cmd->pred[i] = prec[i];

@@ -126,6 +126,8 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     }
   for (auto& v : h->pending_pred) v.clear();
 
+  h->want_done_events = T > 1;
+  if (T > 1) RC(ce_retire(h, true));   // prefill orders compute after fills with events: start from a drained copy stream
   CKS(cudaMemcpyAsync(h->ids, ids_host, (size_t)T * 4, cudaMemcpyHostToDevice, cs));
   CKS(cudaEventRecord(h->step_start, cs));
   if (h->o.flags & PROMOE_F_TRACE) {

@@ -16,7 +16,7 @@ from oracle.forward import OracleModel
 
 def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional[int] = None,
                stride: Optional[int] = None, chunk_bytes: int = 0, predictor_mode: int = 1, flags: Optional[int] = None,
-               decode_ids: Optional[List[int]] = None, max_inflight: int = 0, warm: bool = True) -> Dict:
+               decode_ids: Optional[List[int]] = None, max_inflight: int = 0, warm: bool = True, high_group: int = 0) -> Dict:
     from paper_2410_22134_b200 import binding as B
     from paper_2410_22134_b200.engine import ProMoE
 
@@ -28,7 +28,7 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
     n_moe = s.n_layers - s.n_dense_layers
     C = cache_slots // n_moe
     eng = ProMoE(weights, cache_slots=cache_slots, stride=stride, chunk_bytes=chunk_bytes,
-                 predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight)
+                 predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight, high_group=high_group)
     use_pred = predictor_mode == B.PRED_MLP
     ora = OracleModel(weights, stride=stride, slots_per_layer=C, use_predictor=use_pred)
     sim = ProMoECacheSim(n_moe, s.n_experts, C, warm=bool(flags & B.F_WARM))

@@ -56,7 +56,7 @@ def test_config1_variants(chunk, mode, stride, slots, warm):
     w = synth.make_weights(cfg, predictor="skip")
     ids = synth.make_decode_ids(cfg, 12).tolist()
     out = run_parity(cfg, w, synth.make_prompt(cfg, 19), 12, cache_slots=slots, stride=stride, chunk_bytes=chunk,
-                     predictor_mode=mode, decode_ids=ids, warm=warm)
+                     predictor_mode=mode, decode_ids=ids, warm=warm, high_group=1 if chunk == 1 << 16 else 0)
     _report(f"c1 mode{mode} s{stride} slots{slots} chunk{chunk}", out)
     if slots == 16:
         assert out["stats"]["misses"] == 0 and out["stats"]["h2d_bytes"] == 0
@@ -144,7 +144,7 @@ def test_outputs_independent_of_cache_parameters():
             assert np.array_equal(a, b), f"tcgen05 path: logits differ bitwise for {kw}"
     variants = [dict(cache_slots=4), dict(cache_slots=8, stride=2), dict(cache_slots=8, chunk_bytes=1 << 14),
                 dict(cache_slots=12, predictor_mode=B.PRED_NONE), dict(cache_slots=8, flags=B.F_REORDER | B.F_TRACE),
-                dict(cache_slots=4, chunk_bytes=1 << 18, max_inflight=1)]
+                dict(cache_slots=4, chunk_bytes=1 << 18, max_inflight=1), dict(cache_slots=8, chunk_bytes=1 << 16, high_group=2)]
     for kw in variants:
         out = run_gpu_only(cfg, w, prompt, ids, **kw)
         for a, b in zip(base["logits"], out["logits"]):
