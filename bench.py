@@ -164,7 +164,8 @@ def workload_config(cfg, args):
                         f"{s.n_layers}L H{s.hidden} E{s.n_experts} top{s.top_k} I{s.expert_inter}, batch 1, "
                         f"prompt {cfg.prompt_len} + {cfg.decode_steps} decode",
             "cache_slots": cfg.cache_slots, "cache_fraction": cfg.slots_per_layer / s.n_experts, "stride": cfg.stride,
-            "predictor": args.predictor, "decode_ids": args.decode, "chunk_bytes": args.chunk_mb << 20,
+            "predictor": args.predictor, "decode_ids": args.decode, "chunk_bytes": args.chunk_mb << 20, "max_spec_decode": args.max_spec_decode,
+            "max_spec_prefill": args.max_spec_prefill,
             "l2": "inputs larger than L2 (each request streams >> 126 MB of expert weights)"}
 
 
@@ -223,7 +224,7 @@ def run_ours(args, cfg, rank, world, dist):
     torch.cuda.set_device(local)
     peaks = load_peaks()
     s = cfg.shape
-    weights = synth.make_weights(cfg, predictor=args.predictor)
+    weights = synth.make_weights(cfg, predictor="skip" if args.predictor == "none" else args.predictor)
     wb = 4 if s.wdtype == 0 else 2
     Be = 3 * s.hidden * s.expert_inter * wb
     h2d_gbs = B.promoe_measure_h2d(256 << 20, 2, 5)
@@ -233,7 +234,7 @@ def run_ours(args, cfg, rank, world, dist):
     flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | (B.F_TENSOR if args.tensor else 0)
     eng = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_mb << 20,
                  predictor_mode=B.PRED_MLP if args.predictor != "none" else B.PRED_NONE, flags=flags,
-                 max_inflight=args.inflight)
+                 max_inflight=args.inflight, max_spec_decode=args.max_spec_decode, max_spec_prefill=args.max_spec_prefill)
     for _ in range(args.warmup):
         run_request(eng, cfg, prompt, decode_ids, greedy)
     if dist is not None:
@@ -367,6 +368,8 @@ def main():
                     help="decode ids: seeded random (locality-neutral, default) or greedy argmax")
     ap.add_argument("--chunk-mb", type=int, default=4)
     ap.add_argument("--inflight", type=int, default=0)
+    ap.add_argument("--max-spec-decode", type=int, default=0, help="allocations per PushPredicted in decode (0 = top_k, <0 = none)")
+    ap.add_argument("--max-spec-prefill", type=int, default=0, help="allocations per PushPredicted in prefill (<=0 = none)")
     ap.add_argument("--tensor", type=int, default=1, help="prefill GEMMs on tcgen05 (bf16 weights)")
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--decode-steps", type=int, default=0)

@@ -75,6 +75,10 @@ typedef struct {
   int32_t max_inflight;    /* chunks kept in flight on the copy stream (P:191 bounded delay); 0 = default 2 */
   int32_t high_group;      /* chunks per HIGH (precise) copy operation; 0 = the whole remaining fill in ONE copy (measured
                               fastest); ready flags are written behind every operation */
+  int32_t max_spec_decode; /* experts of one PushPredicted that may ALLOCATE a slot in a decode step (listed order = most
+                              confident first); 0 = default top_k (all, as Alg. 2), < 0 = none (touch only) */
+  int32_t max_spec_prefill;/* same for a prefill step (T > 1); <= 0 = default none: with 50-100 % of the experts needed
+                               an allocation only swaps one needed expert for another (G7) */
   void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
 } promoe_opts_t;
 

@@ -25,6 +25,11 @@ every touch / alloc sets stamp ← ++clock (LRU = smallest stamp).
   push_predicted(m, preds)         (Alg. 2 l.1-10; predictor of MoE layer m - stride)
      for e in listed order: holds a slot → touch (Alg. 2 l.3-5); else alloc(PRED); the experts of this
        same list are protected (one push never evicts its own predictions); no victim → SKIP.
+     max_spec (SURVEY G3 knob): at most max_spec experts of one push may ALLOCATE (the list is ordered by
+       descending predictor score, so the most confident ones go first); further non-cached ones → SKIP.
+       Defaults (G3/G7): decode = top_k (every prediction may allocate, as in Alg. 2); prefill = 0 —
+       with T > 1 tokens 50-100 % of the experts are needed and a per-layer LRU has no free slot, so
+       an allocation only swaps one needed expert for another; predictions then only refresh LRU stamps.
 
 alloc victim (Alg. 1 l.4 `cache.replace_with`): lowest-index EMPTY slot, else smallest stamp among unprotected.
 """
@@ -172,28 +177,30 @@ class ProMoECacheSim:
             self.origin[m][s] = RESIDENT
         return rec
 
-    def push_predicted(self, m: int, preds: Sequence[int]) -> PredRecord:
+    def push_predicted(self, m: int, preds: Sequence[int], max_spec: Optional[int] = None) -> PredRecord:
         rec = PredRecord()
         preds = [int(e) for e in preds]
         protected = set(preds)
         self._pending_pred[m] = list(preds)
+        allocs = 0
         for e in preds:
             s = self.slot_of(m, e)
             if s >= 0:
                 self._touch(m, s)
                 rec.expert.append(e); rec.action.append(ACT_TOUCH); rec.slot.append(s); rec.victim.append(-1)
                 continue
-            s = self._victim(m, protected)
+            s = self._victim(m, protected) if (max_spec is None or allocs < max_spec) else -1
             if s < 0:
                 rec.expert.append(e); rec.action.append(ACT_SKIP); rec.slot.append(-1); rec.victim.append(-1)
                 continue
             old = self._install(m, s, e, PRED)
+            allocs += 1
             self.stats.pred_allocs += 1
             rec.expert.append(e); rec.action.append(ACT_ALLOC); rec.slot.append(s); rec.victim.append(old)
         return rec
 
     def run_step(self, needed_per_layer: Sequence[Sequence[int]],
-                 pred_per_layer: Sequence[Optional[Sequence[int]]], stride: int):
+                 pred_per_layer: Sequence[Optional[Sequence[int]]], stride: int, max_spec: Optional[int] = None):
         """One prefill/decode step.  needed_per_layer[m] = experts the gate of MoE layer m selected (any token);
         pred_per_layer[m] = list predicted BY the predictor at MoE layer m FOR layer m+stride, or None.
         Order inside a layer: push_precise(m) then push_predicted(m+stride) (SURVEY O3 step 2 then 4; G5: no
@@ -204,6 +211,6 @@ class ProMoECacheSim:
             prec = self.push_precise(m, needed_per_layer[m])
             pr = None
             if pred_per_layer[m] is not None and m + stride < self.L:
-                pr = self.push_predicted(m + stride, pred_per_layer[m])
+                pr = self.push_predicted(m + stride, pred_per_layer[m], max_spec)
             out.append((prec, pr))
         return out

@@ -139,7 +139,8 @@ def compare_step(gpu: Dict[str, np.ndarray], st: StepTrace, n_experts: int, rep:
             rep.top1_near_tie += 1
 
 
-def compare_cache(sim: ProMoECacheSim, gpu: Dict[str, np.ndarray], stride: int, use_pred: bool) -> None:
+def compare_cache(sim: ProMoECacheSim, gpu: Dict[str, np.ndarray], stride: int, use_pred: bool,
+                  max_spec: Optional[int] = None) -> None:
     """P3: drive O3 with the GPU's own routing + prediction lists for one step; records must match bit for bit."""
     Lm, E = sim.L, sim.E
     needed = [sorted(set(int(e) for e in gpu["sel"][m].reshape(-1))) for m in range(Lm)]
@@ -147,7 +148,7 @@ def compare_cache(sim: ProMoECacheSim, gpu: Dict[str, np.ndarray], stride: int, 
     for m in range(Lm):
         n = int(gpu["predlist"][m, 0])
         preds.append(gpu["predlist"][m, 1:1 + n].tolist() if use_pred else None)
-    out = sim.run_step(needed, preds, stride)
+    out = sim.run_step(needed, preds, stride, max_spec)
     for m, (prec, _) in enumerate(out):
         row = gpu["precise"][m]
         n = int(row[0])

@@ -62,6 +62,8 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   h->n_chunks = (int)((h->Be + h->chunk_bytes - 1) / h->chunk_bytes);
   h->max_inflight = op->max_inflight > 0 ? op->max_inflight : 2;
   h->high_group = op->high_group > 0 ? op->high_group : 0;
+  h->max_spec_decode = op->max_spec_decode == 0 ? s.top_k : std::max(0, op->max_spec_decode);
+  h->max_spec_prefill = op->max_spec_prefill <= 0 ? 0 : op->max_spec_prefill;
   h->maxT = s.max_seq;
   h->qkv_w = (s.n_q_heads + 2 * s.n_kv_heads) * s.head_dim;
   h->ffn_w = s.n_shared_inter > s.dense_inter ? s.n_shared_inter : s.dense_inter;

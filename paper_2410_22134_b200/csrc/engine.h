@@ -38,6 +38,7 @@ struct promoe {
   promoe_opts_t o{};
   int Lm = 0, C = 0, wb = 2, n_chunks = 0, max_inflight = 2;
   size_t Be = 0, chunk_bytes = 0;
+  int max_spec_decode = 0, max_spec_prefill = 0;   // allocations allowed per PushPredicted (knob G3)
   int maxT = 0, qkv_w = 0, ffn_w = 0, nsplit = 1;
   cudaStream_t cs = nullptr, ps = nullptr;
   bool own_cs = false, dense_loaded = false, experts_loaded = false;

@@ -68,7 +68,7 @@ struct LayerCmd {
 // One thread block (one warp) runs PushPrecise(m) then PushPredicted(m+stride) (Alg. 2) and writes:
 //  problems[i] for the needed experts in launch order (row ranges from offset[] when T > 1),
 //  dec_order[j] (decode: launch position -> j), the trace records and the host command.
-void launch_slot_table(SlotTable tbl, int m, int stride, const int32_t* sel, int T, int k, const int32_t* offset,
+void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int32_t* sel, int T, int k, const int32_t* offset,
                        const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* j_of_problem, LayerCmd* cmd,

@@ -32,7 +32,7 @@ struct SlotView {
   }
 };
 
-__global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, int stride,
+__global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, int stride, int max_spec,
                                                          const int32_t* __restrict__ sel, int T, int k,
                                                          const int32_t* __restrict__ offset,
                                                          const int32_t* __restrict__ pred_list,
@@ -151,13 +151,15 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
     np = pred_list[0];
     for (int e = 0; e < E; ++e) prot[e] = 0;
     for (int i = 0; i < np; ++i) prot[pred_list[1 + i]] = 1;
+    int allocs = 0;   // at most max_spec experts of one push may allocate (knob G3; most confident first)
     for (int i = 0; i < np; ++i) {
       const int e = pred_list[1 + i];
       int32_t* r = prec + 5 * i;
       int s = t.expert_slot[e];
       if (s >= 0) { t.touch(s); r[0] = e; r[1] = 0; r[2] = s; r[3] = -1; r[4] = (int32_t)t.gen[s]; }
       else {
-        s = t.victim(prot);
+        s = allocs < max_spec ? t.victim(prot) : -1;
+        if (s >= 0) ++allocs;
         if (s < 0) { r[0] = e; r[1] = 2; r[2] = -1; r[3] = -1; r[4] = 0; }
         else { const int old = t.install(s, e, 1); r[0] = e; r[1] = 1; r[2] = s; r[3] = old; r[4] = (int32_t)t.gen[s]; }
       }
@@ -195,13 +197,13 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   }
 }
 
-void launch_slot_table(SlotTable tbl, int m, int stride, const int32_t* sel, int T, int k, const int32_t* offset,
+void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int32_t* sel, int T, int k, const int32_t* offset,
                        const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
                        int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st) {
   (void)reorder;
-  slot_table_kernel<<<1, 256, 0, st>>>(tbl, m, stride, sel, T, k, offset, pred_list, slot_base, slot_bytes,
+  slot_table_kernel<<<1, 256, 0, st>>>(tbl, m, stride, max_spec, sel, T, k, offset, pred_list, slot_base, slot_bytes,
                                        flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of,
                                        cmd, seq, trace_precise, trace_pred);
 }

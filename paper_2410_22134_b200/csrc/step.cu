@@ -178,7 +178,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
       plist = h->pred_list + (size_t)m * (1 + E);
     }
     if (T > 1) launch_permute(sel, T, k, E, h->count + (size_t)m * E, offset, perm, inv, cs);   // A8
-    launch_slot_table(h->tbl, m, h->o.stride, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
+    launch_slot_table(h->tbl, m, h->o.stride, T == 1 ? h->max_spec_decode : h->max_spec_prefill, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
                       (h->o.flags & PROMOE_F_REORDER) != 0, h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb,
                       h->problems, h->n_prob, h->row_of, h->cmd_dev + m, seq,
                       h->trace_precise + (size_t)m * (1 + 5 * E),

@@ -16,7 +16,8 @@ from oracle.forward import OracleModel
 
 def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional[int] = None,
                stride: Optional[int] = None, chunk_bytes: int = 0, predictor_mode: int = 1, flags: Optional[int] = None,
-               decode_ids: Optional[List[int]] = None, max_inflight: int = 0, warm: bool = True, high_group: int = 0) -> Dict:
+               decode_ids: Optional[List[int]] = None, max_inflight: int = 0, warm: bool = True, high_group: int = 0,
+               max_spec_decode: int = 0, max_spec_prefill: int = 0) -> Dict:
     from paper_2410_22134_b200 import binding as B
     from paper_2410_22134_b200.engine import ProMoE
 
@@ -28,11 +29,15 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
     n_moe = s.n_layers - s.n_dense_layers
     C = cache_slots // n_moe
     eng = ProMoE(weights, cache_slots=cache_slots, stride=stride, chunk_bytes=chunk_bytes,
-                 predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight, high_group=high_group)
+                 predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight, high_group=high_group,
+                 max_spec_decode=max_spec_decode, max_spec_prefill=max_spec_prefill)
     use_pred = predictor_mode == B.PRED_MLP
     ora = OracleModel(weights, stride=stride, slots_per_layer=C, use_predictor=use_pred)
     sim = ProMoECacheSim(n_moe, s.n_experts, C, warm=bool(flags & B.F_WARM))
     rep = ParityReport()
+    # library defaults (include/promoe.h): decode top_k allocations per push, prefill none
+    ms_dec = s.top_k if max_spec_decode == 0 else max(0, max_spec_decode)
+    ms_pre = max(0, max_spec_prefill)
     all_logits = []
     try:
         ids = [int(x) for x in prompt]
@@ -41,7 +46,7 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
         tr = eng.trace(T)
         st = oracle_step_matching(ora, ids, tr["sel"], rep)
         compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred)
-        compare_cache(sim, tr, stride, use_pred)
+        compare_cache(sim, tr, stride, use_pred, ms_pre)
         all_logits.append(logits)
         nxt = st.next_token
         for i in range(decode_steps):
@@ -50,7 +55,7 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
             tr = eng.trace(1)
             st = oracle_step_matching(ora, [tok], tr["sel"], rep)
             compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred)
-            compare_cache(sim, tr, stride, use_pred)
+            compare_cache(sim, tr, stride, use_pred, ms_dec)
             all_logits.append(logits)
             nxt = st.next_token
         stats = eng.stats()

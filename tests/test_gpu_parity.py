@@ -62,6 +62,15 @@ def test_config1_variants(chunk, mode, stride, slots, warm):
         assert out["stats"]["misses"] == 0 and out["stats"]["h2d_bytes"] == 0
 
 
+@pytest.mark.parametrize("ms_dec,ms_pre", [(1, 0), (-1, 2), (2, 4)])
+def test_max_spec_variants(ms_dec, ms_pre):
+    """Knob G3: allocations allowed per PushPredicted (decode / prefill) — traces bit-exact for every setting."""
+    cfg = synth.get_config("c1")
+    w = synth.make_weights(cfg, predictor="skip")
+    out = run_parity(cfg, w, synth.make_prompt(cfg), 10, max_spec_decode=ms_dec, max_spec_prefill=ms_pre)
+    _report(f"c1 max_spec {ms_dec}/{ms_pre}", out)
+
+
 def test_config1b_tcgen05():
     """c1 with bf16 weights through the tcgen05 prefill path (c1b exercises the tensor-core path)."""
     from paper_2410_22134_b200 import binding as B

@@ -225,3 +225,28 @@ def test_cancelled_prediction_keeps_slot_until_lru_evicts_it():
     sim.begin_step()
     rec = sim.push_precise(0, [3])                # 7 is now the LRU victim
     assert rec.victim == [7]
+
+
+# ---- max_spec knob (SURVEY G3 / DESIGN G7): allocations allowed per PushPredicted --------------------------------
+def test_max_spec_zero_only_touches():
+    """max_spec = 0: a push never allocates; cached predictions are touched (Alg. 2 l.3-5), the rest SKIP, and the
+    slot set is unchanged — so demand misses follow the textbook LRU with extra touches."""
+    from oracle.cache_sim import ACT_SKIP, ACT_TOUCH, ProMoECacheSim
+    sim = ProMoECacheSim(1, 8, 4, warm=True)          # slots: experts 0,1,2,3 ; 0 oldest
+    rec = sim.push_predicted(0, [5, 1, 6, 0], max_spec=0)
+    assert rec.action == [ACT_SKIP, ACT_TOUCH, ACT_SKIP, ACT_TOUCH]
+    assert sorted(sim.slot_expert[0]) == [0, 1, 2, 3] and sim.stats.pred_allocs == 0
+    # LRU order is now 2, 3, 1, 0 (oldest first): a demand miss evicts 2
+    out = sim.push_precise(0, [7])
+    assert out.victim == [2]
+
+
+def test_max_spec_limits_allocations_in_listed_order():
+    from oracle.cache_sim import ACT_ALLOC, ACT_SKIP, ACT_TOUCH, ProMoECacheSim
+    sim = ProMoECacheSim(1, 8, 4, warm=True)
+    rec = sim.push_predicted(0, [5, 6, 1, 7], max_spec=1)
+    assert rec.action == [ACT_ALLOC, ACT_SKIP, ACT_TOUCH, ACT_SKIP]
+    assert rec.victim[0] == 0 and sim.stats.pred_allocs == 1
+    a = ProMoECacheSim(1, 8, 4, warm=True); b = ProMoECacheSim(1, 8, 4, warm=True)
+    ra = a.push_predicted(0, [5, 6, 1, 7]); rb = b.push_predicted(0, [5, 6, 1, 7], max_spec=4)
+    assert ra.as_tuples() == rb.as_tuples() and a.slot_expert == b.slot_expert    # None ≡ no limit
