@@ -64,6 +64,7 @@ typedef struct {
 #define PROMOE_F_REORDER 2   /* reordered inference: cached -> being prefetched -> missing */
 #define PROMOE_F_WARM 4      /* warm start: experts 0..C-1 resident in every layer (G4) */
 #define PROMOE_F_TRACE 8     /* record routing / permutation / cache traces for promoe_get_trace */
+#define PROMOE_F_NOFUSE 32  /* decode with the unfused per-op kernels (19 launches per layer) instead of the fused 7 */
 #define PROMOE_F_TENSOR 16   /* prefill GEMMs on tcgen05 tensor cores (bf16 weights only); else SIMT fp32 */
 
 typedef struct {

@@ -89,7 +89,7 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->perm, (size_t)Lm * T * k)); CK(dalloc(&h->inv, (size_t)Lm * T * k));
     CK(dalloc(&h->pred_list, (size_t)Lm * (1 + E))); CK(dalloc(&h->trace_precise, (size_t)Lm * (1 + 5 * E)));
     CK(dalloc(&h->trace_pred, (size_t)Lm * (1 + 4 * E))); CK(dalloc(&h->row_of, (size_t)k)); CK(dalloc(&h->n_prob, (size_t)1));
-    CK(dalloc(&h->problems, (size_t)E)); CK(dalloc(&h->shared_prob, (size_t)L)); CK(dalloc(&h->err_dev, (size_t)1));
+    CK(dalloc(&h->problems, (size_t)E)); CK(dalloc(&h->shared_prob, (size_t)L)); CK(dalloc(&h->err_dev, (size_t)1)); CK(dalloc(&h->attn_cnt, (size_t)s.n_q_heads));
     if ((op->flags & PROMOE_F_TENSOR) && s.wdtype == 1) {
       h->tc = tc_create(&h->err);
       if (!h->tc) return PROMOE_ECUDA;
@@ -123,6 +123,9 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(cudaHostAlloc((void**)&h->cmd_host, sizeof(LayerCmd) * Lm, cudaHostAllocMapped));
     memset((void*)h->cmd_host, 0, sizeof(LayerCmd) * Lm);
     CK(cudaHostGetDevicePointer((void**)&h->cmd_dev, (void*)h->cmd_host, 0));
+    CK(cudaHostAlloc((void**)&h->logits_pin, sizeof(float) * (size_t)s.vocab, cudaHostAllocDefault));
+    CK(cudaHostAlloc((void**)&h->ids_pin, sizeof(int32_t) * (size_t)T, cudaHostAllocDefault));
+    CK(cudaHostAlloc((void**)&h->err_pin, sizeof(int), cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->flagsrc_host, sizeof(uint32_t) * 65536, cudaHostAllocDefault));
     {
       cudaDriverEntryPointQueryResult qr;
@@ -158,7 +161,7 @@ extern "C" void promoe_destroy(promoe_t* h) {
   void* bufs[] = {h->x, h->u1, h->u, h->qkv, h->attn, h->zraw, h->p1, h->p2, h->act, h->yexp, h->sact, h->sy,
                   h->sgate, h->attn_ws, h->xf, h->logits, h->kcache, h->vcache, h->cos_t, h->sin_t, h->ids, h->sel,
                   h->count, h->offset, h->perm, h->inv, h->gates, h->margin, h->z, h->pred_list, h->trace_precise,
-                  h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->slots, h->flags,
+                  h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->attn_cnt, h->slots, h->flags,
                   h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock};
   for (void* b : bufs) if (b) cudaFree(b);
   if (h->xsA) cudaFree(h->xsA);
@@ -167,6 +170,9 @@ extern "C" void promoe_destroy(promoe_t* h) {
   if (h->tc) tc_destroy(h->tc);
   if (h->cmd_host) cudaFreeHost((void*)h->cmd_host);
   if (h->flagsrc_host) cudaFreeHost(h->flagsrc_host);
+  if (h->logits_pin) cudaFreeHost(h->logits_pin);
+  if (h->ids_pin) cudaFreeHost(h->ids_pin);
+  if (h->err_pin) cudaFreeHost(h->err_pin);
   for (auto& p : h->phys) if (p.done) cudaEventDestroy(p.done);
   for (auto e : h->ev_ring) if (e) cudaEventDestroy(e);
   for (auto e : h->ev_ring_start) if (e) cudaEventDestroy(e);
@@ -235,6 +241,7 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
   CK(cudaMemset(h->tbl.origin, 0, (size_t)Lm * C));
   CK(cudaMemset(h->flags, 0, (size_t)Lm * C * h->n_chunks * 4));
   CK(cudaMemset(h->err_dev, 0, 4));
+  CK(cudaMemset(h->attn_cnt, 0, (size_t)h->s.n_q_heads * 4));
   h->mirror = se;
   h->low.clear();
   if (ce_retire(h, true)) return PROMOE_ECUDA;

@@ -65,6 +65,12 @@ struct promoe {
           *n_prob = nullptr;
   pmk::FfnProblem *problems = nullptr, *shared_prob = nullptr;
   int* err_dev = nullptr;
+  // pinned host staging: no pageable buffer is ever handed to an async copy (a pageable D2H above the driver's
+  // staging threshold was seen to stall the copy stream for seconds while a flag-gated kernel was resident)
+  float* logits_pin = nullptr;
+  int32_t* ids_pin = nullptr;
+  int* err_pin = nullptr;
+  int* attn_cnt = nullptr;       // [n_q_heads] arrival counters of the fused decode attention (zero between launches)
   // tcgen05 path (PROMOE_F_TENSOR, bf16 weights): activation operands as bf16 hi/lo planes; the lo plane of each
   // buffer starts *_half elements after the hi plane
   pmk::TcContext* tc = nullptr;

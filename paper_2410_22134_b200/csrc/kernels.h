@@ -43,6 +43,7 @@ void launch_pred_list(const float* p, int T, int E, int k, int cap, int32_t* pre
 void launch_permute(const int32_t* sel, int T, int k, int E, int32_t* count, int32_t* offset, int32_t* perm,
                     int32_t* inv, cudaStream_t st);
 
+struct RouteFuse;
 // A6 slot table.  State of ONE model (all MoE layers) lives in device memory, laid out by SlotTable.
 struct SlotTable {
   int32_t* slot_expert;      // [Lm, C]  expert in slot or -1
@@ -72,7 +73,8 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* j_of_problem, LayerCmd* cmd,
-                       uint32_t seq, int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st);
+                       uint32_t seq, int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st,
+                       const RouteFuse* fuse = nullptr);
 
 // A9 decode expert FFN (GEMV, T == 1) over a problem list in launch order.
 //  gateup: act[p, i] = silu(Wg_p[i,:].u) * (Wu_p[i,:].u)     down: y[p, h] = Wd_p[h,:].act[p,:]
@@ -88,6 +90,29 @@ void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src
                                  int act_stride, int wdtype, cudaStream_t st);
 void launch_ffn_down_gemm_simt(const float* act, int act_stride, const FfnProblem* probs, int p0, int np,
                                int max_rows, int rows_override, int max_inter, int H, float* y, int wdtype, cudaStream_t st);
+
+// ---- fused decode kernels (kernels_decode.cu) ---------------------------------------------------------------
+struct GemvSeg { const void* w; float* out; int n; int flags; };
+struct NormGemvArgs {
+  const float* x; const float* gain; float eps; int K;
+  float* u_out;                       // normalised vector (written by CTA 0) or nullptr
+  GemvSeg seg[4]; int nseg;           // plain row segments (router | predictor W1 | shared gate ...)
+  const void* wg; const void* wu; float* act; int n_sw;   // SwiGLU pairs of the resident FFN (n_sw = 0: none)
+  int n_rows_total;                   // filled by the launcher
+};
+void launch_norm_multi_gemv(const NormGemvArgs& a, int wdtype, cudaStream_t st);
+void launch_attn_decode_fused(const float* qkv, const float* cos_t, const float* sin_t, float* kcache, float* vcache,
+                              float* ws, float* out, int* counters, int pos, int nq, int nkv, int d, int max_seq,
+                              int nsplit, cudaStream_t st);
+void launch_ffn_down_combine(const float* act, int act_stride, const FfnProblem* probs, const int32_t* row_of,
+                             const float* gates, int k, const FfnProblem* shared, const float* sact,
+                             const float* sgate_logit, int H, float* x, int wdtype, size_t chunk_bytes, int* err,
+                             cudaStream_t st);
+// fused front end of the slot-table kernel for T == 1: top-k + gates on (zraw + bias), predictor W2 GEMV + list
+struct RouteFuse {
+  const float* zraw; const float* bias; float* z_out; int32_t* sel; float* gates; float* margin;
+  const float* p1; const void* pred_w2; int ph; int wdtype; int32_t* pred_out; int k; int cap;
+};
 
 // A10 combine: out[t,:] = hres[t,:] + sum_j (fixed j order) g[t,j] * yexp[row(t,j),:] (+ sgate[t]*shared[t,:]).
 //  row(t,j) = inv[t*k+j] (prefill) or pos_of_j[j] (decode).  shared may be nullptr; sgate nullptr => 1.

@@ -4,39 +4,6 @@
 
 namespace pmk {
 
-// ---------------------------------------------------------------------------------------------------------
-// Warp-shuffle top-k.  One warp per token; lane holds experts lane, lane+32, ... (NPL per lane, E <= 32*NPL).
-// Selection order: descending value, ties → lower index (BASELINE.json north_star).
-// Returns in lane j (j < k) nothing: winners are written by lane 0 through the callback arrays.
-template <int NPL>
-__device__ __forceinline__ void warp_topk(float (&v)[NPL], int E, int k, int lane, int* sel_out, float* val_out,
-                                          float* next_val) {
-  // sel_out / val_out: per-warp shared or global arrays of length k, written by lane 0.
-  for (int it = 0; it <= k; ++it) {
-    float best = -INFINITY; int bi = 0x7fffffff;
-#pragma unroll
-    for (int q = 0; q < NPL; ++q) {
-      const int e = lane + 32 * q;
-      if (e < E && (v[q] > best || (v[q] == best && e < bi))) { best = v[q]; bi = e; }
-    }
-    // lanes with nothing left keep bi = INT_MAX and best = -inf
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      const float ob = __shfl_xor_sync(0xffffffffu, best, o);
-      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-      if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
-    }
-    if (it == k) { *next_val = (bi == 0x7fffffff) ? -INFINITY : best; break; }
-    if (lane == 0) { sel_out[it] = bi; val_out[it] = best; }
-    // retire the winner
-#pragma unroll
-    for (int q = 0; q < NPL; ++q)
-      if (lane + 32 * q == bi) v[q] = -INFINITY;
-    if (it + 1 == E) { *next_val = -INFINITY; break; }   // k == E: nothing left
-  }
-}
-
-constexpr int kMaxK = 16;
 
 // A4: z (+bias) → sel [T,k], gates = softmax over the selected logits (Σ = 1, reading G8), margin.
 template <int NPL>

@@ -33,15 +33,15 @@ struct SlotView {
 };
 
 __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, int stride, int max_spec,
-                                                         const int32_t* __restrict__ sel, int T, int k,
+                                                         const int32_t* sel, int T, int k,
                                                          const int32_t* __restrict__ offset,
-                                                         const int32_t* __restrict__ pred_list,
+                                                         const int32_t* pred_list,
                                                          const uint8_t* slot_base, size_t slot_bytes,
                                                          const uint32_t* flag_base, int flags_per_slot, int H,
                                                          int inter, int wbytes, FfnProblem* problems,
                                                          int32_t* n_problems, int32_t* row_of, LayerCmd* cmd,
                                                          uint32_t seq, int32_t* trace_precise,
-                                                         int32_t* trace_pred) {
+                                                         int32_t* trace_pred, RouteFuse rf) {
   __shared__ uint8_t needed[kMaxE];
   __shared__ uint8_t prot[kMaxE];
   __shared__ int16_t order[kMaxE];
@@ -59,6 +59,49 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   __shared__ unsigned long long t_clock;
   __shared__ int32_t s_pred[kMaxE + 1];
   const int E = tbl.E, C = tbl.C;
+  // ---- fused decode front end (T == 1): router top-k + gates, predictor W2 GEMV + predicted list
+  if (rf.zraw) {
+    __shared__ float s_p2[kMaxE];
+    __shared__ int f_sel[2][kMaxK];
+    __shared__ float f_val[2][kMaxK];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (rf.pred_out) {
+      for (int e = warp; e < E; e += 8) {
+        const float v = rf.wdtype == 0 ? row_dot<float>((const float*)rf.pred_w2 + (size_t)e * rf.ph, rf.p1, rf.ph, lane)
+                                       : row_dot<__nv_bfloat16>((const __nv_bfloat16*)rf.pred_w2 + (size_t)e * rf.ph, rf.p1, rf.ph, lane);
+        if (lane == 0) s_p2[e] = v;
+      }
+    }
+    __syncthreads();
+    if (warp == 0) {            // A4: top-k by logit (ties → lower index), gates = softmax over the selected
+      float v[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const int e = lane + 32 * q;
+        v[q] = -INFINITY;
+        if (e < E) { v[q] = rf.zraw[e] + (rf.bias ? rf.bias[e] : 0.f); if (rf.z_out) rf.z_out[e] = v[q]; }
+      }
+      float nxt;
+      warp_topk<8>(v, E, rf.k, lane, f_sel[0], f_val[0], &nxt);
+      __syncwarp();
+      const float zmax = f_val[0][0];
+      const float ex = (lane < rf.k) ? expf(f_val[0][lane] - zmax) : 0.f;
+      const float sum = warp_sum(ex);
+      if (lane < rf.k) { rf.sel[lane] = f_sel[0][lane]; rf.gates[lane] = ex / sum; }
+      if (lane == 0 && rf.margin) rf.margin[0] = (rf.k < E) ? f_val[0][rf.k - 1] - nxt : INFINITY;
+    } else if (warp == 1 && rf.pred_out) {   // A5: top-k of the predictor scores, listed by descending score
+      float v[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) { const int e = lane + 32 * q; v[q] = (e < E) ? s_p2[e] : -INFINITY; }
+      float nxt;
+      warp_topk<8>(v, E, rf.k, lane, f_sel[1], f_val[1], &nxt);
+      __syncwarp();
+      const int np_ = min(rf.k, rf.cap);
+      if (lane == 0) rf.pred_out[0] = np_;
+      if (lane < np_) rf.pred_out[1 + lane] = f_sel[1][lane];
+    }
+    __syncthreads();   // sel / pred_out (global) are read below by this same block
+  }
   const int mt_ = m + stride;
   const bool have_t = pred_list != nullptr && mt_ < tbl.Lm;
   for (int i = threadIdx.x; i < C; i += blockDim.x) {
@@ -201,11 +244,13 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
-                       int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st) {
+                       int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf) {
   (void)reorder;
+  RouteFuse f{};
+  if (rf) f = *rf;
   slot_table_kernel<<<1, 256, 0, st>>>(tbl, m, stride, max_spec, sel, T, k, offset, pred_list, slot_base, slot_bytes,
                                        flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of,
-                                       cmd, seq, trace_precise, trace_pred);
+                                       cmd, seq, trace_precise, trace_pred, f);
 }
 
 }  // namespace pmk

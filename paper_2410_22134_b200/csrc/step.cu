@@ -17,6 +17,9 @@
 #include "engine.h"
 #include "gemm_tc.h"
 
+#include <chrono>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 using namespace pmk;
@@ -105,6 +108,63 @@ static int expert_batch(promoe_t* h, const int32_t* perm, int i, int j, int max_
 
 #define RC(expr) do { int rc_ = (expr); if (rc_ != PROMOE_OK) return rc_; } while (0)
 
+// One layer of the batch-1 decode step with the fused kernels of kernels_decode.cu (7 launches instead of 19).
+static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
+  const promoe_shape_t& s = h->s;
+  const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter, wd = s.wdtype;
+  const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim;
+  cudaStream_t cs = h->cs;
+  const size_t kv_layer = (size_t)nkv * s.max_seq * d;
+  NormGemvArgs a{};                                                                      // K1
+  a.x = h->x; a.gain = h->ln1[l]; a.eps = s.rms_eps; a.K = H;
+  a.seg[0] = GemvSeg{h->wqkv[l], h->qkv, h->qkv_w, 0}; a.nseg = 1;
+  launch_norm_multi_gemv(a, wd, cs);
+  launch_attn_decode_fused(h->qkv, h->cos_t, h->sin_t, h->kcache + (size_t)l * kv_layer, h->vcache + (size_t)l * kv_layer,   // K2
+                           h->attn_ws, h->attn, h->attn_cnt, pos0, nq, nkv, d, s.max_seq, h->nsplit, cs);
+  launch_gemv(h->attn, h->wo[l], h->x, H, nq * d, wd, LIN_ACC, cs);                      // K3
+  NormGemvArgs b{};                                                                      // K4
+  b.x = h->x; b.gain = h->ln2[l]; b.eps = s.rms_eps; b.K = H; b.u_out = h->u;
+  if (l < s.n_dense_layers) {
+    b.wg = h->ffn_gate[l]; b.wu = h->ffn_up[l]; b.act = h->sact; b.n_sw = s.dense_inter;
+    launch_norm_multi_gemv(b, wd, cs);
+    launch_ffn_down_combine(nullptr, 0, nullptr, nullptr, nullptr, 0, h->shared_prob + l, h->sact, nullptr, H, h->x, wd,
+                            h->chunk_bytes, h->err_dev, cs);
+    return PROMOE_OK;
+  }
+  const int m = l - s.n_dense_layers;
+  const uint32_t seq = step_seq * 4096u + (uint32_t)m + 1u;
+  int32_t* sel = h->sel + (size_t)m * h->maxT * k;
+  float* gates = h->gates + (size_t)m * h->maxT * k;
+  const bool mlp = h->o.predictor_mode == PROMOE_PRED_MLP;
+  b.seg[b.nseg++] = GemvSeg{h->router[l], h->zraw, E, 0};
+  if (mlp) b.seg[b.nseg++] = GemvSeg{h->pred_w1[l], h->p1, s.pred_hidden, LIN_RELU};
+  if (s.n_shared_inter && s.shared_gate) b.seg[b.nseg++] = GemvSeg{h->shared_gate_w[l], h->sgate, 1, 0};
+  launch_norm_multi_gemv(b, wd, cs);
+  int32_t* plist = (mlp || h->o.predictor_mode == PROMOE_PRED_TRACE) ? h->pred_list + (size_t)m * (1 + E) : nullptr;
+  RouteFuse rf{};                                                                        // K5
+  rf.zraw = h->zraw; rf.bias = s.router_bias ? h->router_bias[l] : nullptr; rf.z_out = h->z + (size_t)m * h->maxT * E;
+  rf.sel = sel; rf.gates = gates; rf.margin = h->margin + (size_t)m * h->maxT;
+  rf.p1 = h->p1; rf.pred_w2 = mlp ? h->pred_w2[l] : nullptr; rf.ph = s.pred_hidden; rf.wdtype = wd;
+  rf.pred_out = mlp ? plist : nullptr; rf.k = k; rf.cap = C;
+  launch_slot_table(h->tbl, m, h->o.stride, h->max_spec_decode, sel, 1, k, nullptr, plist,
+                    (h->o.flags & PROMOE_F_REORDER) != 0, h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb, h->problems,
+                    h->n_prob, h->row_of, h->cmd_dev + m, seq, h->trace_precise + (size_t)m * (1 + 5 * E),
+                    (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf);
+  // The shared expert's gate/up GEMV (resident weights) is enqueued BEHIND the slot-table kernel and BEFORE the host
+  // looks at the command: it covers the device→host→device hand-over.  The flag-gated kernels K6/K7 must NOT be
+  // enqueued before the copies they wait for: when the driver multiplexes both streams onto one hardware queue a
+  // resident spinning kernel starves the copy (seen on B200: 4 s flag time-outs), so copies always go first.
+  if (s.n_shared_inter)
+    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, cs);
+  RC(ce_wait_cmd(h, m, seq));                                                            // A7
+  RC(ce_process_cmd(h, m, nullptr));
+  launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
+  launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, s.n_shared_inter ? h->shared_prob + l : nullptr,   // K7
+                          h->sact, (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, H, h->x, wd, h->chunk_bytes,
+                          h->err_dev, cs);
+  return PROMOE_OK;
+}
+
 static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_out) {
   const promoe_shape_t& s = h->s;
   const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter;
@@ -128,7 +188,8 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
 
   h->want_done_events = T > 1;
   if (T > 1) RC(ce_retire(h, true));   // prefill orders compute after fills with events: start from a drained copy stream
-  CKS(cudaMemcpyAsync(h->ids, ids_host, (size_t)T * 4, cudaMemcpyHostToDevice, cs));
+  memcpy(h->ids_pin, ids_host, (size_t)T * 4);
+  CKS(cudaMemcpyAsync(h->ids, h->ids_pin, (size_t)T * 4, cudaMemcpyHostToDevice, cs));
   CKS(cudaEventRecord(h->step_start, cs));
   if (h->o.flags & PROMOE_F_TRACE) {
     CKS(cudaMemsetAsync(h->trace_pred, 0, (size_t)Lm * (1 + 4 * E) * 4, cs));
@@ -137,7 +198,9 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
   launch_embed(h->ids, h->emb, h->x, T, H, wd, cs);
   const size_t kv_layer = (size_t)nkv * s.max_seq * d;
   std::vector<int> deferred;
+  const bool fused = T == 1 && !(h->o.flags & PROMOE_F_NOFUSE);
   for (int l = 0; l < s.n_layers; ++l) {
+    if (fused) { RC(decode_layer_fused(h, l, step_seq, pos0)); continue; }
     // ---- attention block (A1-A3)
     launch_rmsnorm(h->x, h->ln1[l], h->u1, T, H, s.rms_eps, cs);
     RC(linear(h, h->u1, h->wqkv[l], h->qkv, T, h->qkv_w, H, 0));
@@ -240,18 +303,23 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     }
   }
   // ---- last token: final norm + lm_head
-  launch_rmsnorm(h->x + (size_t)(T - 1) * H, h->final_norm, h->xf, 1, H, s.rms_eps, cs);
-  launch_gemv(h->xf, h->lm_head, h->logits, s.vocab, H, wd, 0, cs);
+  {
+    NormGemvArgs f{};
+    f.x = h->x + (size_t)(T - 1) * H; f.gain = h->final_norm; f.eps = s.rms_eps; f.K = H;
+    f.seg[0] = GemvSeg{h->lm_head, h->logits, s.vocab, 0}; f.nseg = 1;
+    launch_norm_multi_gemv(f, wd, cs);
+  }
   CKS(cudaEventRecord(h->step_end, cs));
-  int err_host = 0;
-  if (logits_out) CKS(cudaMemcpyAsync(logits_out, h->logits, (size_t)s.vocab * 4, cudaMemcpyDeviceToHost, cs));
-  CKS(cudaMemcpyAsync(&err_host, h->err_dev, 4, cudaMemcpyDeviceToHost, cs));
+  if (logits_out) CKS(cudaMemcpyAsync(h->logits_pin, h->logits, (size_t)s.vocab * 4, cudaMemcpyDeviceToHost, cs));
+  CKS(cudaMemcpyAsync(h->err_pin, h->err_dev, 4, cudaMemcpyDeviceToHost, cs));
   // keep feeding LOW chunks while the tail of the step drains (no-preempt mode may leave some queued)
   while (cudaStreamQuery(cs) == cudaErrorNotReady) {
     int rc = ce_pump_low(h);
     if (rc) return rc;
   }
   CKS(cudaStreamSynchronize(cs));
+  const int err_host = *h->err_pin;
+  if (logits_out) memcpy(logits_out, h->logits_pin, (size_t)s.vocab * 4);
   float ms = 0.f;
   CKS(cudaEventElapsedTime(&ms, h->step_start, h->step_end));
   int rc = ce_retire(h, false);

@@ -71,6 +71,17 @@ def test_max_spec_variants(ms_dec, ms_pre):
     _report(f"c1 max_spec {ms_dec}/{ms_pre}", out)
 
 
+@pytest.mark.parametrize("name", ["c1", "c1b"])
+def test_config1_unfused_decode(name):
+    """PROMOE_F_NOFUSE: the per-op decode kernels (kept as the readable reference of the fused ones)."""
+    from paper_2410_22134_b200 import binding as B
+    cfg = synth.get_config(name)
+    w = synth.make_weights(cfg, predictor="skip")
+    out = run_parity(cfg, w, synth.make_prompt(cfg), cfg.decode_steps,
+                     flags=B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_NOFUSE)
+    _report(f"{name}/unfused", out)
+
+
 def test_config1b_tcgen05():
     """c1 with bf16 weights through the tcgen05 prefill path (c1b exercises the tensor-core path)."""
     from paper_2410_22134_b200 import binding as B
