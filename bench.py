@@ -187,21 +187,44 @@ def aggregate(local_tokens: float, local_seconds: float, dist=None):
     return float(tok.item()), float(sec.item())
 
 
-def run_request(eng, cfg, prompt, decode_ids, greedy: bool):
-    """reset → prefill → decode_steps × decode.  Returns per-phase device ms, wall s, stats deltas."""
+def run_request(eng, cfg, prompt, decode_ids, greedy: bool, record=None, inject=None):
+    """reset → prefill → decode_steps × decode.  Returns per-phase device ms, wall s, stats deltas.
+    record: list that receives, per step, the needed experts of every MoE layer (from the library's routing trace);
+    inject: such a list from an earlier pass — step t's predictor at layer m is given the TRUE needed set of layer
+    m+stride (oracle-routing predictor, the upper bound of BASELINE.json configs[4]); routing does not depend on
+    the cache, so a reactive pass and the injected pass see the same selections."""
     import numpy as np
     eng.reset()
+    Lm, k = eng.n_moe, eng.s.top_k
+
+    def needed_of_last_step(T):
+        from paper_2410_22134_b200 import binding as B
+        sel = B.promoe_get_trace(eng.h, B.TRACE_SEL, np.int32).reshape(Lm, T * k)
+        return [sorted(set(int(e) for e in row)) for row in sel]
+
+    def inject_step(t):
+        need, st = inject[t], eng.stride
+        eng.set_prediction_trace([need[m + st][:eng.slots_per_layer] if m + st < Lm else None for m in range(Lm)])
+
     s0 = eng.stats()
+    if inject is not None:
+        inject_step(0)
     w0 = time.perf_counter()
     logits = eng.prefill(prompt)
     w1 = time.perf_counter()
     s1 = eng.stats()
+    if record is not None:
+        record.append(needed_of_last_step(len(prompt)))
     tok = int(np.argmax(logits))
     dec_ms = []
     for i in range(cfg.decode_steps):
         if not greedy:
             tok = int(decode_ids[i])
+        if inject is not None:
+            inject_step(1 + i)
         logits = eng.decode(tok)
+        if record is not None:
+            record.append(needed_of_last_step(1))
         dec_ms.append(eng.stats()["last_step_ms"])
         if greedy:
             tok = int(np.argmax(logits))
@@ -224,7 +247,26 @@ def run_ours(args, cfg, rank, world, dist):
     torch.cuda.set_device(local)
     peaks = load_peaks()
     s = cfg.shape
-    weights = synth.make_weights(cfg, predictor="skip" if args.predictor == "none" else args.predictor)
+    pred_kind = "skip" if args.predictor in ("none", "trace") else args.predictor
+    if world > 1:
+        # replicas share ONE host copy of the routed experts (a /dev/shm mapping drawn by local rank 0; every rank's
+        # library registers it with cudaHostRegister) — 8 private pinned copies of 25-90 GB would not fit the host
+        n_moe = s.n_layers - s.n_dense_layers
+        per = 3 * s.hidden * s.expert_inter
+        dt = torch.float32 if s.wdtype == 0 else torch.bfloat16
+        path = f"/dev/shm/promoe_experts_{os.environ.get('MASTER_PORT', '0')}_{cfg.name}"
+        if local == 0:
+            buf = torch.from_file(path, shared=True, size=n_moe * s.n_experts * per, dtype=dt).view(n_moe, s.n_experts, per)
+            weights = synth.make_weights(cfg, predictor=pred_kind, experts_buf=buf, fill_experts=True)
+        dist.barrier()
+        if local != 0:
+            buf = torch.from_file(path, shared=True, size=n_moe * s.n_experts * per, dtype=dt).view(n_moe, s.n_experts, per)
+            weights = synth.make_weights(cfg, predictor=pred_kind, experts_buf=buf, fill_experts=False)
+        dist.barrier()
+        if local == 0:
+            os.unlink(path)          # the mappings keep the memory alive until the processes exit
+    else:
+        weights = synth.make_weights(cfg, predictor=pred_kind)
     wb = 4 if s.wdtype == 0 else 2
     Be = 3 * s.hidden * s.expert_inter * wb
     h2d_gbs = B.promoe_measure_h2d(256 << 20, 2, 5)
@@ -232,18 +274,27 @@ def run_ours(args, cfg, rank, world, dist):
     decode_ids = synth.make_decode_ids(cfg).tolist()
     greedy = args.decode == "greedy"
     flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | (B.F_TENSOR if args.tensor else 0)
+    inject = None
+    if args.predictor == "trace":      # pass 0: reactive run that records the routing of every step
+        rec_eng = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, predictor_mode=B.PRED_NONE,
+                         flags=flags | B.F_TRACE, device=f"cuda:{local}")
+        inject = []
+        run_request(rec_eng, cfg, prompt, decode_ids, greedy, record=inject)
+        rec_eng.close()
+    pmode = {"none": B.PRED_NONE, "trace": B.PRED_TRACE}.get(args.predictor, B.PRED_MLP)
     eng = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_mb << 20,
-                 predictor_mode=B.PRED_MLP if args.predictor != "none" else B.PRED_NONE, flags=flags,
-                 max_inflight=args.inflight, max_spec_decode=args.max_spec_decode, max_spec_prefill=args.max_spec_prefill)
+                 predictor_mode=pmode, flags=flags,
+                 max_inflight=args.inflight, max_spec_decode=args.max_spec_decode, max_spec_prefill=args.max_spec_prefill,
+                 device=f"cuda:{local}")
     for _ in range(args.warmup):
-        run_request(eng, cfg, prompt, decode_ids, greedy)
+        run_request(eng, cfg, prompt, decode_ids, greedy, inject=inject)
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     clocks = ClockSampler(local)
     clocks.start()
     t0 = time.perf_counter()
-    reqs = [run_request(eng, cfg, prompt, decode_ids, greedy) for _ in range(args.steps)]
+    reqs = [run_request(eng, cfg, prompt, decode_ids, greedy, inject=inject) for _ in range(args.steps)]
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
@@ -313,8 +364,8 @@ def run_ours(args, cfg, rank, world, dist):
     allhit = None
     if rank == 0 and not args.no_allhit:
         n_moe = s.n_layers - s.n_dense_layers
-        full = ProMoE(weights, cache_slots=n_moe * s.n_experts, stride=cfg.stride, predictor_mode=B.PRED_MLP if args.predictor != "none" else B.PRED_NONE,
-                      flags=flags, chunk_bytes=args.chunk_mb << 20)
+        full = ProMoE(weights, cache_slots=n_moe * s.n_experts, stride=cfg.stride, predictor_mode=B.PRED_NONE if args.predictor in ("none", "trace") else B.PRED_MLP,
+                      flags=flags, chunk_bytes=args.chunk_mb << 20, device=f"cuda:{local}")
         run_request(full, cfg, prompt, decode_ids, greedy)
         r = run_request(full, cfg, prompt, decode_ids, greedy)
         full.close()
@@ -363,7 +414,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c2")
-    ap.add_argument("--predictor", default="skip", choices=["skip", "random", "none"])
+    ap.add_argument("--predictor", default="skip", choices=["skip", "random", "none", "trace"],
+                    help="skip: training-free MLP weights (default); none: reactive cache; trace: oracle-routing upper bound")
     ap.add_argument("--decode", default="random", choices=["random", "greedy"],
                     help="decode ids: seeded random (locality-neutral, default) or greedy argmax")
     ap.add_argument("--chunk-mb", type=int, default=4)

@@ -262,16 +262,28 @@ extern "C" int promoe_load_experts(promoe_t* h, const void* const* host_ptrs, si
   if (expert_bytes != h->Be) { h->err = "load_experts: expert_bytes != 3*H*I*sizeof(w)"; return PROMOE_EINVAL; }
   const size_t n = (size_t)h->Lm * h->s.n_experts;
   h->expert_host.assign(host_ptrs, host_ptrs + n);
+  bool contiguous = true;
   for (size_t i = 0; i < n; ++i) {
     if (!host_ptrs[i]) { h->err = "load_experts: null expert pointer"; return PROMOE_EINVAL; }
+    if (i && (const char*)host_ptrs[i] != (const char*)host_ptrs[i - 1] + expert_bytes) contiguous = false;
+  }
+  auto unregistered = [](const void* p) {
     cudaPointerAttributes at{};
-    cudaError_t e = cudaPointerGetAttributes(&at, host_ptrs[i]);
-    if (e != cudaSuccess || at.type == cudaMemoryTypeUnregistered) {
-      (void)cudaGetLastError();
-      CK(cudaHostRegister((void*)host_ptrs[i], expert_bytes, cudaHostRegisterDefault));
-      h->registered.push_back((void*)host_ptrs[i]);
-      h->st.registered_host_bytes += expert_bytes;
-    }
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return true; }
+    return at.type == cudaMemoryTypeUnregistered;
+  };
+  if (contiguous && unregistered(host_ptrs[0])) {      // one mapping (e.g. a shared-memory file shared by all ranks)
+    CK(cudaHostRegister((void*)host_ptrs[0], n * expert_bytes, cudaHostRegisterPortable));
+    h->registered.push_back((void*)host_ptrs[0]);
+    h->st.registered_host_bytes += n * expert_bytes;
+  } else {
+    for (size_t i = 0; i < n; ++i)
+      if (unregistered(host_ptrs[i])) {
+        CK(cudaHostRegister((void*)host_ptrs[i], expert_bytes, cudaHostRegisterDefault));
+        h->registered.push_back((void*)host_ptrs[i]);
+        h->st.registered_host_bytes += expert_bytes;
+      }
   }
   h->experts_loaded = true;
   return promoe_init_cache_state(h, true);

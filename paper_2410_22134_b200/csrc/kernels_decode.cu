@@ -257,21 +257,34 @@ __global__ void __launch_bounds__(256) ffn_down_combine_kernel(const float* __re
   __shared__ int s_ni, s_ok;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r0 = blockIdx.x * DC_ROWS;
+  // prologue in parallel: thread j loads problem j (j == k: the shared expert) and waits for the chunk flags of the
+  // down rows this CTA reads; thread 0 then cuts the dot products into items
+  __shared__ FfnProblem s_pb[kMaxK + 1];
+  __shared__ const float* s_xv[kMaxK + 1];
+  __shared__ int s_okj[kMaxK + 1];
+  const int nj = k + (shared ? 1 : 0);
+  if (threadIdx.x < nj) {
+    const int j = threadIdx.x;
+    const int row = (j < k) ? row_of[j] : 0;
+    const FfnProblem pb = (j < k) ? probs[row] : *shared;
+    int ok = 1;
+    if (j < k && pb.flags) {      // bytes of rows [r0, r0 + DC_ROWS) of the down matrix inside the slot image
+      const size_t row_b = (size_t)pb.inter * sizeof(WT), off = 2 * (size_t)pb.inter * H * sizeof(WT);
+      const int c0 = (int)((off + (size_t)r0 * row_b) / chunk_bytes);
+      const int c1 = (int)((off + (size_t)min(H, r0 + DC_ROWS) * row_b - 1) / chunk_bytes);
+      ok = wait_chunks(pb.flags, c0, c1, pb.gen, err);
+    }
+    s_pb[j] = pb; s_xv[j] = (j < k) ? act + (size_t)row * act_stride : sact; s_okj[j] = ok;
+  }
+  __syncthreads();
   if (threadIdx.x == 0) {
     int ni = 0, ok = 1;
-    for (int j = 0; j <= k; ++j) {
-      if (j == k && !shared) break;
-      const FfnProblem pb = (j < k) ? probs[row_of[j]] : *shared;
-      const float* xv = (j < k) ? act + (size_t)row_of[j] * act_stride : sact;
-      if (j < k && pb.flags) {      // bytes of rows [r0, r0 + DC_ROWS) of the down matrix inside the slot image
-        const size_t row_b = (size_t)pb.inter * sizeof(WT), off = 2 * (size_t)pb.inter * H * sizeof(WT);
-        const int c0 = (int)((off + (size_t)r0 * row_b) / chunk_bytes);
-        const int c1 = (int)((off + (size_t)min(H, r0 + DC_ROWS) * row_b - 1) / chunk_bytes);
-        ok = ok && wait_chunks(pb.flags, c0, c1, pb.gen, err);
-      }
-      for (int o = 0; o < pb.inter && ni < DC_MAX_ITEMS; o += DC_PIECE) {
-        it_w[ni] = pb.wd; it_x[ni] = xv; it_ld[ni] = pb.inter; it_off[ni] = o; it_len[ni] = min(DC_PIECE, pb.inter - o);
-        it_j[ni] = j; ++ni;
+    for (int j = 0; j < nj; ++j) {
+      ok = ok && s_okj[j];
+      const int inter = s_pb[j].inter;
+      for (int o = 0; o < inter && ni < DC_MAX_ITEMS; o += DC_PIECE) {
+        it_w[ni] = s_pb[j].wd; it_x[ni] = s_xv[j]; it_ld[ni] = inter; it_off[ni] = o; it_len[ni] = min(DC_PIECE, inter - o);
+        it_j[ni] = (j < k) ? j : k; ++ni;
       }
     }
     s_ni = ni; s_ok = ok;

@@ -32,7 +32,40 @@ struct SlotView {
   }
 };
 
-__global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, int stride, int max_spec,
+// Fused decode front end, instantiated per experts-per-lane count so that only a small piece of code is fetched
+// (a single-CTA kernel runs from a cold instruction cache: code size is latency).
+template <int NPL>
+__device__ __noinline__ void front_route(const RouteFuse& rf, int E, int lane, int* f_sel, float* f_val) {
+  float v[NPL];
+#pragma unroll
+  for (int q = 0; q < NPL; ++q) {
+    const int e = lane + 32 * q;
+    v[q] = -INFINITY;
+    if (e < E) { v[q] = rf.zraw[e] + (rf.bias ? rf.bias[e] : 0.f); if (rf.z_out) rf.z_out[e] = v[q]; }
+  }
+  float nxt;
+  warp_topk<NPL>(v, E, rf.k, lane, f_sel, f_val, &nxt);
+  __syncwarp();
+  const float zmax = f_val[0];
+  const float ex = (lane < rf.k) ? expf(f_val[lane] - zmax) : 0.f;
+  const float sum = warp_sum(ex);
+  if (lane < rf.k) { rf.sel[lane] = f_sel[lane]; rf.gates[lane] = ex / sum; }
+  if (lane == 0 && rf.margin) rf.margin[0] = (rf.k < E) ? f_val[rf.k - 1] - nxt : INFINITY;
+}
+template <int NPL>
+__device__ __noinline__ void front_pred(const RouteFuse& rf, const float* s_p2, int E, int lane, int* f_sel, float* f_val) {
+  float v[NPL];
+#pragma unroll
+  for (int q = 0; q < NPL; ++q) { const int e = lane + 32 * q; v[q] = (e < E) ? s_p2[e] : -INFINITY; }
+  float nxt;
+  warp_topk<NPL>(v, E, rf.k, lane, f_sel, f_val, &nxt);
+  __syncwarp();
+  const int np_ = min(rf.k, rf.cap);
+  if (lane == 0) rf.pred_out[0] = np_;
+  if (lane < np_) rf.pred_out[1 + lane] = f_sel[lane];
+}
+
+__global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, int stride, int max_spec,
                                                          const int32_t* sel, int T, int k,
                                                          const int32_t* __restrict__ offset,
                                                          const int32_t* pred_list,
@@ -66,42 +99,47 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
     __shared__ float f_val[2][kMaxK];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (rf.pred_out) {
-      for (int e = warp; e < E; e += 8) {
-        const float v = rf.wdtype == 0 ? row_dot<float>((const float*)rf.pred_w2 + (size_t)e * rf.ph, rf.p1, rf.ph, lane)
-                                       : row_dot<__nv_bfloat16>((const __nv_bfloat16*)rf.pred_w2 + (size_t)e * rf.ph, rf.p1, rf.ph, lane);
+      const int nwarps = blockDim.x >> 5;
+      for (int e = warp; e < E; e += nwarps) {      // compact loops: this single-CTA kernel runs from a cold
+        float acc = 0.f;                              // instruction cache, code size is latency
+        if (rf.wdtype == 0) {
+          const float* wr = (const float*)rf.pred_w2 + (size_t)e * rf.ph;
+#pragma unroll 1
+          for (int kk = lane * 4; kk + 4 <= rf.ph; kk += 128) {
+            float wv[4]; WVec<float>::load(wr + kk, wv);
+            const float4 xv = *reinterpret_cast<const float4*>(rf.p1 + kk);
+            acc = fmaf(wv[0], xv.x, acc); acc = fmaf(wv[1], xv.y, acc); acc = fmaf(wv[2], xv.z, acc); acc = fmaf(wv[3], xv.w, acc);
+          }
+        } else {
+          const __nv_bfloat16* wr = (const __nv_bfloat16*)rf.pred_w2 + (size_t)e * rf.ph;
+#pragma unroll 1
+          for (int kk = lane * 8; kk + 8 <= rf.ph; kk += 256) {
+            float wv[8]; WVec<__nv_bfloat16>::load(wr + kk, wv);
+            const float4 x0 = *reinterpret_cast<const float4*>(rf.p1 + kk), x1 = *reinterpret_cast<const float4*>(rf.p1 + kk + 4);
+            acc = fmaf(wv[0], x0.x, acc); acc = fmaf(wv[1], x0.y, acc); acc = fmaf(wv[2], x0.z, acc); acc = fmaf(wv[3], x0.w, acc);
+            acc = fmaf(wv[4], x1.x, acc); acc = fmaf(wv[5], x1.y, acc); acc = fmaf(wv[6], x1.z, acc); acc = fmaf(wv[7], x1.w, acc);
+          }
+        }
+        const float v = warp_sum(acc);
         if (lane == 0) s_p2[e] = v;
       }
     }
     __syncthreads();
     if (warp == 0) {            // A4: top-k by logit (ties → lower index), gates = softmax over the selected
-      float v[8];
-#pragma unroll
-      for (int q = 0; q < 8; ++q) {
-        const int e = lane + 32 * q;
-        v[q] = -INFINITY;
-        if (e < E) { v[q] = rf.zraw[e] + (rf.bias ? rf.bias[e] : 0.f); if (rf.z_out) rf.z_out[e] = v[q]; }
-      }
-      float nxt;
-      warp_topk<8>(v, E, rf.k, lane, f_sel[0], f_val[0], &nxt);
-      __syncwarp();
-      const float zmax = f_val[0][0];
-      const float ex = (lane < rf.k) ? expf(f_val[0][lane] - zmax) : 0.f;
-      const float sum = warp_sum(ex);
-      if (lane < rf.k) { rf.sel[lane] = f_sel[0][lane]; rf.gates[lane] = ex / sum; }
-      if (lane == 0 && rf.margin) rf.margin[0] = (rf.k < E) ? f_val[0][rf.k - 1] - nxt : INFINITY;
+      if (E <= 32) front_route<1>(rf, E, lane, f_sel[0], f_val[0]);
+      else if (E <= 64) front_route<2>(rf, E, lane, f_sel[0], f_val[0]);
+      else if (E <= 128) front_route<4>(rf, E, lane, f_sel[0], f_val[0]);
+      else front_route<8>(rf, E, lane, f_sel[0], f_val[0]);
     } else if (warp == 1 && rf.pred_out) {   // A5: top-k of the predictor scores, listed by descending score
-      float v[8];
-#pragma unroll
-      for (int q = 0; q < 8; ++q) { const int e = lane + 32 * q; v[q] = (e < E) ? s_p2[e] : -INFINITY; }
-      float nxt;
-      warp_topk<8>(v, E, rf.k, lane, f_sel[1], f_val[1], &nxt);
-      __syncwarp();
-      const int np_ = min(rf.k, rf.cap);
-      if (lane == 0) rf.pred_out[0] = np_;
-      if (lane < np_) rf.pred_out[1 + lane] = f_sel[1][lane];
+      if (E <= 32) front_pred<1>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
+      else if (E <= 64) front_pred<2>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
+      else if (E <= 128) front_pred<4>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
+      else front_pred<8>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
     }
     __syncthreads();   // sel / pred_out (global) are read below by this same block
   }
+  __shared__ int32_t s_sel1[kMaxK];
+  if (T == 1) { if (threadIdx.x < k) s_sel1[threadIdx.x] = sel[threadIdx.x]; }
   const int mt_ = m + stride;
   const bool have_t = pred_list != nullptr && mt_ < tbl.Lm;
   for (int i = threadIdx.x; i < C; i += blockDim.x) {
@@ -118,24 +156,38 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   }
   if (have_t) for (int i = threadIdx.x; i <= E; i += blockDim.x) s_pred[i] = pred_list[i];
   if (threadIdx.x == 0) t_clock = *tbl.clock;
-  for (int e = threadIdx.x; e < kMaxE; e += blockDim.x) { needed[e] = 0; prot[e] = 0; }
+  __shared__ uint8_t prot2[kMaxE];       // membership of the predicted list (one push never evicts its own predictions)
+  for (int e = threadIdx.x; e < kMaxE; e += blockDim.x) { needed[e] = 0; prot[e] = 0; prot2[e] = 0; }
   __syncthreads();
-  for (int i = threadIdx.x; i < T * k; i += blockDim.x) needed[sel[i]] = 1;   // same-value writes
+  for (int i = threadIdx.x; i < T * k; i += blockDim.x) { const int e = sel[i]; needed[e] = 1; prot[e] = 1; }   // same-value writes
+  if (have_t) for (int i = threadIdx.x; i < s_pred[0]; i += blockDim.x) prot2[s_pred[1 + i]] = 1;
   __syncthreads();
   if (threadIdx.x == 0) {
 
   SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
   // ---- PushPrecise(m): classes A (cached) → B (being prefetched) → C (not begun), ascending id inside
-  int n = 0, nA = 0, nB = 0;
-  for (int e = 0; e < E; ++e)
-    if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] != 1) { order[n] = e; cls[n++] = 0; }
-  nA = n;
-  for (int e = 0; e < E; ++e)
-    if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] == 1) { order[n] = e; cls[n++] = 1; }
-  nB = n - nA;
-  for (int e = 0; e < E; ++e)
-    if (needed[e] && v.expert_slot[e] < 0) { order[n] = e; cls[n++] = 2; }
-  (void)nB;
+  int n = 0;
+  if (T == 1) {      // decode: only the k selected experts — sort them by id instead of scanning all E
+    int ids[kMaxK];
+    for (int j = 0; j < k; ++j) {
+      int e = s_sel1[j], q = j;
+      while (q > 0 && ids[q - 1] > e) { ids[q] = ids[q - 1]; --q; }
+      ids[q] = e;
+    }
+    for (int c = 0; c < 3; ++c)
+      for (int j = 0; j < k; ++j) {
+        const int e = ids[j], sl = v.expert_slot[e];
+        const int ce = sl < 0 ? 2 : (v.origin[sl] == 1 ? 1 : 0);
+        if (ce == c) { order[n] = e; cls[n++] = (uint8_t)c; }
+      }
+  } else {
+    for (int e = 0; e < E; ++e)
+      if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] != 1) { order[n] = e; cls[n++] = 0; }
+    for (int e = 0; e < E; ++e)
+      if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] == 1) { order[n] = e; cls[n++] = 1; }
+    for (int e = 0; e < E; ++e)
+      if (needed[e] && v.expert_slot[e] < 0) { order[n] = e; cls[n++] = 2; }
+  }
   if (trace_precise) trace_precise[0] = n;
   // touch A then B (Alg. 2 l.15-17)
   for (int i = 0; i < n && cls[i] != 2; ++i) {
@@ -146,8 +198,7 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   }
   // class C: alloc; a needed expert not yet computed in launch order is pinned (G2); all pinned → wait for the
   // next finish in launch order
-  for (int e = 0; e < E; ++e) prot[e] = needed[e];
-  int fin = 0;
+  int fin = 0;                 // prot[] == needed[] was prepared in parallel
   for (int i = 0; i < n; ++i) {
     if (cls[i] != 2) continue;
     const int e = order[i];
@@ -182,7 +233,7 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   *n_problems = n;
   if (row_of && T == 1)
     for (int j = 0; j < k; ++j)
-      for (int i = 0; i < n; ++i) if (order[i] == sel[j]) row_of[j] = i;
+      for (int i = 0; i < n; ++i) if (order[i] == s_sel1[j]) row_of[j] = i;
 
   // ---- PushPredicted(m + stride) (Alg. 2 l.1-10): touch cached, alloc missing as PRED; one push never evicts
   // its own predictions; no victim → skip.
@@ -192,8 +243,7 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
     SlotView t{t_se[1], t_es[1], t_stamp[1], t_gen[1], t_org[1], &t_clock, C, E};
     const int32_t* pred_list = s_pred;
     np = pred_list[0];
-    for (int e = 0; e < E; ++e) prot[e] = 0;
-    for (int i = 0; i < np; ++i) prot[pred_list[1 + i]] = 1;
+    const uint8_t* prot = prot2;
     int allocs = 0;   // at most max_spec experts of one push may allocate (knob G3; most confident first)
     for (int i = 0; i < np; ++i) {
       const int e = pred_list[1 + i];
@@ -232,11 +282,11 @@ __global__ void __launch_bounds__(256) slot_table_kernel(SlotTable tbl, int m, i
   for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
   for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) cmd->pred[i] = prec[i];
   if (threadIdx.x == 0) { cmd->n_needed = s_n; cmd->n_pred = s_np; cmd->pred_target = m + stride; }
-  __threadfence_system();
+  __threadfence_system();      // every writer orders its own stores before the barrier
   __syncthreads();
   if (threadIdx.x == 0) {
-    __threadfence_system();
-    cmd->seq = seq;        // release: the host issuer polls this word
+    volatile uint32_t* sq = &cmd->seq;
+    *sq = seq;                 // release: the host issuer polls this word
   }
 }
 
@@ -248,7 +298,7 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
   (void)reorder;
   RouteFuse f{};
   if (rf) f = *rf;
-  slot_table_kernel<<<1, 256, 0, st>>>(tbl, m, stride, max_spec, sel, T, k, offset, pred_list, slot_base, slot_bytes,
+  slot_table_kernel<<<1, (rf && T == 1) ? 1024 : 256, 0, st>>>(tbl, m, stride, max_spec, sel, T, k, offset, pred_list, slot_base, slot_bytes,
                                        flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of,
                                        cmd, seq, trace_precise, trace_pred, f);
 }

@@ -17,9 +17,6 @@
 #include "engine.h"
 #include "gemm_tc.h"
 
-#include <chrono>
-#include <cstdio>
-#include <cstdlib>
 #include <cstring>
 
 using namespace pmk;

@@ -37,6 +37,7 @@ class ProMoE:
         s = self.s
         self.n_moe = s.n_layers - s.n_dense_layers
         self.slots_per_layer = cache_slots // self.n_moe
+        self.stride = stride
         opts = B.promoe_opts_t(cache_slots=cache_slots, stride=stride, chunk_bytes=chunk_bytes,
                                predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight, high_group=high_group,
                                max_spec_decode=max_spec_decode, max_spec_prefill=max_spec_prefill,

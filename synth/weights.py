@@ -75,7 +75,10 @@ class Weights:
                 img[2 * hi:].view(s.hidden, s.expert_inter))
 
 
-def make_weights(cfg: RunConfig, predictor: str = "skip", pin: Optional[bool] = None) -> Weights:
+def make_weights(cfg: RunConfig, predictor: str = "skip", pin: Optional[bool] = None,
+                 experts_buf: Optional[torch.Tensor] = None, fill_experts: bool = True) -> Weights:
+    """experts_buf: caller-provided [n_moe, E, 3·H·I] host tensor (e.g. a shared-memory mapping used by all ranks of a
+    node); fill_experts=False: the buffer already holds the values (another rank drew them)."""
     s = cfg.shape
     seed = cfg.seed
     dt = torch.float32 if s.wdtype == 0 else torch.bfloat16
@@ -144,9 +147,13 @@ def make_weights(cfg: RunConfig, predictor: str = "skip", pin: Optional[bool] = 
     per = expert_elems(s)
     if pin is None:
         pin = torch.cuda.is_available()
-    experts = torch.empty((n_moe, E, per), dtype=dt, pin_memory=bool(pin))
+    if experts_buf is not None:
+        assert tuple(experts_buf.shape) == (n_moe, E, per) and experts_buf.dtype == dt
+        experts = experts_buf
+    else:
+        experts = torch.empty((n_moe, E, per), dtype=dt, pin_memory=bool(pin))
     hi = H * s.expert_inter
-    for mi, l in enumerate(moe_ids):
+    for mi, l in enumerate(moe_ids if fill_experts else []):
         # gate/up rows have fan-in H, down rows fan-in I; one draw per (layer, matrix) over all experts
         for k, (name, std) in enumerate((("gate", H ** -0.5), ("up", H ** -0.5), ("down", s.expert_inter ** -0.5))):
             _normal(seed, f"l{l}.experts.{name}", (E, hi), std, dt, out=experts[mi, :, k * hi:(k + 1) * hi])

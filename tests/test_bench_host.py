@@ -65,3 +65,19 @@ def test_step_work_matches_paper_byte_count():
     t, bound, terms = bench.roofline_time(1e9, 6.4e9, 1e12, 50.0, 6400.0, 1000.0)
     t2, bound2, _ = step_roofline_seconds(1e9, 6.4e9, 1e12, 50e9, 6400e9, 1000e12)
     assert bound == bound2 == "h2d" and abs(t - t2) < 1e-12 and abs(t - 0.02) < 1e-12
+
+
+def test_shared_expert_buffer_matches_private_copy(tmp_path):
+    """bench.py --gpus N: local rank 0 draws the routed experts into a shared mapping, the other ranks map it."""
+    import synth
+    cfg = synth.get_config("c1b")
+    ref = synth.make_weights(cfg, pin=False)
+    s = cfg.shape
+    n = (s.n_layers - s.n_dense_layers) * s.n_experts * 3 * s.hidden * s.expert_inter
+    path = str(tmp_path / "experts.bin")
+    a = torch.from_file(path, shared=True, size=n, dtype=torch.bfloat16).view_as(ref.experts)
+    wa = synth.make_weights(cfg, pin=False, experts_buf=a, fill_experts=True)
+    b = torch.from_file(path, shared=True, size=n, dtype=torch.bfloat16).view_as(ref.experts)
+    wb = synth.make_weights(cfg, pin=False, experts_buf=b, fill_experts=False)
+    assert torch.equal(wa.experts, ref.experts) and torch.equal(wb.experts, ref.experts)
+    assert all(torch.equal(wb.dense[k], ref.dense[k]) for k in ref.dense)

@@ -145,6 +145,21 @@ def test_mini_configs(name, tensor):
     assert out["report"].max_hidden_ratio <= 1.0
 
 
+@pytest.mark.parametrize("name", ["c2", "c3"])
+def test_full_size_configs(name):
+    """BASELINE.json configs[1], configs[2] at FULL size (all layers, real vocab, 25-30 GB of routed experts in pinned
+    host memory) in the launch configuration bench.py times (tcgen05 prefill, fused decode, default chunking): a
+    48-token prompt + 3 decode steps is what the oracle finishes in about a minute; every selection, permutation
+    and cache record of those steps is compared, hidden state and logits within tolerance."""
+    from paper_2410_22134_b200 import binding as B
+    cfg = synth.get_config(name)
+    w = synth.make_weights(cfg, predictor="skip")
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR
+    out = run_parity(cfg, w, synth.make_prompt(cfg, 48), 3, flags=flags, chunk_bytes=4 << 20, max_spec_decode=1)
+    _report(name + "-full", out)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+
+
 def test_outputs_independent_of_cache_parameters():
     """P:439 'equivalent to the original model' + P:277: logits BITWISE identical across cache budget, stride, chunk
     size, predictor mode, warm/cold start and preemption (fixed-order combine, no atomics)."""
