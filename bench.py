@@ -293,12 +293,14 @@ def run_ours(args, cfg, rank, world, dist):
     torch.cuda.synchronize()
     clocks = ClockSampler(local)
     clocks.start()
+    launches0 = eng.stats()["kernel_launches"]
     t0 = time.perf_counter()
     reqs = [run_request(eng, cfg, prompt, decode_ids, greedy, inject=inject) for _ in range(args.steps)]
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
     wall = time.perf_counter() - t0
+    launches = eng.stats()["kernel_launches"] - launches0
     clk = clocks.stop()
 
     K = args.steps
@@ -377,6 +379,34 @@ def run_ours(args, cfg, rank, world, dist):
         exposed = max(0.0, dec_s / K - comp_dec_s)
         hidden = max(0.0, 1.0 - exposed / copy_s) if copy_s > 0 else None
 
+    # ---- context points (one request each, not the headline): reactive LRU cache without prefetch (BASELINE.json
+    # configs[4] "no-prefetch reactive baseline") and the oracle-routing predictor (its upper bound)
+    variants = None
+    if rank == 0 and args.variants:
+        variants = {}
+        for name, pm in (("reactive_no_prefetch", B.PRED_NONE), ("oracle_routing_predictor", B.PRED_TRACE)):
+            inj = None
+            if pm == B.PRED_TRACE:
+                rec = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, predictor_mode=B.PRED_NONE,
+                             flags=flags | B.F_TRACE, device=f"cuda:{local}")
+                inj = []
+                run_request(rec, cfg, prompt, decode_ids, greedy, record=inj)
+                rec.close()
+            v = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_mb << 20,
+                       predictor_mode=pm, flags=flags, max_inflight=args.inflight, device=f"cuda:{local}")
+            run_request(v, cfg, prompt, decode_ids, greedy, inject=inj)
+            r = run_request(v, cfg, prompt, decode_ids, greedy, inject=inj)
+            v.close()
+            need_d, need_p = r["dec"]["need_experts"] * Be, r["pre"]["need_experts"] * Be
+            variants[name] = {
+                "decode_tokens_per_s": cfg.decode_steps / (r["decode_ms"] / 1e3),
+                "prefill_tokens_per_s": cfg.prompt_len / (r["prefill_ms"] / 1e3),
+                "decode_roofline_frac": need_d / (h2d_gbs * 1e9) / (r["decode_ms"] / 1e3),
+                "prefill_roofline_frac": need_p / (h2d_gbs * 1e9) / (r["prefill_ms"] / 1e3),
+                "hit_rate": (r["dec"]["hits_resident"] + r["dec"]["hits_prefetch"]) / max(1, r["dec"]["accesses"]),
+                "h2d_bytes_needed_per_token": need_d / cfg.decode_steps,
+                "h2d_bytes_moved_per_token": r["dec"]["h2d_bytes"] / cfg.decode_steps}
+
     cpu = None
     if rank == 0 and not args.no_cpu:
         o = oracle_sample(cfg, weights, args.ref_prompt, args.ref_decode)
@@ -385,10 +415,6 @@ def run_ours(args, cfg, rank, world, dist):
                "sample": f"prefill {args.ref_prompt} + {args.ref_decode} decode tokens of {cfg.name} (of {cfg.prompt_len} + {cfg.decode_steps})"}
     if rank != 0:
         return
-    # kernels launched inside the timed region: decode step = embed + per layer (2 rmsnorm, qkv, rope, attn×2, wo, ...)
-    n_moe = s.n_layers - s.n_dense_layers
-    per_layer_dec = 7 + 2 + (3 if args.predictor != "none" else 0) + 1 + (2 if s.n_shared_inter else 0) + (1 if s.shared_gate else 0) + 3
-    launches = K * (cfg.decode_steps * (1 + n_moe * per_layer_dec + s.n_dense_layers * 10 + 2))
     line = {"metric": METRIC, "value": g_dec_tok / g_dec_s, "unit": "tokens/s", "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": 1e3 * wall / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32 activations x bf16 weights, f32 accumulate" if s.wdtype else "f32",
@@ -403,7 +429,7 @@ def run_ours(args, cfg, rank, world, dist):
             "step_roofline": {"h2d_gbs_measured": h2d_gbs, "hbm_gbs": peaks["hbm_gbs"], "bf16_tflops": peaks["bf16_tflops_sustained"],
                               "peaks": peaks["source"], "decode": roof_dec, "prefill": roof_pre},
             "cache": {"decode": cs_dec, "prefill": cs_pre, "hidden_copy_fraction_decode": hidden},
-            "all_resident": allhit, "cpu_baseline": cpu}
+            "all_resident": allhit, "variants": variants, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
 
 
@@ -420,7 +446,7 @@ def main():
                     help="decode ids: seeded random (locality-neutral, default) or greedy argmax")
     ap.add_argument("--chunk-mb", type=int, default=4)
     ap.add_argument("--inflight", type=int, default=0)
-    ap.add_argument("--max-spec-decode", type=int, default=0, help="allocations per PushPredicted in decode (0 = top_k, <0 = none)")
+    ap.add_argument("--max-spec-decode", type=int, default=1, help="allocations per PushPredicted in decode (0 = top_k as in Alg. 2, <0 = none); default 1: on a B200 one layer of\n                    compute hides about half an expert copy (profiles/r01_sweep_c2.md)")
     ap.add_argument("--max-spec-prefill", type=int, default=0, help="allocations per PushPredicted in prefill (<=0 = none)")
     ap.add_argument("--tensor", type=int, default=1, help="prefill GEMMs on tcgen05 (bf16 weights)")
     ap.add_argument("--prompt-len", type=int, default=0)
@@ -429,6 +455,7 @@ def main():
     ap.add_argument("--ref-decode", type=int, default=3, help="oracle sample: decode tokens")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-allhit", action="store_true")
+    ap.add_argument("--variants", type=int, default=1, help="also measure the reactive and oracle-routing context points")
     args = ap.parse_args()
 
     import synth

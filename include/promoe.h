@@ -115,6 +115,7 @@ typedef struct {
   uint64_t h2d_bytes;           /* bytes physically copied */
   uint64_t fetched_at_gate, fetched_at_gate_of;  /* FetchRate numerator / denominator */
   uint64_t registered_host_bytes; /* expert host bytes the library had to cudaHostRegister */
+  uint64_t kernel_launches;     /* kernels launched by the library in this process so far (all handles) */
   double copy_busy_ms;          /* copy-stream busy time, from per-chunk events */
   double step_ms;               /* sum of step times (compute-stream events) */
   double last_step_ms;

@@ -53,7 +53,8 @@ class promoe_stats_t(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in (
         "steps", "tokens", "accesses", "hits_resident", "hits_prefetch", "misses", "evictions", "predicted",
         "predicted_correct", "pred_allocs", "need_experts", "chunks_issued", "chunks_cancelled", "chunks_high",
-        "chunks_low", "h2d_bytes", "fetched_at_gate", "fetched_at_gate_of", "registered_host_bytes")] + [
+        "chunks_low", "h2d_bytes", "fetched_at_gate", "fetched_at_gate_of", "registered_host_bytes",
+        "kernel_launches")] + [
         ("copy_busy_ms", C.c_double), ("step_ms", C.c_double), ("last_step_ms", C.c_double),
         ("timeouts", C.c_int32), ("reserved", C.c_int32)]
 

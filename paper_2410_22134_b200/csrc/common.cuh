@@ -8,6 +8,9 @@ namespace pmk {
 
 constexpr int kWarp = 32;
 
+// number of kernels launched by this library (host-side counter, bumped by every launch_* wrapper; promoe_stats)
+extern unsigned long long g_launches;
+
 // ---- 16-byte vectorised weight loads, widened exactly to fp32 (weights are bf16 or fp32; G1) -------------
 template <typename WT> struct WVec;
 template <> struct WVec<float> {

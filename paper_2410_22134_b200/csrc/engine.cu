@@ -13,6 +13,7 @@
 using namespace pmk;
 
 static std::string g_create_err;
+namespace pmk { unsigned long long g_launches = 0; }
 
 #define CK(call)                                                                                   \
   do {                                                                                             \
@@ -309,6 +310,7 @@ extern "C" int promoe_get_slots(promoe_t* h, int32_t m, int32_t* out) {
 extern "C" int promoe_stats(promoe_t* h, promoe_stats_t* out) {
   if (!h || !out) return PROMOE_EINVAL;
   *out = h->st;
+  out->kernel_launches = pmk::g_launches;
   return PROMOE_OK;
 }
 

@@ -251,6 +251,7 @@ __global__ void __launch_bounds__(256) split_rows_kernel(const float* __restrict
 }
 void launch_split_rows(const float* x, const int32_t* row_src, int src_div, int rows, int K, __nv_bfloat16* hi,
                        size_t lo_off, cudaStream_t st) {
+  ++g_launches;
   if (rows > 0) split_rows_kernel<<<rows, 256, 0, st>>>(x, row_src, src_div, K, hi, lo_off);
 }
 
@@ -308,6 +309,7 @@ static const CUtensorMap* get_map(TcContext* c, const void* base, int K, int row
 }
 
 bool tc_launch(TcContext* c, const TcGemm& g, cudaStream_t st, std::string* err) {
+  ++g_launches;
   if (!c || !g.a0 || !g.b_hi || g.K < 8 || g.N < 1 || (g.K % 8)) { if (err) *err = "tc_launch: unsupported arguments"; return false; }
   const size_t stage = (g.swiglu ? 2 : 1) * (size_t)TC_A_BYTES + 2 * (size_t)TC_B_BYTES;
   const size_t smem = TC_STAGES * stage + 256 + 1024;

@@ -29,6 +29,7 @@ __global__ void rope_append_kernel(float* __restrict__ qkv, const float* __restr
 }
 void launch_rope_append(float* qkv, const float* cos_t, const float* sin_t, float* kcache, float* vcache, int T,
                         int pos0, int nq, int nkv, int d, int max_seq, cudaStream_t st) {
+  ++g_launches;
   rope_append_kernel<<<dim3(T, nq + nkv), d / 2, 0, st>>>(qkv, cos_t, sin_t, kcache, vcache, pos0, nq, nkv, d,
                                                          max_seq);
 }
@@ -129,9 +130,11 @@ __global__ void attn_decode_merge_kernel(const float* __restrict__ ws, float* __
 }
 void launch_attn_decode(const float* qkv, const float* kcache, const float* vcache, float* out, float* ws,
                         int n_pos, int nq, int nkv, int d, int max_seq, int nsplit, cudaStream_t st) {
+  ++g_launches;
   dim3 grid(nq, nsplit);
   if (d == 128) attn_decode_kernel<128><<<grid, 128, 0, st>>>(qkv, kcache, vcache, ws, n_pos, nq, nkv, max_seq, nsplit);
   else attn_decode_kernel<64><<<grid, 128, 0, st>>>(qkv, kcache, vcache, ws, n_pos, nq, nkv, max_seq, nsplit);
+  ++g_launches;   // second kernel of this wrapper
   attn_decode_merge_kernel<<<nq, 128, 0, st>>>(ws, out, d, nsplit);
 }
 
@@ -250,6 +253,7 @@ __global__ void __launch_bounds__(256) attn_prefill_kernel(const float* __restri
 }
 void launch_attn_prefill(const float* qkv, const float* kcache, const float* vcache, float* out, int T, int pos0,
                          int nq, int nkv, int d, int max_seq, cudaStream_t st) {
+  ++g_launches;
   dim3 grid((T + 63) / 64, nq);
   const size_t smem = (size_t)(2 * d * 68 + 64 * d + 64 * 68) * sizeof(float);
   if (d == 128) {

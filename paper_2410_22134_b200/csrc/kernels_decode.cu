@@ -88,6 +88,7 @@ __global__ void __launch_bounds__(256) norm_multi_gemv_kernel(NormGemvArgs a) {
   }
 }
 void launch_norm_multi_gemv(const NormGemvArgs& a_in, int wdtype, cudaStream_t st) {
+  ++g_launches;
   NormGemvArgs a = a_in;
   a.n_rows_total = a.n_sw;
   for (int s = 0; s < a.nseg; ++s) a.n_rows_total += a.seg[s].n;
@@ -230,6 +231,7 @@ __global__ void __launch_bounds__(128) attn_decode_fused_kernel(const float* __r
 void launch_attn_decode_fused(const float* qkv, const float* cos_t, const float* sin_t, float* kcache, float* vcache,
                               float* ws, float* out, int* counters, int pos, int nq, int nkv, int d, int max_seq,
                               int nsplit, cudaStream_t st) {
+  ++g_launches;
   dim3 grid(nq, nsplit);
   if (d == 128) attn_decode_fused_kernel<128><<<grid, 128, 0, st>>>(qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);
   else attn_decode_fused_kernel<64><<<grid, 128, 0, st>>>(qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);
@@ -321,6 +323,7 @@ void launch_ffn_down_combine(const float* act, int act_stride, const FfnProblem*
                              const float* gates, int k, const FfnProblem* shared, const float* sact,
                              const float* sgate_logit, int H, float* x, int wdtype, size_t chunk_bytes, int* err,
                              cudaStream_t st) {
+  ++g_launches;
   const int blocks = (H + DC_ROWS - 1) / DC_ROWS;
   if (wdtype == 0) ffn_down_combine_kernel<float><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, H, x, chunk_bytes, err);
   else ffn_down_combine_kernel<__nv_bfloat16><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, H, x, chunk_bytes, err);

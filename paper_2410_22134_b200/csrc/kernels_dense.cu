@@ -14,6 +14,7 @@ __global__ void embed_kernel(const int32_t* __restrict__ ids, const WT* __restri
   for (int i = threadIdx.x; i < H; i += blockDim.x) x[(size_t)t * H + i] = wload1(row + i);
 }
 void launch_embed(const int32_t* ids, const void* emb, float* x, int T, int H, int wdtype, cudaStream_t st) {
+  ++g_launches;
   if (wdtype == 0) embed_kernel<float><<<T, 256, 0, st>>>(ids, (const float*)emb, x, H);
   else embed_kernel<__nv_bfloat16><<<T, 256, 0, st>>>(ids, (const __nv_bfloat16*)emb, x, H);
 }
@@ -37,6 +38,7 @@ __global__ void __launch_bounds__(256) rmsnorm_kernel(const float* __restrict__ 
   for (int i = threadIdx.x; i < H; i += 256) y[(size_t)t * H + i] = xr[i] * r * w[i];
 }
 void launch_rmsnorm(const float* x, const float* w, float* y, int T, int H, float eps, cudaStream_t st) {
+  ++g_launches;
   rmsnorm_kernel<<<T, 256, 0, st>>>(x, w, y, H, eps);
 }
 
@@ -60,6 +62,7 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ x, 
   }
 }
 void launch_gemv(const float* x, const void* w, float* y, int N, int K, int wdtype, int flags, cudaStream_t st) {
+  ++g_launches;
   int blocks = (N + 7) / 8;
   if (blocks > 148 * 8) blocks = 148 * 8;   // 8 CTAs x 8 warps resident per SM; grid-stride over rows
   if (wdtype == 0) gemv_kernel<float><<<blocks, 256, 0, st>>>(x, (const float*)w, y, N, K, flags);
@@ -127,6 +130,7 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(const float* __restrict_
 }
 void launch_gemm_simt(const float* x, const void* w, float* y, int T, int N, int K, int wdtype, int flags,
                       cudaStream_t st) {
+  ++g_launches;
   dim3 grid((N + GB - 1) / GB, (T + GB - 1) / GB);
   if (wdtype == 0) gemm_simt_kernel<float><<<grid, 256, 0, st>>>(x, (const float*)w, y, T, N, K, flags);
   else gemm_simt_kernel<__nv_bfloat16><<<grid, 256, 0, st>>>(x, (const __nv_bfloat16*)w, y, T, N, K, flags);
@@ -138,6 +142,7 @@ __global__ void add_kernel(const float* __restrict__ a, const float* __restrict_
   if (i < n) out[i] = a[i] + b[i];
 }
 void launch_add(const float* a, const float* b, float* out, size_t n, cudaStream_t st) {
+  ++g_launches;
   add_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, b, out, n);
 }
 

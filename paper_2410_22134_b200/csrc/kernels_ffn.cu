@@ -158,6 +158,7 @@ __global__ void __launch_bounds__(256) ffn_gemm_simt_kernel(const float* __restr
 
 void launch_ffn_gateup_gemv(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
                             int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st) {
+  ++g_launches;
   const int tiles = (max_inter + 7) / 8;
   WDISPATCH((ffn_gateup_gemv_kernel<float><<<n_probs * tiles, 256, 0, st>>>(u, probs, nullptr, tiles, H, act,
                                                                             act_stride, chunk_bytes, err)),
@@ -166,6 +167,7 @@ void launch_ffn_gateup_gemv(const float* u, const FfnProblem* probs, int n_probs
 }
 void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int max_inter,
                           int H, float* y, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st) {
+  ++g_launches;
   (void)max_inter;
   const int tiles = (H + 7) / 8;
   WDISPATCH((ffn_down_gemv_kernel<float><<<n_probs * tiles, 256, 0, st>>>(act, act_stride, probs, nullptr, tiles, H,
@@ -176,6 +178,7 @@ void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* pr
 void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src_div, const FfnProblem* probs,
                                  int p0, int np, int max_rows, int rows_override, int max_inter, int H, float* act,
                                  int act_stride, int wdtype, cudaStream_t st) {
+  ++g_launches;
   dim3 grid((max_inter + FB - 1) / FB, (max_rows + FB - 1) / FB, np);
   WDISPATCH((ffn_gemm_simt_kernel<float, true><<<grid, 256, 0, st>>>(x, H, row_src, src_div, probs, p0, H, act,
                                                                      act_stride, rows_override)),
@@ -185,6 +188,7 @@ void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src
 void launch_ffn_down_gemm_simt(const float* act, int act_stride, const FfnProblem* probs, int p0, int np,
                                int max_rows, int rows_override, int max_inter, int H, float* y, int wdtype,
                                cudaStream_t st) {
+  ++g_launches;
   (void)max_inter;
   dim3 grid((H + FB - 1) / FB, (max_rows + FB - 1) / FB, np);
   WDISPATCH((ffn_gemm_simt_kernel<float, false><<<grid, 256, 0, st>>>(act, act_stride, nullptr, 1, probs, p0, H, y,

@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(128) topk_gate_kernel(const float* __restrict_
 }
 void launch_topk_gate(const float* z, const float* bias, int T, int E, int k, float* z_out, int32_t* sel,
                       float* gates, float* margin, cudaStream_t st) {
+  ++g_launches;
   const int blocks = (T + 3) / 4;
   if (E <= 32) topk_gate_kernel<1><<<blocks, 128, 0, st>>>(z, bias, T, E, k, z_out, sel, gates, margin);
   else if (E <= 64) topk_gate_kernel<2><<<blocks, 128, 0, st>>>(z, bias, T, E, k, z_out, sel, gates, margin);
@@ -93,6 +94,7 @@ __global__ void __launch_bounds__(256) pred_list_kernel(const float* __restrict_
   if (threadIdx.x == 0) pred[0] = min(nvoted, cap);
 }
 void launch_pred_list(const float* p, int T, int E, int k, int cap, int32_t* pred, cudaStream_t st) {
+  ++g_launches;
   if (E <= 32) pred_list_kernel<1><<<1, 256, 0, st>>>(p, T, E, k, cap, pred);
   else if (E <= 64) pred_list_kernel<2><<<1, 256, 0, st>>>(p, T, E, k, cap, pred);
   else if (E <= 128) pred_list_kernel<4><<<1, 256, 0, st>>>(p, T, E, k, cap, pred);
@@ -193,6 +195,7 @@ __global__ void __launch_bounds__(PT) permute_kernel(const int32_t* __restrict__
 }
 void launch_permute(const int32_t* sel, int T, int k, int E, int32_t* count, int32_t* offset, int32_t* perm,
                     int32_t* inv, cudaStream_t st) {
+  ++g_launches;
   permute_kernel<<<1, PT, 0, st>>>(sel, T * k, E, count, offset, perm, inv);
 }
 
@@ -216,6 +219,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const float* __restrict__ 
 }
 void launch_combine(const float* hres, const float* yexp, const int32_t* row_of, const float* gates, int T, int k,
                     int H, const float* shared, const float* sgate_logit, float* out, cudaStream_t st) {
+  ++g_launches;
   combine_kernel<<<T, 256, 0, st>>>(hres, yexp, row_of, gates, k, H, shared, sgate_logit, out);
 }
 

@@ -295,6 +295,7 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
                        int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf) {
+  ++g_launches;
   (void)reorder;
   RouteFuse f{};
   if (rf) f = *rf;

@@ -25,4 +25,4 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(B.promoe_shape_t) == 17 * 4 + 2 * 4
     assert ctypes.sizeof(B.promoe_opts_t) == 48
     assert ctypes.sizeof(B.promoe_dense_t) == 15 * 8
-    assert ctypes.sizeof(B.promoe_stats_t) == 19 * 8 + 3 * 8 + 8
+    assert ctypes.sizeof(B.promoe_stats_t) == 20 * 8 + 3 * 8 + 8
