@@ -106,8 +106,8 @@ void launch_attn_decode_fused(const float* qkv, const float* cos_t, const float*
                               int nsplit, cudaStream_t st);
 void launch_ffn_down_combine(const float* act, int act_stride, const FfnProblem* probs, const int32_t* row_of,
                              const float* gates, int k, const FfnProblem* shared, const float* sact,
-                             const float* sgate_logit, int H, float* x, int wdtype, size_t chunk_bytes, int* err,
-                             cudaStream_t st);
+                             const float* sgate_logit, const float* shared_y, int H, float* x, int wdtype,
+                             size_t chunk_bytes, int* err, cudaStream_t st);
 // fused front end of the slot-table kernel for T == 1: top-k + gates on (zraw + bias), predictor W2 GEMV + list
 struct RouteFuse {
   const float* zraw; const float* bias; float* z_out; int32_t* sel; float* gates; float* margin;

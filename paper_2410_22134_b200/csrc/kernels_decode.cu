@@ -250,7 +250,8 @@ __global__ void __launch_bounds__(256) ffn_down_combine_kernel(const float* __re
                                                                const float* __restrict__ gates, int k,
                                                                const FfnProblem* __restrict__ shared,
                                                                const float* __restrict__ sact,
-                                                               const float* __restrict__ sgate_logit, int H,
+                                                               const float* __restrict__ sgate_logit,
+                                                               const float* __restrict__ shared_y, int H,
                                                                float* __restrict__ x, size_t chunk_bytes, int* err) {
   __shared__ const void* it_w[DC_MAX_ITEMS];     // weight matrix base of the item
   __shared__ const float* it_x[DC_MAX_ITEMS];    // activation vector of the item
@@ -310,9 +311,10 @@ __global__ void __launch_bounds__(256) ffn_down_combine_kernel(const float* __re
       for (; it < ni && it_j[it] == j; ++it) d += part[rr][it];
       y = fmaf(gates[j], d, y);
     }
-    if (shared) {
+    if (shared || shared_y) {     // shared expert: down rows computed here, or precomputed (shared_y) under the copies
       float d = 0.f;
-      for (; it < ni; ++it) d += part[rr][it];
+      if (shared) { for (; it < ni; ++it) d += part[rr][it]; }
+      else d = shared_y[r0 + rr];
       const float sg = sgate_logit ? 1.f / (1.f + expf(-sgate_logit[0])) : 1.f;
       y += sg * d;
     }
@@ -321,12 +323,12 @@ __global__ void __launch_bounds__(256) ffn_down_combine_kernel(const float* __re
 }
 void launch_ffn_down_combine(const float* act, int act_stride, const FfnProblem* probs, const int32_t* row_of,
                              const float* gates, int k, const FfnProblem* shared, const float* sact,
-                             const float* sgate_logit, int H, float* x, int wdtype, size_t chunk_bytes, int* err,
-                             cudaStream_t st) {
+                             const float* sgate_logit, const float* shared_y, int H, float* x, int wdtype,
+                             size_t chunk_bytes, int* err, cudaStream_t st) {
   ++g_launches;
   const int blocks = (H + DC_ROWS - 1) / DC_ROWS;
-  if (wdtype == 0) ffn_down_combine_kernel<float><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, H, x, chunk_bytes, err);
-  else ffn_down_combine_kernel<__nv_bfloat16><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, H, x, chunk_bytes, err);
+  if (wdtype == 0) ffn_down_combine_kernel<float><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
+  else ffn_down_combine_kernel<__nv_bfloat16><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
 }
 
 }  // namespace pmk

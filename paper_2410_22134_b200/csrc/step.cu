@@ -124,7 +124,7 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   if (l < s.n_dense_layers) {
     b.wg = h->ffn_gate[l]; b.wu = h->ffn_up[l]; b.act = h->sact; b.n_sw = s.dense_inter;
     launch_norm_multi_gemv(b, wd, cs);
-    launch_ffn_down_combine(nullptr, 0, nullptr, nullptr, nullptr, 0, h->shared_prob + l, h->sact, nullptr, H, h->x, wd,
+    launch_ffn_down_combine(nullptr, 0, nullptr, nullptr, nullptr, 0, h->shared_prob + l, h->sact, nullptr, nullptr, H, h->x, wd,
                             h->chunk_bytes, h->err_dev, cs);
     return PROMOE_OK;
   }
@@ -151,14 +151,16 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   // looks at the command: it covers the device→host→device hand-over.  The flag-gated kernels K6/K7 must NOT be
   // enqueued before the copies they wait for: when the driver multiplexes both streams onto one hardware queue a
   // resident spinning kernel starves the copy (seen on B200: 4 s flag time-outs), so copies always go first.
-  if (s.n_shared_inter)
+  if (s.n_shared_inter) {   // the whole shared expert runs under the hand-over / the copies; K7 only adds σ(gate)·sy
     launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, cs);
+    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, cs);
+  }
   RC(ce_wait_cmd(h, m, seq));                                                            // A7
   RC(ce_process_cmd(h, m, nullptr));
   launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
-  launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, s.n_shared_inter ? h->shared_prob + l : nullptr,   // K7
-                          h->sact, (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, H, h->x, wd, h->chunk_bytes,
-                          h->err_dev, cs);
+  launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,                 // K7
+                          (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, s.n_shared_inter ? h->sy : nullptr, H, h->x,
+                          wd, h->chunk_bytes, h->err_dev, cs);
   return PROMOE_OK;
 }
 
