@@ -444,8 +444,8 @@ def main():
                     help="skip: training-free MLP weights (default); none: reactive cache; trace: oracle-routing upper bound")
     ap.add_argument("--decode", default="random", choices=["random", "greedy"],
                     help="decode ids: seeded random (locality-neutral, default) or greedy argmax")
-    ap.add_argument("--chunk-mb", type=int, default=4)
-    ap.add_argument("--inflight", type=int, default=0)
+    ap.add_argument("--chunk-mb", type=int, default=8, help="LOW (predicted) fills are issued in chunks of this size")
+    ap.add_argument("--inflight", type=int, default=1, help="LOW chunks kept in flight (bounded preemption delay, P:191)")
     ap.add_argument("--max-spec-decode", type=int, default=1, help="allocations per PushPredicted in decode (0 = top_k as in Alg. 2, <0 = none); default 1: on a B200 one layer of\n                    compute hides about half an expert copy (profiles/r01_sweep_c2.md)")
     ap.add_argument("--max-spec-prefill", type=int, default=0, help="allocations per PushPredicted in prefill (<=0 = none)")
     ap.add_argument("--tensor", type=int, default=1, help="prefill GEMMs on tcgen05 (bf16 weights)")

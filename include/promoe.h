@@ -196,7 +196,8 @@ PROMOE_API int promoe_op_permute(const int32_t* sel, int32_t T, int32_t k, int32
 
 /* expert FFN row A9 on one resident weight set: y[T,H] = Wd.(silu(Wg.x) * (Wu.x)); x [T,H], act_ws [T,I] scratch,
  * prob_ws >= 64 bytes of device scratch (problem record).  path: 0 auto, 1 HBM-streaming GEMV (T == 1),
- * 2 SIMT grouped GEMM, 3 tcgen05 grouped GEMM (bf16 weights). */
+ * 2 SIMT grouped GEMM, 3 tcgen05 grouped GEMM (bf16 weights), 4 TMA-fed (cp.async.bulk) gate/up GEMV (T == 1, bf16,
+ * H <= 2048). */
 PROMOE_API int promoe_op_expert_ffn(const float* x, const void* wg, const void* wu, const void* wd, float* act_ws,
                                     float* y, void* prob_ws, int32_t T, int32_t H, int32_t I, int32_t wdtype,
                                     int32_t path, int32_t reserved, void* stream);

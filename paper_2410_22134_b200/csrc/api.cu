@@ -155,8 +155,11 @@ extern "C" int promoe_op_expert_ffn(const float* x, const void* wg, const void* 
   if (cudaMemcpyAsync(prob_ws, &pb, sizeof(pb), cudaMemcpyHostToDevice, st) != cudaSuccess) return PROMOE_ECUDA;
   const FfnProblem* dp = (const FfnProblem*)prob_ws;
   if (path == 0) path = (T == 1) ? 1 : 2;
-  if (path == 1) {
+  if (path == 1 || path == 4) {     // 4 = TMA-fed gate/up GEMV (bf16, H <= 2048), else register-fed
     if (T != 1) return PROMOE_EINVAL;
+    if (path == 4) {
+      if (wdtype != 1 || !launch_ffn_gateup_gemv_tma(x, dp, 1, I, H, act_ws, I, (size_t)1 << 20, nullptr, st)) return PROMOE_EINVAL;
+    } else
     launch_ffn_gateup_gemv(x, dp, 1, I, H, act_ws, I, wdtype, (size_t)1 << 20, nullptr, st);
     launch_ffn_down_gemv(act_ws, I, dp, 1, I, H, y, wdtype, (size_t)1 << 20, nullptr, st);
   } else if (path == 2) {

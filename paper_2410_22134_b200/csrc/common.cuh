@@ -49,11 +49,12 @@ __device__ __forceinline__ float silu(float a) { return a / (1.0f + expf(-a)); }
 // ---- one weight row · x, fp32 accumulate: the HBM-streaming inner loop of every decode GEMV -------------------
 // K must be a multiple of the 16-byte vector width; the summation order depends on (K, lane) only, so results
 // are bit-identical wherever the row lives (slot, shared expert, any launch order).
-template <typename WT>
+template <typename WT, int UNR = 4>
 __device__ __forceinline__ float row_dot(const WT* __restrict__ wrow, const float* __restrict__ x, int K, int lane) {
   constexpr int V = WVec<WT>::N;
-  constexpr int UNR = 4;
-  float acc[UNR] = {0.f, 0.f, 0.f, 0.f};
+  float acc[UNR];
+#pragma unroll
+  for (int u = 0; u < UNR; ++u) acc[u] = 0.f;
   int k = lane * V;
   const int step = 32 * V;
   for (; k + (UNR - 1) * step + V <= K; k += UNR * step) {
@@ -79,7 +80,13 @@ __device__ __forceinline__ float row_dot(const WT* __restrict__ wrow, const floa
 #pragma unroll
     for (int q = 0; q < V; ++q) acc[0] = fmaf(wv[q], __ldg(x + k + q), acc[0]);
   }
-  return warp_sum((acc[0] + acc[1]) + (acc[2] + acc[3]));
+  float tot = 0.f;
+  if (UNR == 4) tot = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+  else {
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) tot += acc[u];
+  }
+  return warp_sum(tot);
 }
 
 

@@ -81,6 +81,9 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
 // chunk geometry: image = [gate | up | down], chunk c covers bytes [c*chunk_bytes, (c+1)*chunk_bytes).
 void launch_ffn_gateup_gemv(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
                             int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st);
+// TMA-fed variant (bf16 weights, H <= 2048, H % 256 == 0); false = shape unsupported, nothing launched
+bool launch_ffn_gateup_gemv_tma(const float* u, const FfnProblem* probs, int n_probs, int inter, int H, float* act,
+                                int act_stride, size_t chunk_bytes, int* err, cudaStream_t st);
 void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int max_inter,
                           int H, float* y, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st);
 // A9 prefill grouped SwiGLU FFN, SIMT fp32: problems [p0, p0+np) each with its row range; x rows are gathered

@@ -202,3 +202,21 @@ def test_op_expert_ffn_tcgen05(B, T, H, I):
     ref = swiglu_ffn(x.double(), wg, wu, wdn)
     err = (y.cpu().double() - ref).abs().max().item()
     assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
+
+
+@pytest.mark.parametrize("H,I", [(256, 512), (2048, 1408), (1024, 264 * 8)])
+def test_op_expert_ffn_tma_gemv(B, H, I):
+    """Decode gate/up GEMV fed by cp.async.bulk through a shared-memory ring (path 4)."""
+    from oracle.forward import swiglu_ffn
+    x = _w((1, H), torch.float32, 7, 1.0)
+    wg, wu, wdn = _w((I, H), torch.bfloat16, 8), _w((I, H), torch.bfloat16, 9), _w((H, I), torch.bfloat16, 10)
+    xd, wgd, wud, wdd = x.cuda(), wg.cuda(), wu.cuda(), wdn.cuda()
+    act = torch.empty((1, I), device="cuda"); y = torch.full((1, H), float("nan"), device="cuda")
+    ws = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    rc = B.lib().promoe_op_expert_ffn(xd.data_ptr(), wgd.data_ptr(), wud.data_ptr(), wdd.data_ptr(), act.data_ptr(),
+                                      y.data_ptr(), ws.data_ptr(), 1, H, I, 1, 4, 0, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    ref = swiglu_ffn(x.double(), wg, wu, wdn)
+    err = (y.cpu().double() - ref).abs().max().item()
+    assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
