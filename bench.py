@@ -433,6 +433,86 @@ def run_ours(args, cfg, rank, world, dist):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: sweep on the DeepSeek-MoE-16B-shaped decoder — expert-cache budget 25/50/75 % x
+    predictor stride 1/2/3 x H2D chunk 1/4/16 MiB, plus the oracle-routing predictor and the reactive cache per
+    budget; prompts 128 / 2048, 256 decode steps.  One JSON line per point (tokens/s, hit rate, hidden-copy
+    fraction, % of the per-step roofline)."""
+    import dataclasses
+    import torch
+    import synth
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+    torch.cuda.set_device(0)
+    peaks = load_peaks()
+    base = synth.get_config("c3", shape_overrides={"max_seq": 2048 + 256}, decode_steps=args.decode_steps or 256)
+    s = base.shape
+    n_moe = s.n_layers - s.n_dense_layers
+    Be = 3 * s.hidden * s.expert_inter * 2
+    h2d = B.promoe_measure_h2d(256 << 20, 2, 5)
+    w0 = synth.make_weights(base, predictor="skip")
+    decode_ids = synth.make_decode_ids(base).tolist()
+    prompts = {n: synth.make_prompt(base, n).tolist() for n in (128, 2048)}
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TENSOR
+    wcache = {1: w0}
+
+    def weights_for(stride):
+        if stride not in wcache:      # the skip predictor's weights depend on the stride; the experts are shared
+            wcache[stride] = synth.make_weights(dataclasses.replace(base, stride=stride), predictor="skip",
+                                                experts_buf=w0.experts, fill_experts=False)
+        return wcache[stride]
+
+    def one(cfg, eng, prompt, inject=None):
+        run_request(eng, dataclasses.replace(cfg, decode_steps=4), prompt[:64], decode_ids, False)       # warm-up
+        return run_request(eng, cfg, prompt, decode_ids, False, inject=inject)
+
+    compute = {}
+    full = ProMoE(w0, cache_slots=n_moe * s.n_experts, stride=1, predictor_mode=B.PRED_MLP, flags=flags)
+    for n, pr in prompts.items():
+        r = one(dataclasses.replace(base, prompt_len=n), full, pr)
+        compute[n] = (r["prefill_ms"], r["decode_ms"])
+    full.close()
+    routing = {}
+    points = []
+    for frac in (0.25, 0.5, 0.75):
+        slots = int(s.n_experts * frac) * n_moe
+        grid = [("mlp", st, ch) for st in (1, 2, 3) for ch in (1, 4, 16)] + [("trace", 1, 4), ("none", 1, 4)]
+        for mode, stride, chunk in grid:
+            w = weights_for(stride if mode == "mlp" else 1)
+            pm = {"mlp": B.PRED_MLP, "trace": B.PRED_TRACE, "none": B.PRED_NONE}[mode]
+            for n, pr in prompts.items():
+                cfg = dataclasses.replace(base, prompt_len=n, cache_slots=slots, stride=stride)
+                inj = None
+                if mode == "trace":
+                    if n not in routing:     # routing does not depend on the cache: record it once per prompt
+                        rec = ProMoE(w, cache_slots=slots, stride=1, predictor_mode=B.PRED_NONE, flags=flags | B.F_TRACE)
+                        routing[n] = []
+                        run_request(rec, cfg, pr, decode_ids, False, record=routing[n])
+                        rec.close()
+                    inj = routing[n]
+                eng = ProMoE(w, cache_slots=slots, stride=stride, chunk_bytes=chunk << 20, predictor_mode=pm, flags=flags,
+                             max_inflight=args.inflight, max_spec_decode=0 if mode == "trace" else args.max_spec_decode)
+                r = one(cfg, eng, pr, inject=inj)
+                eng.close()
+                d, p = r["dec"], r["pre"]
+                dec_s, pre_s = r["decode_ms"] / 1e3, r["prefill_ms"] / 1e3
+                copy_s = d["copy_busy_ms"] / 1e3
+                exposed = max(0.0, dec_s - compute[n][1] / 1e3)
+                pt = {"budget": frac, "predictor": mode, "stride": stride, "chunk_mib": chunk, "prompt": n,
+                      "decode_tokens_per_s": cfg.decode_steps / dec_s, "prefill_tokens_per_s": n / pre_s,
+                      "hit_rate": (d["hits_resident"] + d["hits_prefetch"]) / max(1, d["accesses"]),
+                      "hit_rate_resident": d["hits_resident"] / max(1, d["accesses"]),
+                      "predictor_accuracy": d["predicted_correct"] / max(1, d["predicted"]),
+                      "hidden_copy_fraction": max(0.0, 1.0 - exposed / copy_s) if copy_s > 0 else None,
+                      "byte_efficiency": d["need_experts"] * Be / max(1, d["h2d_bytes"]),
+                      "decode_roofline_frac": d["need_experts"] * Be / (h2d * 1e9) / dec_s,
+                      "prefill_roofline_frac": p["need_experts"] * Be / (h2d * 1e9) / pre_s}
+                points.append(pt)
+                print(json.dumps(pt), flush=True)
+    print(json.dumps({"sweep": "c5", "points": len(points), "h2d_gbs": h2d, "hbm_gbs": peaks["hbm_gbs"],
+                      "compute_only_ms": {str(k): v for k, v in compute.items()}}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -453,11 +533,15 @@ def main():
     ap.add_argument("--decode-steps", type=int, default=0)
     ap.add_argument("--ref-prompt", type=int, default=32, help="oracle sample: prompt tokens")
     ap.add_argument("--ref-decode", type=int, default=3, help="oracle sample: decode tokens")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] grid on the c3 shape (one JSON line per point)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-allhit", action="store_true")
     ap.add_argument("--variants", type=int, default=1, help="also measure the reactive and oracle-routing context points")
     args = ap.parse_args()
 
+    if args.sweep:
+        run_sweep(args)
+        return
     import synth
     over = {}
     if args.prompt_len:
