@@ -356,7 +356,7 @@ def run_ours(args, cfg, rank, world, dist):
     prof = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(prof):
         try:
-            kernel_roof["traffic"] = json.load(open(prof)).get("ffn_gateup_gemv_kernel")
+            kernel_roof["traffic"] = json.load(open(prof)).get(cfg.name, {}).get("ffn_gateup_gemv_kernel")
         except Exception:
             pass
     eng.close()

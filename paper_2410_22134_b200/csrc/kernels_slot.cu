@@ -100,28 +100,38 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (rf.pred_out) {
       const int nwarps = blockDim.x >> 5;
-      for (int e = warp; e < E; e += nwarps) {      // compact loops: this single-CTA kernel runs from a cold
-        float acc = 0.f;                              // instruction cache, code size is latency
+      // compact loops (this single-CTA kernel runs from a cold instruction cache: code size is latency), but two
+      // rows per warp with both rows' loads issued before any FMA: one DRAM round trip per 2 x 256 elements
+      for (int e = warp; e < E; e += 2 * nwarps) {
+        const int e1 = e + nwarps;
+        const bool two = e1 < E;
+        float a0 = 0.f, a1 = 0.f;
         if (rf.wdtype == 0) {
-          const float* wr = (const float*)rf.pred_w2 + (size_t)e * rf.ph;
-#pragma unroll 1
+          const float* w0 = (const float*)rf.pred_w2 + (size_t)e * rf.ph;
+          const float* w1 = (const float*)rf.pred_w2 + (size_t)(two ? e1 : e) * rf.ph;
+#pragma unroll 2
           for (int kk = lane * 4; kk + 4 <= rf.ph; kk += 128) {
-            float wv[4]; WVec<float>::load(wr + kk, wv);
+            float v0[4], v1[4];
+            WVec<float>::load(w0 + kk, v0); WVec<float>::load(w1 + kk, v1);
             const float4 xv = *reinterpret_cast<const float4*>(rf.p1 + kk);
-            acc = fmaf(wv[0], xv.x, acc); acc = fmaf(wv[1], xv.y, acc); acc = fmaf(wv[2], xv.z, acc); acc = fmaf(wv[3], xv.w, acc);
+            a0 = fmaf(v0[0], xv.x, a0); a0 = fmaf(v0[1], xv.y, a0); a0 = fmaf(v0[2], xv.z, a0); a0 = fmaf(v0[3], xv.w, a0);
+            a1 = fmaf(v1[0], xv.x, a1); a1 = fmaf(v1[1], xv.y, a1); a1 = fmaf(v1[2], xv.z, a1); a1 = fmaf(v1[3], xv.w, a1);
           }
         } else {
-          const __nv_bfloat16* wr = (const __nv_bfloat16*)rf.pred_w2 + (size_t)e * rf.ph;
-#pragma unroll 1
+          const __nv_bfloat16* w0 = (const __nv_bfloat16*)rf.pred_w2 + (size_t)e * rf.ph;
+          const __nv_bfloat16* w1 = (const __nv_bfloat16*)rf.pred_w2 + (size_t)(two ? e1 : e) * rf.ph;
+#pragma unroll 2
           for (int kk = lane * 8; kk + 8 <= rf.ph; kk += 256) {
-            float wv[8]; WVec<__nv_bfloat16>::load(wr + kk, wv);
+            float v0[8], v1[8];
+            WVec<__nv_bfloat16>::load(w0 + kk, v0); WVec<__nv_bfloat16>::load(w1 + kk, v1);
             const float4 x0 = *reinterpret_cast<const float4*>(rf.p1 + kk), x1 = *reinterpret_cast<const float4*>(rf.p1 + kk + 4);
-            acc = fmaf(wv[0], x0.x, acc); acc = fmaf(wv[1], x0.y, acc); acc = fmaf(wv[2], x0.z, acc); acc = fmaf(wv[3], x0.w, acc);
-            acc = fmaf(wv[4], x1.x, acc); acc = fmaf(wv[5], x1.y, acc); acc = fmaf(wv[6], x1.z, acc); acc = fmaf(wv[7], x1.w, acc);
+            const float xv[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { a0 = fmaf(v0[q], xv[q], a0); a1 = fmaf(v1[q], xv[q], a1); }
           }
         }
-        const float v = warp_sum(acc);
-        if (lane == 0) s_p2[e] = v;
+        a0 = warp_sum(a0); a1 = warp_sum(a1);
+        if (lane == 0) { s_p2[e] = a0; if (two) s_p2[e1] = a1; }
       }
     }
     __syncthreads();
