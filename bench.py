@@ -165,7 +165,7 @@ def workload_config(cfg, args):
                         f"prompt {cfg.prompt_len} + {cfg.decode_steps} decode",
             "cache_slots": cfg.cache_slots, "cache_fraction": cfg.slots_per_layer / s.n_experts, "stride": cfg.stride,
             "predictor": args.predictor, "decode_ids": args.decode, "chunk_bytes": args.chunk_mb << 20, "max_spec_decode": args.max_spec_decode,
-            "max_spec_prefill": args.max_spec_prefill,
+            "max_spec_prefill": args.max_spec_prefill, "low_cap_chunks": args.low_cap, "max_inflight": args.inflight,
             "l2": "inputs larger than L2 (each request streams >> 126 MB of expert weights)"}
 
 
@@ -285,7 +285,7 @@ def run_ours(args, cfg, rank, world, dist):
     eng = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_mb << 20,
                  predictor_mode=pmode, flags=flags,
                  max_inflight=args.inflight, max_spec_decode=args.max_spec_decode, max_spec_prefill=args.max_spec_prefill,
-                 device=f"cuda:{local}")
+                 low_cap_chunks=args.low_cap, device=f"cuda:{local}")
     for _ in range(args.warmup):
         run_request(eng, cfg, prompt, decode_ids, greedy, inject=inject)
     if dist is not None:
@@ -528,6 +528,7 @@ def main():
     ap.add_argument("--inflight", type=int, default=1, help="LOW chunks kept in flight (bounded preemption delay, P:191)")
     ap.add_argument("--max-spec-decode", type=int, default=1, help="allocations per PushPredicted in decode (0 = top_k as in Alg. 2, <0 = none); default 1: on a B200 one layer of\n                    compute hides about half an expert copy (profiles/r01_sweep_c2.md)")
     ap.add_argument("--max-spec-prefill", type=int, default=0, help="allocations per PushPredicted in prefill (<=0 = none)")
+    ap.add_argument("--low-cap", type=int, default=0, help="a LOW fill stops after this many chunks (0 = no cap)")
     ap.add_argument("--tensor", type=int, default=1, help="prefill GEMMs on tcgen05 (bf16 weights)")
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--decode-steps", type=int, default=0)

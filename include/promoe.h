@@ -80,6 +80,9 @@ typedef struct {
                               confident first); 0 = default top_k (all, as Alg. 2), < 0 = none (touch only) */
   int32_t max_spec_prefill;/* same for a prefill step (T > 1); <= 0 = default none: with 50-100 % of the experts needed
                                an allocation only swaps one needed expert for another (G7) */
+  int32_t low_cap_chunks;  /* a LOW (predicted) fill stops after this many chunks; the rest is fetched only if the gate needs
+                              the expert (then as HIGH).  0 = no cap.  Physical only: never changes a trace or an output */
+  int32_t reserved;
   void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
 } promoe_opts_t;
 

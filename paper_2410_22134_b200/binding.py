@@ -39,6 +39,7 @@ class promoe_opts_t(C.Structure):
     _fields_ = [("cache_slots", C.c_int32), ("stride", C.c_int32), ("chunk_bytes", C.c_uint64),
                 ("predictor_mode", C.c_int32), ("flags", C.c_int32), ("max_inflight", C.c_int32),
                 ("high_group", C.c_int32), ("max_spec_decode", C.c_int32), ("max_spec_prefill", C.c_int32),
+                ("low_cap_chunks", C.c_int32), ("reserved", C.c_int32),
                 ("compute_stream", C.c_void_p)]
 
 

@@ -90,43 +90,6 @@ __device__ __forceinline__ float row_dot(const WT* __restrict__ wrow, const floa
 }
 
 
-// Two weight rows against the same x (gate and up rows of a SwiGLU expert): both rows' 16-byte loads are issued
-// before any FMA (8 loads in flight per lane) and x is read once.
-template <typename WT>
-__device__ __forceinline__ void row_dot2(const WT* __restrict__ w0, const WT* __restrict__ w1, const float* __restrict__ x,
-                                         int K, int lane, float* r0, float* r1) {
-  constexpr int V = WVec<WT>::N;
-  constexpr int UNR = 4;
-  float a0[UNR] = {0.f, 0.f, 0.f, 0.f}, a1[UNR] = {0.f, 0.f, 0.f, 0.f};
-  int k = lane * V;
-  const int step = 32 * V;
-  for (; k + (UNR - 1) * step + V <= K; k += UNR * step) {
-    float wv0[UNR][V], wv1[UNR][V];
-#pragma unroll
-    for (int u = 0; u < UNR; ++u) { WVec<WT>::load(w0 + k + u * step, wv0[u]); WVec<WT>::load(w1 + k + u * step, wv1[u]); }
-#pragma unroll
-    for (int u = 0; u < UNR; ++u) {
-      const float4* xp = reinterpret_cast<const float4*>(x + k + u * step);
-#pragma unroll
-      for (int q = 0; q < V / 4; ++q) {
-        const float4 xv = __ldg(xp + q);
-        a0[u] = fmaf(wv0[u][4 * q + 0], xv.x, a0[u]); a1[u] = fmaf(wv1[u][4 * q + 0], xv.x, a1[u]);
-        a0[u] = fmaf(wv0[u][4 * q + 1], xv.y, a0[u]); a1[u] = fmaf(wv1[u][4 * q + 1], xv.y, a1[u]);
-        a0[u] = fmaf(wv0[u][4 * q + 2], xv.z, a0[u]); a1[u] = fmaf(wv1[u][4 * q + 2], xv.z, a1[u]);
-        a0[u] = fmaf(wv0[u][4 * q + 3], xv.w, a0[u]); a1[u] = fmaf(wv1[u][4 * q + 3], xv.w, a1[u]);
-      }
-    }
-  }
-  for (; k + V <= K; k += step) {
-    float wv0[V], wv1[V];
-    WVec<WT>::load(w0 + k, wv0); WVec<WT>::load(w1 + k, wv1);
-#pragma unroll
-    for (int q = 0; q < V; ++q) { const float xv = __ldg(x + k + q); a0[0] = fmaf(wv0[q], xv, a0[0]); a1[0] = fmaf(wv1[q], xv, a1[0]); }
-  }
-  *r0 = warp_sum((a0[0] + a0[1]) + (a0[2] + a0[3]));
-  *r1 = warp_sum((a1[0] + a1[1]) + (a1[2] + a1[3]));
-}
-
 constexpr int kMaxK = 16;
 // ---------------------------------------------------------------------------------------------------------
 // Warp-shuffle top-k.  One warp per token; lane holds experts lane, lane+32, ... (NPL per lane, E <= 32*NPL).

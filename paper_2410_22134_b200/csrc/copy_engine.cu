@@ -31,7 +31,6 @@ using namespace pmk;
     }                                                                                              \
   } while (0)
 
-typedef CUresult (*write32_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
 
 // retire finished timing slots of the ring; `all` = wait for every one (step end)
 int ce_retire(promoe_t* h, bool all) {
@@ -115,11 +114,13 @@ int ce_pump_low(promoe_t* h) {
   int rc = ce_retire(h, false);
   if (rc) return rc;
   while (!h->low.empty() && h->low_inflight < h->max_inflight && (h->high_inflight == 0 || !h->low_yields)) {
-    FillJob j = h->low.front();
+    FillJob& j = h->low.front();
     SlotPhys& p = h->phys[(size_t)j.layer * h->C + j.slot];
-    if (p.gen != j.gen || p.expert != j.expert || p.issued >= h->n_chunks) { h->low.pop_front(); continue; }  // stale / done
+    if (p.gen != j.gen || p.expert != j.expert || p.issued >= h->n_chunks ||
+        (h->low_cap > 0 && j.low_issued >= h->low_cap)) { h->low.pop_front(); continue; }  // stale / done / capped
     rc = issue_chunks(h, j.layer, j.slot, p.issued, p.issued + 1, true);
     if (rc) return rc;
+    j.low_issued++;
     if (p.issued >= h->n_chunks) h->low.pop_front();
   }
   return PROMOE_OK;
@@ -228,7 +229,7 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
         h->mirror[(size_t)mt * C + s] = e;
         p.gen = gen; p.expert = e; p.issued = 0; p.flagged = 0; p.done_valid = false;
       }
-      if (p.issued < h->n_chunks) h->low.push_back(FillJob{mt, s, e, gen, 1});   // alloc, or touch of a cancelled fill (G3)
+      if (p.issued < h->n_chunks) h->low.push_back(FillJob{mt, s, e, gen, 1, 0});   // alloc, or touch of a cancelled fill (G3)
     }
   }
   return ce_pump_low(h);

@@ -63,6 +63,7 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   h->n_chunks = (int)((h->Be + h->chunk_bytes - 1) / h->chunk_bytes);
   h->max_inflight = op->max_inflight > 0 ? op->max_inflight : 2;
   h->high_group = op->high_group > 0 ? op->high_group : 0;
+  h->low_cap = op->low_cap_chunks > 0 ? op->low_cap_chunks : 0;
   h->max_spec_decode = op->max_spec_decode == 0 ? s.top_k : std::max(0, op->max_spec_decode);
   h->max_spec_prefill = op->max_spec_prefill <= 0 ? 0 : op->max_spec_prefill;
   h->maxT = s.max_seq;
@@ -128,15 +129,6 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(cudaHostAlloc((void**)&h->ids_pin, sizeof(int32_t) * (size_t)T, cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->err_pin, sizeof(int), cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->flagsrc_host, sizeof(uint32_t) * 65536, cudaHostAllocDefault));
-    {
-      cudaDriverEntryPointQueryResult qr;
-      void* fn = nullptr;
-      if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
-          qr == cudaDriverEntryPointSuccess)
-        h->fn_write32 = fn;
-      else
-        (void)cudaGetLastError();
-    }
     h->phys.resize((size_t)Lm * C);
     for (auto& p : h->phys) CK(cudaEventCreateWithFlags(&p.done, cudaEventDisableTiming));
     const int ring = 8192;

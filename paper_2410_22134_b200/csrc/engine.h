@@ -18,6 +18,7 @@ struct FillJob {
   int layer, slot, expert;
   uint32_t gen;
   int prio;  // 0 HIGH, 1 LOW
+  int low_issued = 0;   // chunks this LOW job has put on the copy stream (capped by low_cap_chunks)
 };
 // Physical state of a slot (what the copy stream has been asked to do), as opposed to the logical table on
 // the device.  issued = chunks of generation `gen` already enqueued on the copy stream, in chunk order.
@@ -83,9 +84,8 @@ struct promoe {
   pmk::SlotTable tbl{};
   pmk::LayerCmd* cmd_host = nullptr;   // mapped pinned, [Lm]
   pmk::LayerCmd* cmd_dev = nullptr;
-  uint32_t* flagsrc_host = nullptr;       // pinned ring of flag values (fallback flag writes)
+  uint32_t* flagsrc_host = nullptr;       // pinned ring holding the generation values the flag copies read
   size_t flagsrc_pos = 0;
-  void* fn_write32 = nullptr;             // cuStreamWriteValue32, if the driver exposes it
 
   // copy engine (host)
   std::vector<pmk::SlotPhys> phys;     // [Lm*C]
@@ -95,6 +95,7 @@ struct promoe {
   size_t ev_head = 0, ev_tail = 0;        // in flight = [tail, head)
   std::vector<int> ev_is_low;
   int low_inflight = 0, high_inflight = 0;
+  int low_cap = 0;                    // LOW fills stop after this many chunks (0 = no cap)
   int high_group = 0;                 // chunks per HIGH copy operation, 0 = whole remaining fill in one copy
   bool want_done_events = false;      // prefill: per-fill completion events for cudaStreamWaitEvent
   bool low_yields = true;             // LOW chunks wait while HIGH fills are outstanding

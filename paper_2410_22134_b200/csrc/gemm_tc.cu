@@ -92,7 +92,6 @@ struct TcKernelArgs {
   int p0, rows;
   const uint8_t* slot_base;
   unsigned long long a_batch_stride;
-  int use_wd;
   __nv_bfloat16* o_hi;
   unsigned long long o_lo_off;
   int ldo;
@@ -325,7 +324,7 @@ bool tc_launch(TcContext* c, const TcGemm& g, cudaStream_t st, std::string* err)
   if (!mA0 || !mA1 || !mB) return false;
   TcKernelArgs a{};
   a.K = g.K; a.N = g.N; a.a1_row_off = g.a1_row_off; a.probs = g.probs; a.p0 = g.p0; a.rows = g.rows;
-  a.slot_base = g.slot_base; a.a_batch_stride = g.a_batch_stride; a.use_wd = g.use_wd ? 1 : 0;
+  a.slot_base = g.slot_base; a.a_batch_stride = g.a_batch_stride;
   a.o_hi = g.o_hi; a.o_lo_off = g.o_lo_off; a.ldo = g.ldo; a.y = g.y; a.ldy = g.ldy; a.flags = g.flags;
   const int max_rows = g.probs ? g.max_rows : g.rows;
   if (max_rows <= 0) return true;

@@ -30,7 +30,6 @@ struct TcGemm {
   const FfnProblem* probs = nullptr;   // device; row ranges (and, with slot_base, the slot of each problem)
   int p0 = 0, np = 1, rows = 0, max_rows = 0;
   const uint8_t* slot_base = nullptr;  // batch index of a problem = (pb.wg - slot_base) / a_batch_stride
-  bool use_wd = false;                 // slot images: the A operand is the problem's wd (down) instead of wg
   // outputs
   bool swiglu = false;
   __nv_bfloat16* o_hi = nullptr;       // swiglu: silu(g)*u as hi/lo planes [.., ldo]

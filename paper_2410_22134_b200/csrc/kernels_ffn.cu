@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(256) ffn_gateup_gemv_kernel(const float* __res
   const int r = r0 + warp;
   if (r >= pb.inter) return;
   // two passes (4 loads in flight per lane each): 48 registers keep 40 warps/SM resident, so the c2/c3 grid
-  // (5632 / 8448 warps) is a single wave; the fused two-row variant (row_dot2) needs 2 waves and measured slower
+  // (5632 / 8448 warps) is a single wave; a fused two-row variant (8 loads in flight per lane, 2 waves) measured slower: 16.1 vs 12.3 µs
 #ifndef PROMOE_K6_UNR
 #define PROMOE_K6_UNR 4
 #endif

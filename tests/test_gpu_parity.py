@@ -179,7 +179,8 @@ def test_outputs_independent_of_cache_parameters():
             assert np.array_equal(a, b), f"tcgen05 path: logits differ bitwise for {kw}"
     variants = [dict(cache_slots=4), dict(cache_slots=8, stride=2), dict(cache_slots=8, chunk_bytes=1 << 14),
                 dict(cache_slots=12, predictor_mode=B.PRED_NONE), dict(cache_slots=8, flags=B.F_REORDER | B.F_TRACE),
-                dict(cache_slots=4, chunk_bytes=1 << 18, max_inflight=1), dict(cache_slots=8, chunk_bytes=1 << 16, high_group=2)]
+                dict(cache_slots=4, chunk_bytes=1 << 18, max_inflight=1), dict(cache_slots=8, chunk_bytes=1 << 16, high_group=2),
+                dict(cache_slots=8, chunk_bytes=1 << 16, low_cap_chunks=2, max_inflight=1)]
     for kw in variants:
         out = run_gpu_only(cfg, w, prompt, ids, **kw)
         for a, b in zip(base["logits"], out["logits"]):
@@ -207,3 +208,46 @@ def test_prefill_equals_prefill_plus_decode():
     assert np.abs(a - b).max() <= 1e-4 * max(1.0, np.abs(a).max())
     assert np.abs(a - c).max() <= 1e-4 * max(1.0, np.abs(a).max())
     assert int(a.argmax()) == int(b.argmax()) == int(c.argmax())
+
+
+def test_edge_cases_and_error_paths():
+    """Degenerate inputs: zero tokens, id out of range, sequence overflow (errors, no abort); a 1-token prefill is
+    the decode step (bitwise); the handle stays usable after an error."""
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+    cfg = synth.get_config("c1")
+    w = synth.make_weights(cfg)
+    eng = ProMoE(w, cache_slots=8)
+    try:
+        with pytest.raises(B.PromoeError) as e:
+            B.promoe_prefill(eng.h, np.zeros(0, dtype=np.int32), None)
+        assert e.value.code == B.PROMOE_EINVAL
+        with pytest.raises(B.PromoeError) as e:
+            eng.decode(cfg.shape.vocab)                      # id out of range
+        assert e.value.code == B.PROMOE_EINVAL
+        with pytest.raises(B.PromoeError) as e:
+            eng.prefill(list(range(cfg.shape.max_seq + 1)))  # longer than max_seq
+        assert e.value.code == B.PROMOE_ESTATE
+        a = eng.prefill([7])                                 # T = 1 through promoe_prefill
+        eng.reset()
+        b = eng.decode(7)
+        assert np.array_equal(a, b)
+        eng.reset()
+        eng.prefill(synth.make_prompt(cfg, cfg.shape.max_seq - 1).tolist())
+        eng.decode(3)                                        # fills the sequence exactly
+        with pytest.raises(B.PromoeError) as e:
+            eng.decode(3)
+        assert e.value.code == B.PROMOE_ESTATE
+        assert eng.stats()["timeouts"] == 0
+    finally:
+        eng.close()
+
+
+def test_top_k_equals_n_experts():
+    """k = E: every expert is selected, gates are the plain softmax of all logits, margin is +inf, the cache must hold
+    all experts (C >= k) so nothing is ever fetched."""
+    cfg = synth.get_config("c1", shape_overrides={"top_k": 8}, cache_slots=16)
+    w = synth.make_weights(cfg, predictor="random")
+    out = run_parity(cfg, w, synth.make_prompt(cfg, 21), 5)
+    _report("c1 k=E", out)
+    assert out["stats"]["misses"] == 0 and out["stats"]["h2d_bytes"] == 0
