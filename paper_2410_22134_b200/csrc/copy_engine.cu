@@ -138,8 +138,9 @@ void ce_cancel_low(promoe_t* h, int m) {
 }
 
 // Wait (host) for the command of MoE layer m of step `seq`, pumping LOW chunks meanwhile.
-int ce_wait_cmd(promoe_t* h, int m, uint32_t seq) {
-  volatile uint32_t* w = &h->cmd_host[m].seq;
+// part 1 = the needed list (PushPrecise), 2 = the predicted list (PushPredicted, published later by the kernel)
+int ce_wait_cmd(promoe_t* h, int m, uint32_t seq, int part) {
+  volatile uint32_t* w = part == 2 ? &h->cmd_host[m].seq_pred : &h->cmd_host[m].seq;
   const auto t0 = std::chrono::steady_clock::now();
   unsigned spins = 0;
   while (*w != seq) {
@@ -173,11 +174,12 @@ int ce_issue_needed(promoe_t* h, int m, int i, cudaEvent_t after) {
 // Class-C fills whose slot is recycled inside the layer (dep >= 0: prefill with |needed| > C) are NOT
 // issued here: their indices are appended to `deferred` and the step scheduler issues them with
 // ce_issue_needed once the compute of launch position `dep` has been enqueued.
-int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
+int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred, int parts) {
   const LayerCmd& c = h->cmd_host[m];
   const int n = c.n_needed, E = h->s.n_experts, C = h->C;
   promoe_stats_t& st = h->st;
   { int rc0 = ce_retire(h, false); if (rc0) return rc0; }
+  if (parts & 1) {
   if (h->o.flags & PROMOE_F_PREEMPT) ce_cancel_low(h, m);
   // prediction accuracy: |pred ∩ needed| / |pred| for the list pushed into this layer
   std::vector<int32_t>& pend = h->pending_pred[m];
@@ -211,9 +213,10 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred) {
     int rc = ce_issue_needed(h, m, i, nullptr);
     if (rc) return rc;
   }
+  }   // parts & 1
   // PushPredicted(m + stride): LOW jobs (Alg. 2 l.1-10)
   const int mt = c.pred_target;
-  if (c.n_pred > 0 && mt < h->Lm) {
+  if ((parts & 2) && c.n_pred > 0 && mt < h->Lm) {
     std::vector<int32_t>& pd = h->pending_pred[mt];
     pd.clear();
     for (int i = 0; i < c.n_pred; ++i) {

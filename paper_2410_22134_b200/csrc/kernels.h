@@ -57,7 +57,8 @@ struct SlotTable {
 // Command record written to mapped pinned host memory, one per (step, MoE layer).  `seq` is written last
 // (release, system scope); the host issuer polls it.
 struct LayerCmd {
-  volatile uint32_t seq;     // step_seq * 4096 + layer + 1 when valid
+  volatile uint32_t seq;     // step_seq * 4096 + layer + 1 once the NEEDED part (PushPrecise) is valid
+  volatile uint32_t seq_pred;  // same value once the PREDICTED part (PushPredicted) is valid (published later)
   int32_t n_needed;
   int32_t n_pred;            // entries of the push INTO layer (m + stride), 0 if none
   int32_t pred_target;

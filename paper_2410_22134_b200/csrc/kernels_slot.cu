@@ -92,188 +92,202 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   __shared__ unsigned long long t_clock;
   __shared__ int32_t s_pred[kMaxE + 1];
   const int E = tbl.E, C = tbl.C;
-  // ---- fused decode front end (T == 1): router top-k + gates, predictor W2 GEMV + predicted list
-  if (rf.zraw) {
-    __shared__ float s_p2[kMaxE];
-    __shared__ int f_sel[2][kMaxK];
-    __shared__ float f_val[2][kMaxK];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (rf.pred_out) {
-      const int nwarps = blockDim.x >> 5;
-      // compact loops (this single-CTA kernel runs from a cold instruction cache: code size is latency), but two
-      // rows per warp with both rows' loads issued before any FMA: one DRAM round trip per 2 x 256 elements
-      for (int e = warp; e < E; e += 2 * nwarps) {
-        const int e1 = e + nwarps;
-        const bool two = e1 < E;
-        float a0 = 0.f, a1 = 0.f;
-        if (rf.wdtype == 0) {
-          const float* w0 = (const float*)rf.pred_w2 + (size_t)e * rf.ph;
-          const float* w1 = (const float*)rf.pred_w2 + (size_t)(two ? e1 : e) * rf.ph;
-#pragma unroll 2
-          for (int kk = lane * 4; kk + 4 <= rf.ph; kk += 128) {
-            float v0[4], v1[4];
-            WVec<float>::load(w0 + kk, v0); WVec<float>::load(w1 + kk, v1);
-            const float4 xv = *reinterpret_cast<const float4*>(rf.p1 + kk);
-            a0 = fmaf(v0[0], xv.x, a0); a0 = fmaf(v0[1], xv.y, a0); a0 = fmaf(v0[2], xv.z, a0); a0 = fmaf(v0[3], xv.w, a0);
-            a1 = fmaf(v1[0], xv.x, a1); a1 = fmaf(v1[1], xv.y, a1); a1 = fmaf(v1[2], xv.z, a1); a1 = fmaf(v1[3], xv.w, a1);
-          }
-        } else {
-          const __nv_bfloat16* w0 = (const __nv_bfloat16*)rf.pred_w2 + (size_t)e * rf.ph;
-          const __nv_bfloat16* w1 = (const __nv_bfloat16*)rf.pred_w2 + (size_t)(two ? e1 : e) * rf.ph;
-#pragma unroll 2
-          for (int kk = lane * 8; kk + 8 <= rf.ph; kk += 256) {
-            float v0[8], v1[8];
-            WVec<__nv_bfloat16>::load(w0 + kk, v0); WVec<__nv_bfloat16>::load(w1 + kk, v1);
-            const float4 x0 = *reinterpret_cast<const float4*>(rf.p1 + kk), x1 = *reinterpret_cast<const float4*>(rf.p1 + kk + 4);
-            const float xv[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-#pragma unroll
-            for (int q = 0; q < 8; ++q) { a0 = fmaf(v0[q], xv[q], a0); a1 = fmaf(v1[q], xv[q], a1); }
-          }
-        }
-        a0 = warp_sum(a0); a1 = warp_sum(a1);
-        if (lane == 0) { s_p2[e] = a0; if (two) s_p2[e1] = a1; }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  __shared__ float s_p2[kMaxE];
+  __shared__ int f_sel[2][kMaxK];
+  __shared__ float f_val[2][kMaxK];
+  __shared__ int32_t s_sel1[kMaxK];
+  __shared__ uint8_t prot2[kMaxE];       // membership of the predicted list (one push never evicts its own predictions)
+  const int mt_ = m + stride;
+  const bool have_t = pred_list != nullptr && mt_ < tbl.Lm;
+
+  // ================= phase 1: route (fused decode only) + PushPrecise(m) → first publication =====================
+  // The host needs only this part to issue the HIGH copies, so it is published BEFORE the predictor part runs.
+  if (rf.zraw && warp == 0) {     // A4: top-k by logit (ties → lower index), gates = softmax over the selected
+    if (E <= 32) front_route<1>(rf, E, lane, f_sel[0], f_val[0]);
+    else if (E <= 64) front_route<2>(rf, E, lane, f_sel[0], f_val[0]);
+    else if (E <= 128) front_route<4>(rf, E, lane, f_sel[0], f_val[0]);
+    else front_route<8>(rf, E, lane, f_sel[0], f_val[0]);
+  }
+  for (int i = threadIdx.x; i < C; i += blockDim.x) {
+    t_se[0][i] = tbl.slot_expert[(size_t)m * C + i]; t_stamp[0][i] = tbl.stamp[(size_t)m * C + i];
+    t_gen[0][i] = tbl.gen[(size_t)m * C + i]; t_org[0][i] = tbl.origin[(size_t)m * C + i];
+  }
+  for (int e = threadIdx.x; e < E; e += blockDim.x) t_es[0][e] = tbl.expert_slot[(size_t)m * E + e];
+  if (threadIdx.x == 0) t_clock = *tbl.clock;
+  for (int e = threadIdx.x; e < kMaxE; e += blockDim.x) { needed[e] = 0; prot[e] = 0; prot2[e] = 0; }
+  __syncthreads();                // sel (global, written by warp 0 in fused mode) is read below by this same block
+  if (T == 1 && threadIdx.x < k) s_sel1[threadIdx.x] = sel[threadIdx.x];
+  for (int i = threadIdx.x; i < T * k; i += blockDim.x) { const int e = sel[i]; needed[e] = 1; prot[e] = 1; }   // same-value writes
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
+    // classes A (cached) → B (being prefetched) → C (not begun), ascending id inside
+    int n = 0;
+    if (T == 1) {      // decode: only the k selected experts — sort them by id instead of scanning all E
+      int ids[kMaxK];
+      for (int j = 0; j < k; ++j) {
+        int e = s_sel1[j], q = j;
+        while (q > 0 && ids[q - 1] > e) { ids[q] = ids[q - 1]; --q; }
+        ids[q] = e;
       }
+      for (int c = 0; c < 3; ++c)
+        for (int j = 0; j < k; ++j) {
+          const int e = ids[j], sl = v.expert_slot[e];
+          const int ce = sl < 0 ? 2 : (v.origin[sl] == 1 ? 1 : 0);
+          if (ce == c) { order[n] = e; cls[n++] = (uint8_t)c; }
+        }
+    } else {
+      for (int e = 0; e < E; ++e)
+        if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] != 1) { order[n] = e; cls[n++] = 0; }
+      for (int e = 0; e < E; ++e)
+        if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] == 1) { order[n] = e; cls[n++] = 1; }
+      for (int e = 0; e < E; ++e)
+        if (needed[e] && v.expert_slot[e] < 0) { order[n] = e; cls[n++] = 2; }
+    }
+    if (trace_precise) trace_precise[0] = n;
+    // touch A then B (Alg. 2 l.15-17)
+    for (int i = 0; i < n && cls[i] != 2; ++i) {
+      const int e = order[i], sl = v.expert_slot[e];
+      v.touch(sl);
+      int32_t* r = rec + 7 * i;
+      r[0] = e; r[1] = cls[i]; r[2] = sl; r[3] = -1; r[4] = -1; r[5] = (int32_t)v.gen[sl];
+    }
+    // class C: alloc; a needed expert not yet computed in launch order is pinned (G2); all pinned → wait for the
+    // next finish in launch order.  prot[] == needed[] was prepared in parallel.
+    int fin = 0;
+    for (int i = 0; i < n; ++i) {
+      if (cls[i] != 2) continue;
+      const int e = order[i];
+      int dep = -1;
+      int sl = v.victim(prot);
+      while (sl < 0) { prot[order[fin]] = 0; dep = fin; ++fin; sl = v.victim(prot); }
+      const int old = v.install(sl, e, 2);
+      int32_t* r = rec + 7 * i;
+      r[0] = e; r[1] = 2; r[2] = sl; r[3] = old; r[4] = dep; r[5] = (int32_t)v.gen[sl];
+    }
+    for (int sl = 0; sl < C; ++sl) v.origin[sl] = 0;
+    // problem table + decode row map + trace
+    const size_t hi = (size_t)H * inter * wbytes;
+    for (int i = 0; i < n; ++i) {
+      const int32_t* r = rec + 7 * i;
+      const int e = order[i];
+      const int sl = r[2];   // the slot recorded at e's own alloc/touch (a later deferred alloc may recycle it)
+      const uint8_t* img = slot_base + ((size_t)m * C + sl) * slot_bytes;
+      FfnProblem pb;
+      pb.wg = img; pb.wu = img + hi; pb.wd = img + 2 * hi;
+      pb.flags = flag_base + ((size_t)m * C + sl) * flags_per_slot;
+      pb.gen = (uint32_t)r[5];
+      pb.inter = inter;
+      pb.row0 = offset ? offset[e] : i;
+      pb.nrows = offset ? offset[e + 1] - offset[e] : 1;
+      pb.expert = e; pb.pad = 0;
+      problems[i] = pb;
+      rec[7 * i + 6] = pb.nrows;
+      if (trace_precise) for (int q = 0; q < 5; ++q) trace_precise[1 + 5 * i + q] = r[q];
+    }
+    *n_problems = n;
+    if (row_of && T == 1)
+      for (int j = 0; j < k; ++j)
+        for (int i = 0; i < n; ++i) if (order[i] == s_sel1[j]) row_of[j] = i;
+    s_n = n;
+  }
+  __syncthreads();
+  // first publication (posted writes to mapped pinned memory; every writer fences its own stores; seq last)
+  for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
+  if (threadIdx.x == 0) cmd->n_needed = s_n;
+  __threadfence_system();
+  __syncthreads();
+  if (threadIdx.x == 0) { volatile uint32_t* sq = &cmd->seq; *sq = seq; }
+
+  // ================= phase 2: predictor W2 + list (fused decode only) + PushPredicted(m + stride) =================
+  if (rf.zraw && rf.pred_out) {
+    const int nwarps = blockDim.x >> 5;
+    // compact loops (this single-CTA kernel runs from a cold instruction cache: code size is latency); two rows
+    // per warp with both rows' loads issued before any FMA
+    for (int e = warp; e < E; e += 2 * nwarps) {
+      const int e1 = e + nwarps;
+      const bool two = e1 < E;
+      float a0 = 0.f, a1 = 0.f;
+      if (rf.wdtype == 0) {
+        const float* w0 = (const float*)rf.pred_w2 + (size_t)e * rf.ph;
+        const float* w1 = (const float*)rf.pred_w2 + (size_t)(two ? e1 : e) * rf.ph;
+#pragma unroll 2
+        for (int kk = lane * 4; kk + 4 <= rf.ph; kk += 128) {
+          float v0[4], v1[4];
+          WVec<float>::load(w0 + kk, v0); WVec<float>::load(w1 + kk, v1);
+          const float4 xv = *reinterpret_cast<const float4*>(rf.p1 + kk);
+          a0 = fmaf(v0[0], xv.x, a0); a0 = fmaf(v0[1], xv.y, a0); a0 = fmaf(v0[2], xv.z, a0); a0 = fmaf(v0[3], xv.w, a0);
+          a1 = fmaf(v1[0], xv.x, a1); a1 = fmaf(v1[1], xv.y, a1); a1 = fmaf(v1[2], xv.z, a1); a1 = fmaf(v1[3], xv.w, a1);
+        }
+      } else {
+        const __nv_bfloat16* w0 = (const __nv_bfloat16*)rf.pred_w2 + (size_t)e * rf.ph;
+        const __nv_bfloat16* w1 = (const __nv_bfloat16*)rf.pred_w2 + (size_t)(two ? e1 : e) * rf.ph;
+#pragma unroll 2
+        for (int kk = lane * 8; kk + 8 <= rf.ph; kk += 256) {
+          float v0[8], v1[8];
+          WVec<__nv_bfloat16>::load(w0 + kk, v0); WVec<__nv_bfloat16>::load(w1 + kk, v1);
+          const float4 x0 = *reinterpret_cast<const float4*>(rf.p1 + kk), x1 = *reinterpret_cast<const float4*>(rf.p1 + kk + 4);
+          const float xv[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+#pragma unroll
+          for (int q = 0; q < 8; ++q) { a0 = fmaf(v0[q], xv[q], a0); a1 = fmaf(v1[q], xv[q], a1); }
+        }
+      }
+      a0 = warp_sum(a0); a1 = warp_sum(a1);
+      if (lane == 0) { s_p2[e] = a0; if (two) s_p2[e1] = a1; }
     }
     __syncthreads();
-    if (warp == 0) {            // A4: top-k by logit (ties → lower index), gates = softmax over the selected
-      if (E <= 32) front_route<1>(rf, E, lane, f_sel[0], f_val[0]);
-      else if (E <= 64) front_route<2>(rf, E, lane, f_sel[0], f_val[0]);
-      else if (E <= 128) front_route<4>(rf, E, lane, f_sel[0], f_val[0]);
-      else front_route<8>(rf, E, lane, f_sel[0], f_val[0]);
-    } else if (warp == 1 && rf.pred_out) {   // A5: top-k of the predictor scores, listed by descending score
+    if (warp == 0) {              // A5: top-k of the predictor scores, listed by descending score
       if (E <= 32) front_pred<1>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
       else if (E <= 64) front_pred<2>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
       else if (E <= 128) front_pred<4>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
       else front_pred<8>(rf, s_p2, E, lane, f_sel[1], f_val[1]);
     }
-    __syncthreads();   // sel / pred_out (global) are read below by this same block
   }
-  __shared__ int32_t s_sel1[kMaxK];
-  if (T == 1) { if (threadIdx.x < k) s_sel1[threadIdx.x] = sel[threadIdx.x]; }
-  const int mt_ = m + stride;
-  const bool have_t = pred_list != nullptr && mt_ < tbl.Lm;
-  for (int i = threadIdx.x; i < C; i += blockDim.x) {
-    t_se[0][i] = tbl.slot_expert[(size_t)m * C + i]; t_stamp[0][i] = tbl.stamp[(size_t)m * C + i];
-    t_gen[0][i] = tbl.gen[(size_t)m * C + i]; t_org[0][i] = tbl.origin[(size_t)m * C + i];
-    if (have_t) {
+  if (have_t) {
+    for (int i = threadIdx.x; i < C; i += blockDim.x) {
       t_se[1][i] = tbl.slot_expert[(size_t)mt_ * C + i]; t_stamp[1][i] = tbl.stamp[(size_t)mt_ * C + i];
       t_gen[1][i] = tbl.gen[(size_t)mt_ * C + i]; t_org[1][i] = tbl.origin[(size_t)mt_ * C + i];
     }
+    for (int e = threadIdx.x; e < E; e += blockDim.x) t_es[1][e] = tbl.expert_slot[(size_t)mt_ * E + e];
   }
-  for (int e = threadIdx.x; e < E; e += blockDim.x) {
-    t_es[0][e] = tbl.expert_slot[(size_t)m * E + e];
-    if (have_t) t_es[1][e] = tbl.expert_slot[(size_t)mt_ * E + e];
-  }
+  __syncthreads();                // pred_out (global, written above in fused mode) is read below by this same block
   if (have_t) for (int i = threadIdx.x; i <= E; i += blockDim.x) s_pred[i] = pred_list[i];
-  if (threadIdx.x == 0) t_clock = *tbl.clock;
-  __shared__ uint8_t prot2[kMaxE];       // membership of the predicted list (one push never evicts its own predictions)
-  for (int e = threadIdx.x; e < kMaxE; e += blockDim.x) { needed[e] = 0; prot[e] = 0; prot2[e] = 0; }
   __syncthreads();
-  for (int i = threadIdx.x; i < T * k; i += blockDim.x) { const int e = sel[i]; needed[e] = 1; prot[e] = 1; }   // same-value writes
   if (have_t) for (int i = threadIdx.x; i < s_pred[0]; i += blockDim.x) prot2[s_pred[1 + i]] = 1;
   __syncthreads();
   if (threadIdx.x == 0) {
-
-  SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
-  // ---- PushPrecise(m): classes A (cached) → B (being prefetched) → C (not begun), ascending id inside
-  int n = 0;
-  if (T == 1) {      // decode: only the k selected experts — sort them by id instead of scanning all E
-    int ids[kMaxK];
-    for (int j = 0; j < k; ++j) {
-      int e = s_sel1[j], q = j;
-      while (q > 0 && ids[q - 1] > e) { ids[q] = ids[q - 1]; --q; }
-      ids[q] = e;
-    }
-    for (int c = 0; c < 3; ++c)
-      for (int j = 0; j < k; ++j) {
-        const int e = ids[j], sl = v.expert_slot[e];
-        const int ce = sl < 0 ? 2 : (v.origin[sl] == 1 ? 1 : 0);
-        if (ce == c) { order[n] = e; cls[n++] = (uint8_t)c; }
+    // PushPredicted(m + stride) (Alg. 2 l.1-10): touch cached, alloc missing as PRED; one push never evicts its own
+    // predictions; no victim → skip; at most max_spec allocations (knob G3; most confident first)
+    int np = 0;
+    if (have_t) {
+      SlotView t{t_se[1], t_es[1], t_stamp[1], t_gen[1], t_org[1], &t_clock, C, E};
+      np = s_pred[0];
+      int allocs = 0;
+      for (int i = 0; i < np; ++i) {
+        const int e = s_pred[1 + i];
+        int32_t* r = prec + 5 * i;
+        int sl = t.expert_slot[e];
+        if (sl >= 0) { t.touch(sl); r[0] = e; r[1] = 0; r[2] = sl; r[3] = -1; r[4] = (int32_t)t.gen[sl]; }
+        else {
+          sl = allocs < max_spec ? t.victim(prot2) : -1;
+          if (sl >= 0) ++allocs;
+          if (sl < 0) { r[0] = e; r[1] = 2; r[2] = -1; r[3] = -1; r[4] = 0; }
+          else { const int old = t.install(sl, e, 1); r[0] = e; r[1] = 1; r[2] = sl; r[3] = old; r[4] = (int32_t)t.gen[sl]; }
+        }
+        if (trace_pred) for (int q = 0; q < 4; ++q) trace_pred[1 + 4 * i + q] = r[q];
       }
-  } else {
-    for (int e = 0; e < E; ++e)
-      if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] != 1) { order[n] = e; cls[n++] = 0; }
-    for (int e = 0; e < E; ++e)
-      if (needed[e] && v.expert_slot[e] >= 0 && v.origin[v.expert_slot[e]] == 1) { order[n] = e; cls[n++] = 1; }
-    for (int e = 0; e < E; ++e)
-      if (needed[e] && v.expert_slot[e] < 0) { order[n] = e; cls[n++] = 2; }
-  }
-  if (trace_precise) trace_precise[0] = n;
-  // touch A then B (Alg. 2 l.15-17)
-  for (int i = 0; i < n && cls[i] != 2; ++i) {
-    const int e = order[i], s = v.expert_slot[e];
-    v.touch(s);
-    int32_t* r = rec + 7 * i;
-    r[0] = e; r[1] = cls[i]; r[2] = s; r[3] = -1; r[4] = -1; r[5] = (int32_t)v.gen[s];
-  }
-  // class C: alloc; a needed expert not yet computed in launch order is pinned (G2); all pinned → wait for the
-  // next finish in launch order
-  int fin = 0;                 // prot[] == needed[] was prepared in parallel
-  for (int i = 0; i < n; ++i) {
-    if (cls[i] != 2) continue;
-    const int e = order[i];
-    int dep = -1;
-    int s = v.victim(prot);
-    while (s < 0) { prot[order[fin]] = 0; dep = fin; ++fin; s = v.victim(prot); }
-    const int old = v.install(s, e, 2);
-    int32_t* r = rec + 7 * i;
-    r[0] = e; r[1] = 2; r[2] = s; r[3] = old; r[4] = dep; r[5] = (int32_t)v.gen[s];
-  }
-  for (int s = 0; s < C; ++s) v.origin[s] = 0;
-  // problem table + decode row map + trace
-  const size_t hi = (size_t)H * inter * wbytes;
-  for (int i = 0; i < n; ++i) {
-    const int32_t* r = rec + 7 * i;
-    const int e = order[i];
-    // the slot recorded at e's own alloc/touch (a later deferred alloc may recycle it after e finished)
-    const int s = r[2];
-    const uint8_t* img = slot_base + ((size_t)m * C + s) * slot_bytes;
-    FfnProblem pb;
-    pb.wg = img; pb.wu = img + hi; pb.wd = img + 2 * hi;
-    pb.flags = flag_base + ((size_t)m * C + s) * flags_per_slot;
-    pb.gen = (uint32_t)r[5];
-    pb.inter = inter;
-    pb.row0 = offset ? offset[e] : i;
-    pb.nrows = offset ? offset[e + 1] - offset[e] : 1;
-    pb.expert = e; pb.pad = 0;
-    problems[i] = pb;
-    rec[7 * i + 6] = pb.nrows;
-    if (trace_precise) for (int q = 0; q < 5; ++q) trace_precise[1 + 5 * i + q] = r[q];
-  }
-  *n_problems = n;
-  if (row_of && T == 1)
-    for (int j = 0; j < k; ++j)
-      for (int i = 0; i < n; ++i) if (order[i] == s_sel1[j]) row_of[j] = i;
-
-  // ---- PushPredicted(m + stride) (Alg. 2 l.1-10): touch cached, alloc missing as PRED; one push never evicts
-  // its own predictions; no victim → skip.
-  int np = 0;
-  const int mt = m + stride;
-  if (have_t) {
-    SlotView t{t_se[1], t_es[1], t_stamp[1], t_gen[1], t_org[1], &t_clock, C, E};
-    const int32_t* pred_list = s_pred;
-    np = pred_list[0];
-    const uint8_t* prot = prot2;
-    int allocs = 0;   // at most max_spec experts of one push may allocate (knob G3; most confident first)
-    for (int i = 0; i < np; ++i) {
-      const int e = pred_list[1 + i];
-      int32_t* r = prec + 5 * i;
-      int s = t.expert_slot[e];
-      if (s >= 0) { t.touch(s); r[0] = e; r[1] = 0; r[2] = s; r[3] = -1; r[4] = (int32_t)t.gen[s]; }
-      else {
-        s = allocs < max_spec ? t.victim(prot) : -1;
-        if (s >= 0) ++allocs;
-        if (s < 0) { r[0] = e; r[1] = 2; r[2] = -1; r[3] = -1; r[4] = 0; }
-        else { const int old = t.install(s, e, 1); r[0] = e; r[1] = 1; r[2] = s; r[3] = old; r[4] = (int32_t)t.gen[s]; }
-      }
-      if (trace_pred) for (int q = 0; q < 4; ++q) trace_pred[1 + 4 * i + q] = r[q];
     }
+    if (trace_pred) trace_pred[0] = np;
+    s_np = np;
   }
-  if (trace_pred) trace_pred[0] = np;
-  s_n = n; s_np = np;
-  (void)mt;
-  }  // thread 0
   __syncthreads();
+  // second publication
+  for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) cmd->pred[i] = prec[i];
+  if (threadIdx.x == 0) { cmd->n_pred = s_np; cmd->pred_target = m + stride; }
+  __threadfence_system();
+  __syncthreads();
+  if (threadIdx.x == 0) { volatile uint32_t* sq = &cmd->seq_pred; *sq = seq; }
   // write the staged rows back
   for (int i = threadIdx.x; i < C; i += blockDim.x) {
     tbl.slot_expert[(size_t)m * C + i] = t_se[0][i]; tbl.stamp[(size_t)m * C + i] = t_stamp[0][i];
@@ -288,16 +302,6 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     if (have_t) tbl.expert_slot[(size_t)mt_ * E + e] = t_es[1][e];
   }
   if (threadIdx.x == 0) *tbl.clock = t_clock;
-  // publish the command to the host issuer (posted writes to mapped pinned memory), seq last
-  for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
-  for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) cmd->pred[i] = prec[i];
-  if (threadIdx.x == 0) { cmd->n_needed = s_n; cmd->n_pred = s_np; cmd->pred_target = m + stride; }
-  __threadfence_system();      // every writer orders its own stores before the barrier
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    volatile uint32_t* sq = &cmd->seq;
-    *sq = seq;                 // release: the host issuer polls this word
-  }
 }
 
 void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int32_t* sel, int T, int k, const int32_t* offset,

@@ -23,8 +23,8 @@ using namespace pmk;
 
 int ce_retire(promoe_t* h, bool all);
 int ce_pump_low(promoe_t* h);
-int ce_wait_cmd(promoe_t* h, int m, uint32_t seq);
-int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred);
+int ce_wait_cmd(promoe_t* h, int m, uint32_t seq, int part);
+int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred, int parts);
 int ce_issue_deferred(promoe_t* h, int m, int i, cudaEvent_t after);
 
 #define CKS(call)                                                                                  \
@@ -155,12 +155,16 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
     launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, cs);
     launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, cs);
   }
-  RC(ce_wait_cmd(h, m, seq));                                                            // A7
-  RC(ce_process_cmd(h, m, nullptr));
+  RC(ce_wait_cmd(h, m, seq, 1));                                                         // A7: needed list → HIGH fills
+  RC(ce_process_cmd(h, m, nullptr, 1));
   launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
   launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,                 // K7
                           (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, s.n_shared_inter ? h->sy : nullptr, H, h->x,
                           wd, h->chunk_bytes, h->err_dev, cs);
+  // the predicted list is published by the second half of the slot-table kernel, which runs while the host issues
+  // the HIGH copies above: LOW jobs are queued as soon as it is there
+  RC(ce_wait_cmd(h, m, seq, 2));
+  RC(ce_process_cmd(h, m, nullptr, 2));
   return PROMOE_OK;
 }
 
@@ -253,10 +257,11 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
       if (s.shared_gate) { RC(linear(h, h->u, h->shared_gate_w[l], h->sgate, T, 1, H, 0)); sgate = h->sgate; }
     }
     // ---- A7: hand-over to the copy engine
-    int rc = ce_wait_cmd(h, m, seq);
+    int rc = ce_wait_cmd(h, m, seq, 1);
+    if (rc == PROMOE_OK) rc = ce_wait_cmd(h, m, seq, 2);
     if (rc) return rc;
     deferred.clear();
-    rc = ce_process_cmd(h, m, &deferred);
+    rc = ce_process_cmd(h, m, &deferred, 3);
     if (rc) return rc;
     const LayerCmd& cmd = h->cmd_host[m];
     const int n = cmd.n_needed;
