@@ -8,6 +8,25 @@ namespace pmk {
 
 constexpr int kWarp = 32;
 
+// ---- programmatic dependent launch (PDL): the decode step is a chain of ~8 short kernels per layer; launching
+// kernel n+1 while kernel n drains hides its launch / block-scheduling latency.  Every PDL-launched kernel calls
+// pdl_enter() before its first global access: it lets ITS dependents be scheduled and then waits until the kernel
+// in front of it has completed and flushed (so at most the prologue overlaps — no data hazard is possible).
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_enter() { pdl_trigger(); pdl_wait(); }
+extern bool g_use_pdl;   // PROMOE_PDL=0 disables (A/B measurements)
+template <typename... KArgs, typename... Args>
+inline void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = g_use_pdl ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // number of kernels launched by this library (host-side counter, bumped by every launch_* wrapper; promoe_stats)
 extern unsigned long long g_launches;
 

@@ -7,13 +7,17 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstdio>
 #include <cstring>
 
 using namespace pmk;
 
 static std::string g_create_err;
-namespace pmk { unsigned long long g_launches = 0; }
+namespace pmk {
+unsigned long long g_launches = 0;
+bool g_use_pdl = [] { const char* e = getenv("PROMOE_PDL"); return !(e && e[0] == '0'); }();
+}
 
 #define CK(call)                                                                                   \
   do {                                                                                             \

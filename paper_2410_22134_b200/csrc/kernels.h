@@ -81,12 +81,13 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
 //  gateup: act[p, i] = silu(Wg_p[i,:].u) * (Wu_p[i,:].u)     down: y[p, h] = Wd_p[h,:].act[p,:]
 // chunk geometry: image = [gate | up | down], chunk c covers bytes [c*chunk_bytes, (c+1)*chunk_bytes).
 void launch_ffn_gateup_gemv(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
-                            int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st);
+                            int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st,
+                            int static_table = 0);   // 1: records written at load time → early L2 prefetch under PDL
 // TMA-fed variant (bf16 weights, H <= 2048, H % 256 == 0); false = shape unsupported, nothing launched
 bool launch_ffn_gateup_gemv_tma(const float* u, const FfnProblem* probs, int n_probs, int inter, int H, float* act,
                                 int act_stride, size_t chunk_bytes, int* err, cudaStream_t st);
 void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int max_inter,
-                          int H, float* y, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st);
+                          int H, float* y, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st, int static_table = 0);
 // A9 prefill grouped SwiGLU FFN, SIMT fp32: problems [p0, p0+np) each with its row range; x rows are gathered
 // through row_src (permuted position -> row_src[pos] / src_div = token) or direct when row_src == nullptr.
 void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src_div, const FfnProblem* probs,

@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(256) norm_multi_gemv_kernel(NormGemvArgs a) {
   extern __shared__ float xs[];            // [K]
   __shared__ float red[8];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  pdl_enter();
   float ss = 0.f;
   for (int i = threadIdx.x; i < a.K; i += 256) { const float v = a.x[i]; xs[i] = v; ss += v * v; }
   ss = warp_sum(ss);
@@ -96,8 +97,8 @@ void launch_norm_multi_gemv(const NormGemvArgs& a_in, int wdtype, cudaStream_t s
   if (blocks > 148 * 8) blocks = 148 * 8;
   if (blocks < 1) blocks = 1;
   const size_t smem = (size_t)a.K * sizeof(float);
-  if (wdtype == 0) norm_multi_gemv_kernel<float><<<blocks, 256, smem, st>>>(a);
-  else norm_multi_gemv_kernel<__nv_bfloat16><<<blocks, 256, smem, st>>>(a);
+  if (wdtype == 0) launch_pdl(norm_multi_gemv_kernel<float>, dim3(blocks), dim3(256), smem, st, a);
+  else launch_pdl(norm_multi_gemv_kernel<__nv_bfloat16>, dim3(blocks), dim3(256), smem, st, a);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -114,6 +115,7 @@ __global__ void __launch_bounds__(128) attn_decode_fused_kernel(const float* __r
                                                                 int* __restrict__ counters, int pos, int nq, int nkv,
                                                                 int max_seq, int nsplit) {
   constexpr int PER = D / 8, HALF = D / 2;
+  pdl_enter();
   const int h = blockIdx.x, sp = blockIdx.y;
   const int grp_sz = nq / nkv, g = h / grp_sz;
   const int sub = threadIdx.x & 7, grp = threadIdx.x >> 3;
@@ -233,8 +235,8 @@ void launch_attn_decode_fused(const float* qkv, const float* cos_t, const float*
                               int nsplit, cudaStream_t st) {
   ++g_launches;
   dim3 grid(nq, nsplit);
-  if (d == 128) attn_decode_fused_kernel<128><<<grid, 128, 0, st>>>(qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);
-  else attn_decode_fused_kernel<64><<<grid, 128, 0, st>>>(qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);
+  if (d == 128) launch_pdl(attn_decode_fused_kernel<128>, grid, dim3(128), 0, st, qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);
+  else launch_pdl(attn_decode_fused_kernel<64>, grid, dim3(128), 0, st, qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -260,6 +262,7 @@ __global__ void __launch_bounds__(256) ffn_down_combine_kernel(const float* __re
   __shared__ int s_ni, s_ok;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r0 = blockIdx.x * DC_ROWS;
+  pdl_enter();
   // prologue in parallel: thread j loads problem j (j == k: the shared expert) and waits for the chunk flags of the
   // down rows this CTA reads; thread 0 then cuts the dot products into items
   __shared__ FfnProblem s_pb[kMaxK + 1];
@@ -327,8 +330,8 @@ void launch_ffn_down_combine(const float* act, int act_stride, const FfnProblem*
                              size_t chunk_bytes, int* err, cudaStream_t st) {
   ++g_launches;
   const int blocks = (H + DC_ROWS - 1) / DC_ROWS;
-  if (wdtype == 0) ffn_down_combine_kernel<float><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
-  else ffn_down_combine_kernel<__nv_bfloat16><<<blocks, 256, 0, st>>>(act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
+  if (wdtype == 0) launch_pdl(ffn_down_combine_kernel<float>, dim3(blocks), dim3(256), 0, st, act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
+  else launch_pdl(ffn_down_combine_kernel<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
 }
 
 }  // namespace pmk

@@ -52,6 +52,7 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ x, 
   const int lane = threadIdx.x & 31;
   const int warp = (blockIdx.x * 256 + threadIdx.x) >> 5;
   const int nwarps = (gridDim.x * 256) >> 5;
+  pdl_enter();
   for (int n = warp; n < N; n += nwarps) {
     float v = row_dot<WT>(w + (size_t)n * K, x, K, lane);
     if (lane == 0) {
@@ -65,8 +66,8 @@ void launch_gemv(const float* x, const void* w, float* y, int N, int K, int wdty
   ++g_launches;
   int blocks = (N + 7) / 8;
   if (blocks > 148 * 8) blocks = 148 * 8;   // 8 CTAs x 8 warps resident per SM; grid-stride over rows
-  if (wdtype == 0) gemv_kernel<float><<<blocks, 256, 0, st>>>(x, (const float*)w, y, N, K, flags);
-  else gemv_kernel<__nv_bfloat16><<<blocks, 256, 0, st>>>(x, (const __nv_bfloat16*)w, y, N, K, flags);
+  if (wdtype == 0) launch_pdl(gemv_kernel<float>, dim3(blocks), dim3(256), 0, st, x, (const float*)w, y, N, K, flags);
+  else launch_pdl(gemv_kernel<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, x, (const __nv_bfloat16*)w, y, N, K, flags);
 }
 
 // ---------------------------------------------------------------------------------------------------------

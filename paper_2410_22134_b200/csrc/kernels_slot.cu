@@ -93,6 +93,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   __shared__ int32_t s_pred[kMaxE + 1];
   const int E = tbl.E, C = tbl.C;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  pdl_enter();
   __shared__ float s_p2[kMaxE];
   __shared__ int f_sel[2][kMaxK];
   __shared__ float f_val[2][kMaxK];
@@ -313,9 +314,9 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
   (void)reorder;
   RouteFuse f{};
   if (rf) f = *rf;
-  slot_table_kernel<<<1, (rf && T == 1) ? 1024 : 256, 0, st>>>(tbl, m, stride, max_spec, sel, T, k, offset, pred_list, slot_base, slot_bytes,
-                                       flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of,
-                                       cmd, seq, trace_precise, trace_pred, f);
+  launch_pdl(slot_table_kernel, dim3(1), dim3((rf && T == 1) ? 1024 : 256), 0, st, tbl, m, stride, max_spec, sel, T, k, offset, pred_list,
+             slot_base, slot_bytes, flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of, cmd, seq,
+             trace_precise, trace_pred, f);
 }
 
 }  // namespace pmk

@@ -152,8 +152,8 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   // enqueued before the copies they wait for: when the driver multiplexes both streams onto one hardware queue a
   // resident spinning kernel starves the copy (seen on B200: 4 s flag time-outs), so copies always go first.
   if (s.n_shared_inter) {   // the whole shared expert runs under the hand-over / the copies; K7 only adds σ(gate)·sy
-    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, cs);
-    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, cs);
+    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, cs, 1);
+    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, cs, 1);
   }
   RC(ce_wait_cmd(h, m, seq, 1));                                                         // A7: needed list → HIGH fills
   RC(ce_process_cmd(h, m, nullptr, 1));
