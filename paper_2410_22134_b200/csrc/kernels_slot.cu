@@ -116,6 +116,8 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   }
   for (int e = threadIdx.x; e < E; e += blockDim.x) t_es[0][e] = tbl.expert_slot[(size_t)m * E + e];
   if (threadIdx.x == 0) t_clock = *tbl.clock;
+  __shared__ int32_t s_off[kMaxE + 1];    // prefill: group offsets staged in parallel (thread 0 reads them serially below)
+  if (offset) for (int e = threadIdx.x; e <= E; e += blockDim.x) s_off[e] = offset[e];
   for (int e = threadIdx.x; e < kMaxE; e += blockDim.x) { needed[e] = 0; prot[e] = 0; prot2[e] = 0; }
   __syncthreads();                // sel (global, written by warp 0 in fused mode) is read below by this same block
   if (T == 1 && threadIdx.x < k) s_sel1[threadIdx.x] = sel[threadIdx.x];
@@ -180,8 +182,8 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
       pb.flags = flag_base + ((size_t)m * C + sl) * flags_per_slot;
       pb.gen = (uint32_t)r[5];
       pb.inter = inter;
-      pb.row0 = offset ? offset[e] : i;
-      pb.nrows = offset ? offset[e + 1] - offset[e] : 1;
+      pb.row0 = offset ? s_off[e] : i;
+      pb.nrows = offset ? s_off[e + 1] - s_off[e] : 1;
       pb.expert = e; pb.pad = 0;
       problems[i] = pb;
       rec[7 * i + 6] = pb.nrows;

@@ -235,9 +235,15 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     int32_t* plist = nullptr;
     if (h->o.predictor_mode == PROMOE_PRED_MLP) {                                      // A5
       RC(linear(h, h->u, h->pred_w1[l], h->p1, T, s.pred_hidden, H, LIN_RELU, tc));
-      // W2 is tiny (E x ph): SIMT for T > 1, which also leaves the split of u in xsA for the shared expert
+      // the split of u must stay in xsA for the shared expert, so W2's input is split into another buffer
       if (T == 1) launch_gemv(h->p1, h->pred_w2[l], h->p2, E, s.pred_hidden, wd, 0, cs);
-      else launch_gemm_simt(h->p1, h->pred_w2[l], h->p2, T, E, s.pred_hidden, wd, 0, cs);
+      else if (tc && E >= 16) {   // tcgen05 too, with xsG as the split buffer (it is refilled with the gathered rows later)
+        launch_split_rows(h->p1, nullptr, 1, T, s.pred_hidden, h->xsG, h->xsG_half, cs);
+        TcGemm g;
+        g.a0 = h->pred_w2[l]; g.a_rows = E; g.b_hi = h->xsG; g.b_lo_off = h->xsG_half;
+        g.b_rows_cap = (int)(h->xsG_half / s.pred_hidden); g.K = s.pred_hidden; g.N = E; g.rows = T; g.y = h->p2; g.ldy = E;
+        if (!tc_launch(h->tc, g, cs, &h->err)) return PROMOE_ECUDA;
+      } else launch_gemm_simt(h->p1, h->pred_w2[l], h->p2, T, E, s.pred_hidden, wd, 0, cs);
       plist = h->pred_list + (size_t)m * (1 + E);
       launch_pred_list(h->p2, T, E, k, C, plist, cs);
     } else if (h->o.predictor_mode == PROMOE_PRED_TRACE) {
