@@ -70,10 +70,12 @@ typedef struct {
 typedef struct {
   int32_t cache_slots;     /* TOTAL slots; per MoE layer = cache_slots / n_moe_layers (must divide), G14 */
   int32_t stride;          /* predictor at MoE layer m targets MoE layer m+stride; >= 1 */
-  uint64_t chunk_bytes;    /* H2D chunk size; 0 = library default (measured curve) */
+  uint64_t chunk_bytes;    /* chunk size: granularity of the per-chunk ready flags and of the LOW (predicted)
+                              copies; a HIGH (precise) fill covers high_group chunks per copy.  0 = default 4 MiB
+                              (profiles/r01_fill_protocol.md); multiple of 256 */
   int32_t predictor_mode;
   int32_t flags;
-  int32_t max_inflight;    /* chunks kept in flight on the copy stream (P:191 bounded delay); 0 = default 2 */
+  int32_t max_inflight;    /* LOW chunks kept in flight on the copy stream (P:191 bounded preemption delay); 0 = default 2 */
   int32_t high_group;      /* chunks per HIGH (precise) copy operation; 0 = the whole remaining fill in ONE copy (measured
                               fastest); ready flags are written behind every operation */
   int32_t max_spec_decode; /* experts of one PushPredicted that may ALLOCATE a slot in a decode step (listed order = most

@@ -17,6 +17,9 @@ void launch_rmsnorm(const float* x, const float* w, float* y, int T, int H, floa
 enum { LIN_ACC = 1, LIN_RELU = 2 };
 // HBM-streaming GEMV (T == 1): one warp per output row, 16-byte loads.
 void launch_gemv(const float* x, const void* w, float* y, int N, int K, int wdtype, int flags, cudaStream_t st);
+// Small N, any T: one warp per output element (the N = 1 shared-expert gate in prefill).
+void launch_linear_small_n(const float* x, const void* w, float* y, int T, int N, int K, int wdtype, int flags,
+                           cudaStream_t st);
 // SIMT fp32 tiled GEMM (any T).
 void launch_gemm_simt(const float* x, const void* w, float* y, int T, int N, int K, int wdtype, int flags,
                       cudaStream_t st);

@@ -70,6 +70,29 @@ void launch_gemv(const float* x, const void* w, float* y, int N, int K, int wdty
   else launch_pdl(gemv_kernel<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, x, (const __nv_bfloat16*)w, y, N, K, flags);
 }
 
+// Small-N linear for T > 1 (e.g. the shared expert's scalar gate, N = 1): one warp per output element y[t, n].
+template <typename WT>
+__global__ void __launch_bounds__(256) linear_small_n_kernel(const float* __restrict__ x, const WT* __restrict__ w,
+                                                             float* __restrict__ y, int T, int N, int K, int flags) {
+  const int lane = threadIdx.x & 31;
+  const int o = (blockIdx.x * 256 + threadIdx.x) >> 5;
+  if (o >= T * N) return;
+  const int t = o / N, n = o % N;
+  float v = row_dot<WT>(w + (size_t)n * K, x + (size_t)t * K, K, lane);
+  if (lane == 0) {
+    if (flags & LIN_RELU) v = fmaxf(v, 0.f);
+    if (flags & LIN_ACC) v += y[o];
+    y[o] = v;
+  }
+}
+void launch_linear_small_n(const float* x, const void* w, float* y, int T, int N, int K, int wdtype, int flags,
+                           cudaStream_t st) {
+  ++g_launches;
+  const int blocks = (T * N + 7) / 8;
+  if (wdtype == 0) linear_small_n_kernel<float><<<blocks, 256, 0, st>>>(x, (const float*)w, y, T, N, K, flags);
+  else linear_small_n_kernel<__nv_bfloat16><<<blocks, 256, 0, st>>>(x, (const __nv_bfloat16*)w, y, T, N, K, flags);
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // SIMT fp32 GEMM  Y[T,N] (+)= X[T,K] . W[N,K]^T.  64x64x16 tiles, 256 threads, 4x4 micro-tile per thread.
 // Correctness path for prefill (the tcgen05 kernel in gemm_tc.cu is the fast path for bf16 weights).

@@ -47,6 +47,7 @@ static void split_A(promoe_t* h, const float* x, int T, int K) {
 // presplit: xsA already holds the hi/lo split of x.
 static int linear(promoe_t* h, const float* x, const void* w, float* y, int T, int N, int K, int flags, bool presplit = false) {
   if (T == 1) { launch_gemv(x, w, y, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
+  if (N <= 4) { launch_linear_small_n(x, w, y, T, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
   if (!use_tc(h, T) || N < 16) { launch_gemm_simt(x, w, y, T, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
   if (!presplit) split_A(h, x, T, K);
   TcGemm g;
