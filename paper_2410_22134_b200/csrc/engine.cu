@@ -79,6 +79,8 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     if (op->compute_stream) h->cs = (cudaStream_t)op->compute_stream;
     else { CK(cudaStreamCreateWithFlags(&h->cs, cudaStreamNonBlocking)); h->own_cs = true; }
     CK(cudaStreamCreateWithFlags(&h->ps, cudaStreamNonBlocking));
+    CK(cudaStreamCreateWithFlags(&h->cs2, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming)); CK(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
     CK(dalloc(&h->x, (size_t)T * H)); CK(dalloc(&h->u1, (size_t)T * H)); CK(dalloc(&h->u, (size_t)T * H));
     CK(dalloc(&h->qkv, (size_t)T * h->qkv_w)); CK(dalloc(&h->attn, (size_t)T * s.n_q_heads * s.head_dim));
     CK(dalloc(&h->zraw, (size_t)T * E)); CK(dalloc(&h->p1, (size_t)T * s.pred_hidden)); CK(dalloc(&h->p2, (size_t)T * E));
@@ -177,6 +179,9 @@ extern "C" void promoe_destroy(promoe_t* h) {
   if (h->step_start) cudaEventDestroy(h->step_start);
   if (h->step_end) cudaEventDestroy(h->step_end);
   if (h->ps) cudaStreamDestroy(h->ps);
+  if (h->cs2) cudaStreamDestroy(h->cs2);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
   if (h->own_cs && h->cs) cudaStreamDestroy(h->cs);
   delete h;
 }

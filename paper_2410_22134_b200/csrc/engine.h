@@ -42,6 +42,8 @@ struct promoe {
   int max_spec_decode = 0, max_spec_prefill = 0;   // allocations allowed per PushPredicted (knob G3)
   int maxT = 0, qkv_w = 0, ffn_w = 0, nsplit = 1;
   cudaStream_t cs = nullptr, ps = nullptr;
+  cudaStream_t cs2 = nullptr;                 // side compute stream: the shared expert runs beside the slot-table kernel
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   bool own_cs = false, dense_loaded = false, experts_loaded = false;
   std::string err;
 

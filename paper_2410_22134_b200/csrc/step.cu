@@ -138,6 +138,17 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   if (mlp) b.seg[b.nseg++] = GemvSeg{h->pred_w1[l], h->p1, s.pred_hidden, LIN_RELU};
   if (s.n_shared_inter && s.shared_gate) b.seg[b.nseg++] = GemvSeg{h->shared_gate_w[l], h->sgate, 1, 0};
   launch_norm_multi_gemv(b, wd, cs);
+  // The shared expert (resident weights, needs only u) runs on a side stream BESIDE the single-CTA slot-table kernel
+  // and the host hand-over instead of behind them; K7 joins it.  (Ordering of sact / sy / u across layers: the fork
+  // event of the next layer is recorded after this layer's K7, which has waited for the join event.)
+  if (s.n_shared_inter) {
+    if (cudaEventRecord(h->ev_fork, cs) != cudaSuccess || cudaStreamWaitEvent(h->cs2, h->ev_fork, 0) != cudaSuccess) {
+      h->err = "fork of the shared-expert stream failed"; return PROMOE_ECUDA;
+    }
+    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
+    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
+    if (cudaEventRecord(h->ev_join, h->cs2) != cudaSuccess) { h->err = "join event failed"; return PROMOE_ECUDA; }
+  }
   int32_t* plist = (mlp || h->o.predictor_mode == PROMOE_PRED_TRACE) ? h->pred_list + (size_t)m * (1 + E) : nullptr;
   RouteFuse rf{};                                                                        // K5
   rf.zraw = h->zraw; rf.bias = s.router_bias ? h->router_bias[l] : nullptr; rf.z_out = h->z + (size_t)m * h->maxT * E;
@@ -148,17 +159,13 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
                     (h->o.flags & PROMOE_F_REORDER) != 0, h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb, h->problems,
                     h->n_prob, h->row_of, h->cmd_dev + m, seq, h->trace_precise + (size_t)m * (1 + 5 * E),
                     (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf);
-  // The shared expert's gate/up GEMV (resident weights) is enqueued BEHIND the slot-table kernel and BEFORE the host
-  // looks at the command: it covers the device→host→device hand-over.  The flag-gated kernels K6/K7 must NOT be
-  // enqueued before the copies they wait for: when the driver multiplexes both streams onto one hardware queue a
-  // resident spinning kernel starves the copy (seen on B200: 4 s flag time-outs), so copies always go first.
-  if (s.n_shared_inter) {   // the whole shared expert runs under the hand-over / the copies; K7 only adds σ(gate)·sy
-    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, cs, 1);
-    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, cs, 1);
-  }
+  // The flag-gated kernels K6/K7 must NOT be enqueued before the copies they wait for: when the driver multiplexes
+  // the streams onto one hardware queue a resident spinning kernel starves the copy (seen on B200: 4 s flag
+  // time-outs), so copies always go first.
   RC(ce_wait_cmd(h, m, seq, 1));                                                         // A7: needed list → HIGH fills
   RC(ce_process_cmd(h, m, nullptr, 1));
   launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
+  if (s.n_shared_inter && cudaStreamWaitEvent(cs, h->ev_join, 0) != cudaSuccess) { h->err = "join of the shared-expert stream failed"; return PROMOE_ECUDA; }
   launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,                 // K7
                           (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, s.n_shared_inter ? h->sy : nullptr, H, h->x,
                           wd, h->chunk_bytes, h->err_dev, cs);
