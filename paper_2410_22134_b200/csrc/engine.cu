@@ -234,7 +234,7 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
       for (int i = 0; i < C; ++i) { se[(size_t)m * C + i] = i; es[(size_t)m * E + i] = i; stamp[(size_t)m * C + i] = (unsigned long long)m * C + i + 1; }
     clock = (unsigned long long)Lm * C;
   }
-  CK(cudaStreamSynchronize(h->cs)); CK(cudaStreamSynchronize(h->ps));
+  CK(cudaStreamSynchronize(h->cs)); CK(cudaStreamSynchronize(h->ps)); CK(cudaStreamSynchronize(h->cs2));
   CK(cudaMemcpy(h->tbl.slot_expert, se.data(), se.size() * 4, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(h->tbl.expert_slot, es.data(), es.size() * 4, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(h->tbl.stamp, stamp.data(), stamp.size() * 8, cudaMemcpyHostToDevice));
