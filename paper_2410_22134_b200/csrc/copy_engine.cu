@@ -77,14 +77,39 @@ static int write_flags(promoe_t* h, int m, int s) {
 // Enqueue chunks [c0, c1) of the fill (layer m, slot s) on the copy stream.  HIGH: `group` chunks per copy
 // operation (0 = all of them in one), flags written behind every operation; LOW: one chunk per call, flags deferred
 // until the fill completes or a HIGH operation takes it over.  One timing slot brackets the whole call.
+// HIGH fills that the host issues back to back (all missing experts of one layer) share ONE timing slot: event
+// records between the copies cost ≈ 2.5 % of the link (profiles/r01_fill_protocol.md, mode 3 vs plain copies).
+static int batch_begin(promoe_t* h) {
+  if (h->batch_open) return PROMOE_OK;
+  int rc = ring_slot(h, &h->batch_ri);
+  if (rc) return rc;
+  CKC(cudaEventRecord(h->ev_ring_start[h->batch_ri], h->ps));
+  h->batch_open = true; h->batch_used = false;
+  return PROMOE_OK;
+}
+static int batch_end(promoe_t* h) {
+  if (!h->batch_open) return PROMOE_OK;
+  h->batch_open = false;
+  if (!h->batch_used) return PROMOE_OK;        // nothing was copied: the start record is simply re-used later
+  CKC(cudaEventRecord(h->ev_ring[h->batch_ri], h->ps));
+  h->ev_is_low[h->batch_ri] = 0;
+  h->high_inflight++;
+  h->ev_head++;
+  return PROMOE_OK;
+}
+
 static int issue_chunks(promoe_t* h, int m, int s, int c0, int c1, bool low) {
   SlotPhys& p = h->phys[(size_t)m * h->C + s];
   const uint8_t* src = (const uint8_t*)h->expert_host[(size_t)m * h->s.n_experts + p.expert];
   uint8_t* dst = h->slots + ((size_t)m * h->C + s) * h->Be;
-  size_t ri = 0;
-  int rc = ring_slot(h, &ri);
-  if (rc) return rc;
-  CKC(cudaEventRecord(h->ev_ring_start[ri], h->ps));
+  const bool own_slot = !h->batch_open;        // LOW chunks and stand-alone HIGH fills bracket themselves
+  size_t ri = h->batch_ri;
+  int rc;
+  if (own_slot) {
+    rc = ring_slot(h, &ri);
+    if (rc) return rc;
+    CKC(cudaEventRecord(h->ev_ring_start[ri], h->ps));
+  } else h->batch_used = true;
   const int group = low ? 1 : (h->high_group > 0 ? h->high_group : h->n_chunks);
   for (int c = c0; c < c1; c += group) {
     const int ce = std::min(c1, c + group);
@@ -97,11 +122,13 @@ static int issue_chunks(promoe_t* h, int m, int s, int c0, int c1, bool low) {
     if (low) h->st.chunks_low += (uint64_t)(ce - c); else h->st.chunks_high += (uint64_t)(ce - c);
     if (!low || ce == h->n_chunks) { rc = write_flags(h, m, s); if (rc) return rc; }
   }
-  CKC(cudaEventRecord(h->ev_ring[ri], h->ps));
-  h->ev_is_low[ri] = low ? 1 : 0;
-  if (low) h->low_inflight++; else h->high_inflight++;
-  p.fill_seq = h->ev_head;           // complete once the ring tail has passed this slot
-  h->ev_head++;
+  p.fill_seq = h->ev_head;           // complete once the ring tail has passed this slot (the batch's, if batched)
+  if (own_slot) {
+    CKC(cudaEventRecord(h->ev_ring[ri], h->ps));
+    h->ev_is_low[ri] = low ? 1 : 0;
+    if (low) h->low_inflight++; else h->high_inflight++;
+    h->ev_head++;
+  }
   if (c1 == h->n_chunks && h->want_done_events) { CKC(cudaEventRecord(p.done, h->ps)); p.done_valid = true; }
   return PROMOE_OK;
 }
@@ -190,6 +217,7 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred, int parts) {
     pend.clear();
   }
   st.accesses += n;
+  { int rcb = batch_begin(h); if (rcb) return rcb; }
   for (int i = 0; i < n; ++i) {
     const int32_t* r = (const int32_t*)c.need + 7 * i;
     const int e = r[0], cls = r[1], s = r[2], victim = r[3], dep = r[4];
@@ -213,6 +241,7 @@ int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred, int parts) {
     int rc = ce_issue_needed(h, m, i, nullptr);
     if (rc) return rc;
   }
+  { int rce = batch_end(h); if (rce) return rce; }
   }   // parts & 1
   // PushPredicted(m + stride): LOW jobs (Alg. 2 l.1-10)
   const int mt = c.pred_target;

@@ -246,6 +246,7 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
   CK(cudaMemset(h->attn_cnt, 0, (size_t)h->s.n_q_heads * 4));
   h->mirror = se;
   h->low.clear();
+  h->batch_open = false;
   if (ce_retire(h, true)) return PROMOE_ECUDA;
   for (size_t i = 0; i < h->phys.size(); ++i) {
     SlotPhys& p = h->phys[i];

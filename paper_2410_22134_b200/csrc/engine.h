@@ -97,6 +97,8 @@ struct promoe {
   size_t ev_head = 0, ev_tail = 0;        // in flight = [tail, head)
   std::vector<int> ev_is_low;
   int low_inflight = 0, high_inflight = 0;
+  bool batch_open = false, batch_used = false;   // HIGH fills of one command share one timing slot
+  size_t batch_ri = 0;
   int low_cap = 0;                    // LOW fills stop after this many chunks (0 = no cap)
   int high_group = 0;                 // chunks per HIGH copy operation, 0 = whole remaining fill in one copy
   bool want_done_events = false;      // prefill: per-fill completion events for cudaStreamWaitEvent
