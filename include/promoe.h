@@ -61,7 +61,8 @@ typedef struct {
 #define PROMOE_PRED_TRACE 2  /* injected prediction lists (oracle-routing upper bound) */
 /* flags */
 #define PROMOE_F_PREEMPT 1   /* early preemption: drop un-issued LOW chunks of a layer at its gate */
-#define PROMOE_F_REORDER 2   /* reordered inference: cached -> being prefetched -> missing */
+#define PROMOE_F_REORDER 2   /* reordered inference: cached -> being prefetched -> missing.  ALWAYS ON in this version:
+                                the bit is accepted for ABI stability; the ID-order baseline is a later row */
 #define PROMOE_F_WARM 4      /* warm start: experts 0..C-1 resident in every layer (G4) */
 #define PROMOE_F_TRACE 8     /* record routing / permutation / cache traces for promoe_get_trace */
 #define PROMOE_F_NOFUSE 32  /* decode with the unfused per-op kernels (19 launches per layer) instead of the fused 7 */
