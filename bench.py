@@ -353,7 +353,7 @@ def run_ours(args, cfg, rank, world, dist):
                    "bytes_per_launch": bytes_gu, "avg_launch_us": ms_gu * 1e3, "traffic": None,
                    "down_gemv": {"achieved": bytes_dn / (ms_dn * 1e-3) / 1e9, "avg_launch_us": ms_dn * 1e3,
                                  "bytes_per_launch": bytes_dn}}
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    prof = os.path.join(ROOT, "profiles", "traffic.txt")
     if os.path.exists(prof):
         try:
             kernel_roof["traffic"] = json.load(open(prof)).get(cfg.name, {}).get("ffn_gateup_gemv_kernel")
