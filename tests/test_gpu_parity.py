@@ -145,7 +145,9 @@ def test_mini_configs(name, tensor):
     assert out["report"].max_hidden_ratio <= 1.0
 
 
-@pytest.mark.parametrize("name", ["c2", "c3"])
+@pytest.mark.parametrize("name", ["c2", "c3", pytest.param("c4", marks=pytest.mark.skipif(
+    not __import__("os").environ.get("PROMOE_TEST_C4"), reason="90 GB of pinned host memory and minutes of oracle time: "
+    "set PROMOE_TEST_C4=1 (run once per round, result recorded in DESIGN.md)"))])
 def test_full_size_configs(name):
     """BASELINE.json configs[1], configs[2] at FULL size (all layers, real vocab, 25-30 GB of routed experts in pinned
     host memory) in the launch configuration bench.py times (tcgen05 prefill, fused decode, default chunking): a
@@ -155,7 +157,8 @@ def test_full_size_configs(name):
     cfg = synth.get_config(name)
     w = synth.make_weights(cfg, predictor="skip")
     flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR
-    out = run_parity(cfg, w, synth.make_prompt(cfg, 48), 3, flags=flags, chunk_bytes=4 << 20, max_spec_decode=1)
+    T, n_dec = (48, 3) if name != "c4" else (12, 2)
+    out = run_parity(cfg, w, synth.make_prompt(cfg, T), n_dec, flags=flags, chunk_bytes=4 << 20, max_spec_decode=1)
     _report(name + "-full", out)
     assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
 
