@@ -513,6 +513,22 @@ def run_sweep(args):
                       "compute_only_ms": {str(k): v for k, v in compute.items()}}), flush=True)
 
 
+def run_probe_fill():
+    """A7 design evidence: pinned H2D bandwidth of copy-engine copies (promoe_measure_h2d) against SM-issued fills
+    (promoe_measure_sm_fill: a kernel reads mapped host memory with 16-byte loads), per copy size and grid."""
+    import torch
+    from paper_2410_22134_b200 import binding as B
+    torch.cuda.set_device(0)
+    Be = 17301504                                     # one c2/c3 expert image
+    ce = {f"{b >> 20}MiB" if b % (1 << 20) == 0 else str(b): round(B.promoe_measure_h2d(b, 1, 5), 2)
+          for b in (1 << 20, 4 << 20, Be, 256 << 20)}
+    sm = []
+    for nbytes in (Be, 256 << 20):
+        for ctas, thr in ((1, 256), (1, 1024), (2, 1024), (4, 1024), (8, 1024), (32, 1024), (148, 1024), (296, 1024)):
+            sm.append({"bytes": nbytes, "ctas": ctas, "threads": thr, "gbs": round(B.promoe_measure_sm_fill(nbytes, ctas, thr, 5), 2)})
+    print(json.dumps({"probe": "h2d fill: copy engine vs SM-issued", "copy_engine_gbs": ce, "sm_fill": sm}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -535,6 +551,7 @@ def main():
     ap.add_argument("--ref-prompt", type=int, default=32, help="oracle sample: prompt tokens")
     ap.add_argument("--ref-decode", type=int, default=3, help="oracle sample: decode tokens")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] grid on the c3 shape (one JSON line per point)")
+    ap.add_argument("--probe-fill", action="store_true", help="copy-engine vs SM-issued H2D fills (one JSON line), then exit")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-allhit", action="store_true")
     ap.add_argument("--variants", type=int, default=1, help="also measure the reactive and oracle-routing context points")
@@ -542,6 +559,9 @@ def main():
 
     if args.sweep:
         run_sweep(args)
+        return
+    if args.probe_fill:
+        run_probe_fill()
         return
     import synth
     over = {}

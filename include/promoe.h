@@ -173,6 +173,14 @@ PROMOE_API int promoe_get_slots(promoe_t* h, int32_t moe_layer, int32_t* slot_ex
  * (chunk size is chosen from this curve).  Allocates and frees its own buffers. */
 PROMOE_API int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out);
 
+/* Measured bandwidth (GB/s) of an SM-ISSUED fill: a kernel of `ctas` x `threads` reads `bytes` of pinned, mapped
+ * host memory with 16-byte loads and stores them into device memory (no copy engine, no host in the loop) — the
+ * device-side alternative to the copy-engine fills of A7 (Alg. 1 l.6-10 copies chunk by chunk; who issues
+ * the copy is left to the implementation).  DESIGN.md section 7 compares it with promoe_measure_h2d.  Allocates and
+ * frees its own buffers; the copied bytes are verified (PROMOE_ECUDA on mismatch).  bytes: multiple of 64; ctas >= 1;
+ * threads: multiple of 32 in [32, 1024]; best of `reps` timed launches after one warm-up. */
+PROMOE_API int promoe_measure_sm_fill(size_t bytes, int32_t ctas, int32_t threads, int32_t reps, double* gbs_out);
+
 /* Measured cost of the fill protocol itself:
  * n_fills expert images of expert_bytes each, pinned host -> device, back to back on one stream, every fill bracketed
  * by events as in the engine.  mode 0: one copy + one 32-bit stream write per chunk; 1: ONE copy per fill, then one

@@ -24,7 +24,7 @@ EXPORTS = [
     "promoe_create", "promoe_destroy", "promoe_last_error", "promoe_load_dense", "promoe_load_experts",
     "promoe_prefill", "promoe_decode", "promoe_set_prediction_trace", "promoe_stats", "promoe_get_trace",
     "promoe_reset", "promoe_get_slots", "promoe_measure_h2d", "promoe_op_linear", "promoe_op_route",
-    "promoe_op_permute", "promoe_op_expert_ffn", "promoe_kernel_time", "promoe_measure_fill",
+    "promoe_op_permute", "promoe_op_expert_ffn", "promoe_kernel_time", "promoe_measure_fill", "promoe_measure_sm_fill",
 ]
 
 
@@ -99,6 +99,7 @@ def lib() -> C.CDLL:
     L.promoe_op_permute.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_expert_ffn.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
     L.promoe_measure_fill.argtypes = [sz, sz, i32, i32, C.POINTER(C.c_double)]
+    L.promoe_measure_sm_fill.argtypes = [sz, i32, i32, i32, C.POINTER(C.c_double)]
     L.promoe_kernel_time.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     for n in EXPORTS:
         f = getattr(L, n)
@@ -182,6 +183,13 @@ def promoe_kernel_time(h, which: int, reps: int = 200):
     ms, nb = C.c_double(), C.c_double()
     _check(lib().promoe_kernel_time(h, which, reps, C.byref(ms), C.byref(nb)), h)
     return ms.value, nb.value
+
+
+def promoe_measure_sm_fill(nbytes: int, ctas: int, threads: int = 1024, reps: int = 3) -> float:
+    """GB/s of an SM-issued fill (kernel reads pinned mapped host memory); the copied bytes are verified."""
+    g = C.c_double()
+    _check(lib().promoe_measure_sm_fill(nbytes, ctas, threads, reps, C.byref(g)))
+    return g.value
 
 
 def promoe_measure_fill(expert_bytes: int, chunk_bytes: int, mode: int, n_fills: int = 32) -> float:

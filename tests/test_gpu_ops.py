@@ -220,3 +220,16 @@ def test_op_expert_ffn_tma_gemv(B, H, I):
     ref = swiglu_ffn(x.double(), wg, wu, wdn)
     err = (y.cpu().double() - ref).abs().max().item()
     assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
+
+
+def test_measure_sm_fill(B):
+    """SM-issued fill (promoe.h): copied bytes are verified inside the call; ragged 64-byte tail; bad arguments."""
+    L = B.lib()
+    import ctypes as C
+    g = C.c_double()
+    assert L.promoe_measure_sm_fill(0, 1, 256, 1, C.byref(g)) == B.PROMOE_EINVAL
+    assert L.promoe_measure_sm_fill(100, 1, 256, 1, C.byref(g)) == B.PROMOE_EINVAL          # not a multiple of 64
+    assert L.promoe_measure_sm_fill(1 << 20, 1, 100, 1, C.byref(g)) == B.PROMOE_EINVAL      # threads not a warp multiple
+    assert L.promoe_measure_sm_fill(1 << 20, 1, 256, 1, None) == B.PROMOE_EINVAL
+    for nbytes, ctas, thr in [(64, 1, 32), ((1 << 20) + 64, 3, 96), (17301504, 4, 1024), (64 << 20, 148, 256)]:
+        assert B.promoe_measure_sm_fill(nbytes, ctas, thr, 2) > 0.0
