@@ -106,6 +106,7 @@ void launch_norm_multi_gemv(const NormGemvArgs& a_in, int wdtype, cudaStream_t s
 // grid (nq, nsplit), 128 threads; 8 lanes share a key (d/8 contiguous floats each).  The new position `pos` is
 // served from shared memory (rotated k, raw v) by every CTA whose split contains it; exactly one CTA per kv head
 // also writes it into the cache.  counters[nq] must be zero on entry and is left zero.
+constexpr int kMaxSplit = 64;
 template <int D>
 __global__ void __launch_bounds__(128) attn_decode_fused_kernel(const float* __restrict__ qkv,
                                                                 const float* __restrict__ cos_t,
@@ -149,40 +150,50 @@ __global__ void __launch_bounds__(128) attn_decode_fused_kernel(const float* __r
   float m = -INFINITY, l = 0.f, o[PER];
 #pragma unroll
   for (int i = 0; i < PER; ++i) o[i] = 0.f;
-  for (int pb = p0; pb < p1; pb += 16) {      // uniform trip count: the 8-lane shuffles use the full mask
-    const int p = pb + grp;
-    const bool valid = p < p1;
-    float kv[PER], vv[PER];
-    if (valid) {
-      if (p == pos) {
+  // NB passes of 16 keys per round: the loads of all NB passes are issued before the first is consumed (the loop is
+  // latency-bound: 3-5 dependent passes at decode lengths); the arithmetic is per pass, in pass order, as before.
+  constexpr int NB = 3;
+  for (int pb0 = p0; pb0 < p1; pb0 += 16 * NB) {      // uniform trip counts: the 8-lane shuffles use the full mask
+    float kv[NB][PER], vv[NB][PER];
 #pragma unroll
-        for (int i = 0; i < PER; ++i) { kv[i] = sm_k[sub * PER + i]; vv[i] = sm_v[sub * PER + i]; }
-      } else {
-        const float4* kr = reinterpret_cast<const float4*>(kb + (size_t)p * D + sub * PER);
-        const float4* vr = reinterpret_cast<const float4*>(vb + (size_t)p * D + sub * PER);
+    for (int j = 0; j < NB; ++j) {
+      const int p = pb0 + 16 * j + grp;
+      if (p < p1) {
+        if (p == pos) {
 #pragma unroll
-        for (int i = 0; i < PER / 4; ++i) {
-          const float4 a = __ldcs(kr + i), b = __ldcs(vr + i);
-          kv[4 * i] = a.x; kv[4 * i + 1] = a.y; kv[4 * i + 2] = a.z; kv[4 * i + 3] = a.w;
-          vv[4 * i] = b.x; vv[4 * i + 1] = b.y; vv[4 * i + 2] = b.z; vv[4 * i + 3] = b.w;
+          for (int i = 0; i < PER; ++i) { kv[j][i] = sm_k[sub * PER + i]; vv[j][i] = sm_v[sub * PER + i]; }
+        } else {
+          const float4* kr = reinterpret_cast<const float4*>(kb + (size_t)p * D + sub * PER);
+          const float4* vr = reinterpret_cast<const float4*>(vb + (size_t)p * D + sub * PER);
+#pragma unroll
+          for (int i = 0; i < PER / 4; ++i) {
+            const float4 a = __ldcs(kr + i), b = __ldcs(vr + i);
+            kv[j][4 * i] = a.x; kv[j][4 * i + 1] = a.y; kv[j][4 * i + 2] = a.z; kv[j][4 * i + 3] = a.w;
+            vv[j][4 * i] = b.x; vv[j][4 * i + 1] = b.y; vv[j][4 * i + 2] = b.z; vv[j][4 * i + 3] = b.w;
+          }
         }
       }
     }
-    float s = 0.f;
-    if (valid) {
 #pragma unroll
-      for (int i = 0; i < PER; ++i) s = fmaf(q[i], kv[i], s);
+    for (int j = 0; j < NB; ++j) {
+      if (pb0 + 16 * j >= p1) break;                  // uniform over the CTA
+      const bool valid = pb0 + 16 * j + grp < p1;
+      float s = 0.f;
+      if (valid) {
+#pragma unroll
+        for (int i = 0; i < PER; ++i) s = fmaf(q[i], kv[j][i], s);
+      }
+      s += __shfl_xor_sync(0xffffffffu, s, 1);
+      s += __shfl_xor_sync(0xffffffffu, s, 2);
+      s += __shfl_xor_sync(0xffffffffu, s, 4);
+      if (!valid) continue;
+      const float mn = fmaxf(m, s);
+      const float corr = expf(m - mn), pw = expf(s - mn);
+      l = l * corr + pw;
+#pragma unroll
+      for (int i = 0; i < PER; ++i) o[i] = o[i] * corr + pw * vv[j][i];
+      m = mn;
     }
-    s += __shfl_xor_sync(0xffffffffu, s, 1);
-    s += __shfl_xor_sync(0xffffffffu, s, 2);
-    s += __shfl_xor_sync(0xffffffffu, s, 4);
-    if (!valid) continue;
-    const float mn = fmaxf(m, s);
-    const float corr = expf(m - mn), pw = expf(s - mn);
-    l = l * corr + pw;
-#pragma unroll
-    for (int i = 0; i < PER; ++i) o[i] = o[i] * corr + pw * vv[i];
-    m = mn;
   }
   // merge the 16 key groups of this CTA (fixed order)
   if (sub == 0) { sm_m[grp] = m; sm_l[grp] = l; }
@@ -213,19 +224,34 @@ __global__ void __launch_bounds__(128) attn_decode_fused_kernel(const float* __r
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  const volatile float* base = ws + (size_t)h * nsplit * (D + 2);
+  // (M, L) of every split staged in shared memory by one load round, partial rows read with all loads of a
+  // 16-split group in flight (L2 loads: the partials were written by other SMs); same arithmetic order as a serial
+  // loop over the splits.
+  const float* base = ws + (size_t)h * nsplit * (D + 2);
+  __shared__ float sm_M[kMaxSplit], sm_L[kMaxSplit];
+  for (int s2 = threadIdx.x; s2 < nsplit; s2 += 128) {
+    sm_M[s2] = __ldcg(base + (size_t)s2 * (D + 2) + D); sm_L[s2] = __ldcg(base + (size_t)s2 * (D + 2) + D + 1);
+  }
+  __syncthreads();
   float MM = -INFINITY;
-  for (int s2 = 0; s2 < nsplit; ++s2) MM = fmaxf(MM, base[(size_t)s2 * (D + 2) + D]);
+  for (int s2 = 0; s2 < nsplit; ++s2) MM = fmaxf(MM, sm_M[s2]);
   float LL = 0.f;
   for (int s2 = 0; s2 < nsplit; ++s2) {
-    const float ms = base[(size_t)s2 * (D + 2) + D];
-    if (ms != -INFINITY) LL += base[(size_t)s2 * (D + 2) + D + 1] * expf(ms - MM);
+    const float ms = sm_M[s2];
+    if (ms != -INFINITY) LL += sm_L[s2] * expf(ms - MM);
   }
   for (int c = threadIdx.x; c < D; c += 128) {
     float acc = 0.f;
-    for (int s2 = 0; s2 < nsplit; ++s2) {
-      const float ms = base[(size_t)s2 * (D + 2) + D];
-      if (ms != -INFINITY) acc += base[(size_t)s2 * (D + 2) + c] * expf(ms - MM);
+    for (int s0 = 0; s0 < nsplit; s0 += 16) {
+      float pv[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) pv[i] = (s0 + i < nsplit) ? __ldcg(base + (size_t)(s0 + i) * (D + 2) + c) : 0.f;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        if (s0 + i >= nsplit) break;
+        const float ms = sm_M[s0 + i];
+        if (ms != -INFINITY) acc += pv[i] * expf(ms - MM);
+      }
     }
     out[(size_t)h * D + c] = acc / LL;
   }
@@ -234,6 +260,7 @@ void launch_attn_decode_fused(const float* qkv, const float* cos_t, const float*
                               float* ws, float* out, int* counters, int pos, int nq, int nkv, int d, int max_seq,
                               int nsplit, cudaStream_t st) {
   ++g_launches;
+  if (nsplit > kMaxSplit) nsplit = kMaxSplit;       // engine uses 16
   dim3 grid(nq, nsplit);
   if (d == 128) launch_pdl(attn_decode_fused_kernel<128>, grid, dim3(128), 0, st, qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);
   else launch_pdl(attn_decode_fused_kernel<64>, grid, dim3(128), 0, st, qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos, nq, nkv, max_seq, nsplit);

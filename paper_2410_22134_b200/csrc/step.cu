@@ -106,6 +106,17 @@ static int expert_batch(promoe_t* h, const int32_t* perm, int i, int j, int max_
 
 #define RC(expr) do { int rc_ = (expr); if (rc_ != PROMOE_OK) return rc_; } while (0)
 
+// Knock-out timing (measurement builds only, -DPROMOE_KNOCKOUT; never compiled into the product): the environment
+// variable PROMOE_KNOCKOUT is a bit mask of decode kernels NOT to launch (bit 0 K1, 1 K2, 2 K3, 3 K4, 4 shared expert,
+// 6 K6, 7 K7).  Results are then meaningless; the drop in all-resident decode time is that kernel's in-situ cost on
+// the critical path.  K5 cannot be knocked out: the host waits for its command.
+#ifdef PROMOE_KNOCKOUT
+static const int g_knockout = [] { const char* e = getenv("PROMOE_KNOCKOUT"); return e ? atoi(e) : 0; }();
+#define KO(bit) (g_knockout & (1 << (bit)))
+#else
+#define KO(bit) 0
+#endif
+
 // One layer of the batch-1 decode step with the fused kernels of kernels_decode.cu (7 launches instead of 19).
 static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   const promoe_shape_t& s = h->s;
@@ -116,10 +127,10 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   NormGemvArgs a{};                                                                      // K1
   a.x = h->x; a.gain = h->ln1[l]; a.eps = s.rms_eps; a.K = H;
   a.seg[0] = GemvSeg{h->wqkv[l], h->qkv, h->qkv_w, 0}; a.nseg = 1;
-  launch_norm_multi_gemv(a, wd, cs);
-  launch_attn_decode_fused(h->qkv, h->cos_t, h->sin_t, h->kcache + (size_t)l * kv_layer, h->vcache + (size_t)l * kv_layer,   // K2
+  if (!KO(0)) launch_norm_multi_gemv(a, wd, cs);
+  if (!KO(1)) launch_attn_decode_fused(h->qkv, h->cos_t, h->sin_t, h->kcache + (size_t)l * kv_layer, h->vcache + (size_t)l * kv_layer,   // K2
                            h->attn_ws, h->attn, h->attn_cnt, pos0, nq, nkv, d, s.max_seq, h->nsplit, cs);
-  launch_gemv(h->attn, h->wo[l], h->x, H, nq * d, wd, LIN_ACC, cs);                      // K3
+  if (!KO(2)) launch_gemv(h->attn, h->wo[l], h->x, H, nq * d, wd, LIN_ACC, cs);          // K3
   NormGemvArgs b{};                                                                      // K4
   b.x = h->x; b.gain = h->ln2[l]; b.eps = s.rms_eps; b.K = H; b.u_out = h->u;
   if (l < s.n_dense_layers) {
@@ -137,7 +148,7 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   b.seg[b.nseg++] = GemvSeg{h->router[l], h->zraw, E, 0};
   if (mlp) b.seg[b.nseg++] = GemvSeg{h->pred_w1[l], h->p1, s.pred_hidden, LIN_RELU};
   if (s.n_shared_inter && s.shared_gate) b.seg[b.nseg++] = GemvSeg{h->shared_gate_w[l], h->sgate, 1, 0};
-  launch_norm_multi_gemv(b, wd, cs);
+  if (!KO(3)) launch_norm_multi_gemv(b, wd, cs);
   // The shared expert (resident weights, needs only u) runs on a side stream BESIDE the single-CTA slot-table kernel
   // and the host hand-over instead of behind them; K7 joins it.  (Ordering of sact / sy / u across layers: the fork
   // event of the next layer is recorded after this layer's K7, which has waited for the join event.)
@@ -145,8 +156,10 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
     if (cudaEventRecord(h->ev_fork, cs) != cudaSuccess || cudaStreamWaitEvent(h->cs2, h->ev_fork, 0) != cudaSuccess) {
       h->err = "fork of the shared-expert stream failed"; return PROMOE_ECUDA;
     }
-    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
-    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
+    if (!KO(4)) {
+      launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
+      launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
+    }
     if (cudaEventRecord(h->ev_join, h->cs2) != cudaSuccess) { h->err = "join event failed"; return PROMOE_ECUDA; }
   }
   int32_t* plist = (mlp || h->o.predictor_mode == PROMOE_PRED_TRACE) ? h->pred_list + (size_t)m * (1 + E) : nullptr;
@@ -164,11 +177,12 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   // time-outs), so copies always go first.
   RC(ce_wait_cmd(h, m, seq, 1));                                                         // A7: needed list → HIGH fills
   RC(ce_process_cmd(h, m, nullptr, 1));
-  launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
+  if (!KO(6)) launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
   if (s.n_shared_inter && cudaStreamWaitEvent(cs, h->ev_join, 0) != cudaSuccess) { h->err = "join of the shared-expert stream failed"; return PROMOE_ECUDA; }
-  launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,                 // K7
-                          (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, s.n_shared_inter ? h->sy : nullptr, H, h->x,
-                          wd, h->chunk_bytes, h->err_dev, cs);
+  if (!KO(7))
+    launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,               // K7
+                            (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, s.n_shared_inter ? h->sy : nullptr, H, h->x,
+                            wd, h->chunk_bytes, h->err_dev, cs);
   // the predicted list is published by the second half of the slot-table kernel, which runs while the host issues
   // the HIGH copies above: LOW jobs are queued as soon as it is there
   RC(ce_wait_cmd(h, m, seq, 2));
