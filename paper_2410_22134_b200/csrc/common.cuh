@@ -109,6 +109,56 @@ __device__ __forceinline__ float row_dot(const WT* __restrict__ wrow, const floa
 }
 
 
+// row_dot for SHORT rows (K <= NP passes of 32 lanes x 16 bytes; NP = 8: 2048 bf16 / 1024 fp32 elements): every load of the
+// row is issued before the first FMA (row_dot keeps 4 in flight and then walks the tail one dependent load at a time:
+// 3 latency rounds for K = 1408).  Same accumulators, same order → bit-identical to row_dot<WT, 4>.
+template <typename WT> struct WRaw;
+template <> struct WRaw<float> {
+  typedef float4 T;
+  __device__ __forceinline__ static T load(const float* p) { return __ldcs(reinterpret_cast<const float4*>(p)); }
+  __device__ __forceinline__ static void cvt(const T& r, float (&v)[4]) { v[0] = r.x; v[1] = r.y; v[2] = r.z; v[3] = r.w; }
+};
+template <> struct WRaw<__nv_bfloat16> {
+  typedef uint4 T;
+  __device__ __forceinline__ static T load(const __nv_bfloat16* p) { return __ldcs(reinterpret_cast<const uint4*>(p)); }
+  __device__ __forceinline__ static void cvt(const T& r, float (&v)[8]) {
+    v[0] = __uint_as_float(r.x << 16); v[1] = __uint_as_float(r.x & 0xffff0000u);
+    v[2] = __uint_as_float(r.y << 16); v[3] = __uint_as_float(r.y & 0xffff0000u);
+    v[4] = __uint_as_float(r.z << 16); v[5] = __uint_as_float(r.z & 0xffff0000u);
+    v[6] = __uint_as_float(r.w << 16); v[7] = __uint_as_float(r.w & 0xffff0000u);
+  }
+};
+template <typename WT, int NP = 8>
+__device__ __forceinline__ float row_dot_short(const WT* __restrict__ wrow, const float* __restrict__ x, int K, int lane) {
+  constexpr int V = WVec<WT>::N;
+  const int step = 32 * V, k0 = lane * V;
+  typename WRaw<WT>::T raw[NP];
+#pragma unroll
+  for (int j = 0; j < NP; ++j)
+    if (k0 + j * step + V <= K) raw[j] = WRaw<WT>::load(wrow + k0 + j * step);
+  float acc[4] = {0.f, 0.f, 0.f, 0.f};
+  bool main_ok = true;      // row_dot's main loop takes 4 passes at a time while the 4th exists, then the tail feeds acc[0]
+#pragma unroll
+  for (int j = 0; j < NP; ++j) {
+    const int k = k0 + j * step;
+    if ((j & 3) == 0) main_ok = main_ok && (k + 3 * step + V <= K);
+    if (k + V <= K) {
+      float wv[V];
+      WRaw<WT>::cvt(raw[j], wv);
+      float a = main_ok ? acc[j & 3] : acc[0];
+#pragma unroll
+      for (int q = 0; q < V / 4; ++q) {
+        const float4 xv = __ldg(reinterpret_cast<const float4*>(x + k) + q);
+        a = fmaf(wv[4 * q + 0], xv.x, a); a = fmaf(wv[4 * q + 1], xv.y, a);
+        a = fmaf(wv[4 * q + 2], xv.z, a); a = fmaf(wv[4 * q + 3], xv.w, a);
+      }
+      if (main_ok) acc[j & 3] = a; else acc[0] = a;
+    }
+  }
+  return warp_sum((acc[0] + acc[1]) + (acc[2] + acc[3]));
+}
+
+
 constexpr int kMaxK = 16;
 // ---------------------------------------------------------------------------------------------------------
 // Warp-shuffle top-k.  One warp per token; lane holds experts lane, lane+32, ... (NPL per lane, E <= 32*NPL).

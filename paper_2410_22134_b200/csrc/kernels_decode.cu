@@ -273,7 +273,7 @@ void launch_attn_decode_fused(const float* qkv, const float* cos_t, const float*
 // Routed experts are read from their slots behind the chunk-ready flags of exactly the rows this CTA reads.
 constexpr int DC_ROWS = 4, DC_PIECE = 2048, DC_MAX_ITEMS = 192;
 template <typename WT>
-__global__ void __launch_bounds__(256) ffn_down_combine_kernel(const float* __restrict__ act, int act_stride,
+__global__ void __launch_bounds__(256, 4) ffn_down_combine_kernel(const float* __restrict__ act, int act_stride,
                                                                const FfnProblem* __restrict__ probs,
                                                                const int32_t* __restrict__ row_of,
                                                                const float* __restrict__ gates, int k,
@@ -328,7 +328,11 @@ __global__ void __launch_bounds__(256) ffn_down_combine_kernel(const float* __re
   for (int w = warp; w < DC_ROWS * ni; w += 8) {
     const int rr = w / ni, it = w % ni, r = r0 + rr;
     if (r >= H) continue;
-    const float v = row_dot<WT>((const WT*)it_w[it] + (size_t)r * it_ld[it] + it_off[it], it_x[it] + it_off[it], it_len[it], lane);
+    // pieces are <= DC_PIECE = 2048 elements: bf16 rows always take the all-loads-in-flight form
+    const WT* wr = (const WT*)it_w[it] + (size_t)r * it_ld[it] + it_off[it];
+    const int len = it_len[it];
+    const float v = len <= 8 * 32 * WVec<WT>::N ? row_dot_short<WT, 8>(wr, it_x[it] + it_off[it], len, lane)
+                                                 : row_dot<WT>(wr, it_x[it] + it_off[it], len, lane);
     if (lane == 0) part[rr][it] = v;
   }
   __syncthreads();
