@@ -49,9 +49,10 @@ __device__ __forceinline__ float row_dot_s(const WT* __restrict__ wrow, const fl
 
 // ---------------------------------------------------------------------------------------------------------------
 // K1 / K4 / lm_head: u = RMSNorm(x; gain) staged once per CTA in shared memory, then one warp per weight row over a
-// list of segments.  Persistent grid (≤ 148·8 CTAs), rows dealt round-robin to warps.
+// list of segments.  Persistent grid (≤ 148·6 CTAs = one resident wave; the QKV GEMV of c2/c3 is 768 CTAs, which at
+// 48 registers / 5 CTAs per SM spilled into a 28-CTA second wave), rows dealt round-robin to warps.
 template <typename WT>
-__global__ void __launch_bounds__(256) norm_multi_gemv_kernel(NormGemvArgs a) {
+__global__ void __launch_bounds__(256, 6) norm_multi_gemv_kernel(NormGemvArgs a) {
   extern __shared__ float xs[];            // [K]
   __shared__ float red[8];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -94,7 +95,7 @@ void launch_norm_multi_gemv(const NormGemvArgs& a_in, int wdtype, cudaStream_t s
   a.n_rows_total = a.n_sw;
   for (int s = 0; s < a.nseg; ++s) a.n_rows_total += a.seg[s].n;
   int blocks = (a.n_rows_total + 7) / 8;
-  if (blocks > 148 * 8) blocks = 148 * 8;
+  if (blocks > 148 * 6) blocks = 148 * 6;   // 6 CTAs resident per SM (40 registers, __launch_bounds__(256, 6)): one wave
   if (blocks < 1) blocks = 1;
   const size_t smem = (size_t)a.K * sizeof(float);
   if (wdtype == 0) launch_pdl(norm_multi_gemv_kernel<float>, dim3(blocks), dim3(256), smem, st, a);
