@@ -54,7 +54,8 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ x, 
   const int nwarps = (gridDim.x * 256) >> 5;
   pdl_enter();
   for (int n = warp; n < N; n += nwarps) {
-    float v = row_dot<WT>(w + (size_t)n * K, x, K, lane);
+    // rows of <= 8 passes (O-projection, K = 2048 bf16): every load in flight at once; same summation order
+    float v = (K <= 8 * 32 * WVec<WT>::N) ? row_dot_short<WT, 8>(w + (size_t)n * K, x, K, lane) : row_dot<WT>(w + (size_t)n * K, x, K, lane);
     if (lane == 0) {
       if (flags & LIN_RELU) v = fmaxf(v, 0.f);
       if (flags & LIN_ACC) v += y[n];
