@@ -45,7 +45,7 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
         logits = eng.prefill(ids)
         tr = eng.trace(T)
         st = oracle_step_matching(ora, ids, tr["sel"], rep)
-        compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred)
+        compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred, pred_cap=C)
         compare_cache(sim, tr, stride, use_pred, ms_pre)
         all_logits.append(logits)
         nxt = st.next_token
@@ -54,7 +54,7 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
             logits = eng.decode(tok)
             tr = eng.trace(1)
             st = oracle_step_matching(ora, [tok], tr["sel"], rep)
-            compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred)
+            compare_step(tr, st, s.n_experts, rep, gpu_logits=logits, check_pred=use_pred, pred_cap=C)
             compare_cache(sim, tr, stride, use_pred, ms_dec)
             all_logits.append(logits)
             nxt = st.next_token
