@@ -164,8 +164,8 @@ def workload_config(cfg, args):
                         f"{s.n_layers}L H{s.hidden} E{s.n_experts} top{s.top_k} I{s.expert_inter}, batch 1, "
                         f"prompt {cfg.prompt_len} + {cfg.decode_steps} decode",
             "cache_slots": cfg.cache_slots, "cache_fraction": cfg.slots_per_layer / s.n_experts, "stride": cfg.stride,
-            "predictor": args.predictor, "decode_ids": args.decode, "chunk_bytes": args.chunk_mb << 20, "max_spec_decode": args.max_spec_decode,
-            "max_spec_prefill": args.max_spec_prefill, "low_cap_chunks": args.low_cap, "max_inflight": args.inflight,
+            "predictor": args.predictor, "decode_ids": args.decode, "chunk_bytes": args.chunk_kb << 10, "max_spec_decode": args.max_spec_decode,
+            "max_spec_prefill": args.max_spec_prefill, "low_cap_chunks": args.low_cap, "max_inflight": args.inflight, "fetch_ctas": args.fetch_ctas,
             "l2": "inputs larger than L2 (each request streams >> 126 MB of expert weights)"}
 
 
@@ -269,7 +269,7 @@ def run_ours(args, cfg, rank, world, dist):
         weights = synth.make_weights(cfg, predictor=pred_kind)
     wb = 4 if s.wdtype == 0 else 2
     Be = 3 * s.hidden * s.expert_inter * wb
-    h2d_gbs = B.promoe_measure_h2d(256 << 20, 2, 5)
+    h2d_gbs = B.promoe_bench_h2d(256 << 20, 2, 5)
     prompt = synth.make_prompt(cfg).tolist()
     decode_ids = synth.make_decode_ids(cfg).tolist()
     greedy = args.decode == "greedy"
@@ -282,10 +282,10 @@ def run_ours(args, cfg, rank, world, dist):
         run_request(rec_eng, cfg, prompt, decode_ids, greedy, record=inject)
         rec_eng.close()
     pmode = {"none": B.PRED_NONE, "trace": B.PRED_TRACE}.get(args.predictor, B.PRED_MLP)
-    eng = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_mb << 20,
+    eng = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_kb << 10,
                  predictor_mode=pmode, flags=flags,
                  max_inflight=args.inflight, max_spec_decode=args.max_spec_decode, max_spec_prefill=args.max_spec_prefill,
-                 low_cap_chunks=args.low_cap, device=f"cuda:{local}")
+                 low_cap_chunks=args.low_cap, fetch_ctas=args.fetch_ctas, device=f"cuda:{local}")
     for _ in range(args.warmup):
         run_request(eng, cfg, prompt, decode_ids, greedy, inject=inject)
     if dist is not None:
@@ -344,8 +344,8 @@ def run_ours(args, cfg, rank, world, dist):
     cs_dec, cs_pre = cache_stats("dec"), cache_stats("pre")
 
     # ---- dominant kernel, timed live with CUDA events on the launching stream (resident slots ≫ L2)
-    ms_gu, bytes_gu = B.promoe_kernel_time(eng.h, 0, 300)
-    ms_dn, bytes_dn = B.promoe_kernel_time(eng.h, 1, 300)
+    ms_gu, bytes_gu = B.promoe_bench_kernel_time(eng.h, 0, 300)
+    ms_dn, bytes_dn = B.promoe_bench_kernel_time(eng.h, 1, 300)
     ach = bytes_gu / (ms_gu * 1e-3) / 1e9
     kernel_roof = {"kernel": "ffn_gateup_gemv_kernel (A9 decode: gate/up SwiGLU GEMV over top_k resident experts)",
                    "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
@@ -367,7 +367,7 @@ def run_ours(args, cfg, rank, world, dist):
     if rank == 0 and not args.no_allhit:
         n_moe = s.n_layers - s.n_dense_layers
         full = ProMoE(weights, cache_slots=n_moe * s.n_experts, stride=cfg.stride, predictor_mode=B.PRED_NONE if args.predictor in ("none", "trace") else B.PRED_MLP,
-                      flags=flags, chunk_bytes=args.chunk_mb << 20, device=f"cuda:{local}")
+                      flags=flags, chunk_bytes=args.chunk_kb << 10, device=f"cuda:{local}")
         run_request(full, cfg, prompt, decode_ids, greedy)
         r = run_request(full, cfg, prompt, decode_ids, greedy)
         full.close()
@@ -392,7 +392,7 @@ def run_ours(args, cfg, rank, world, dist):
                 inj = []
                 run_request(rec, cfg, prompt, decode_ids, greedy, record=inj)
                 rec.close()
-            v = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_mb << 20,
+            v = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_kb << 10,
                        predictor_mode=pm, flags=flags, max_inflight=args.inflight, device=f"cuda:{local}")
             run_request(v, cfg, prompt, decode_ids, greedy, inject=inj)
             r = run_request(v, cfg, prompt, decode_ids, greedy, inject=inj)
@@ -449,7 +449,7 @@ def run_sweep(args):
     s = base.shape
     n_moe = s.n_layers - s.n_dense_layers
     Be = 3 * s.hidden * s.expert_inter * 2
-    h2d = B.promoe_measure_h2d(256 << 20, 2, 5)
+    h2d = B.promoe_bench_h2d(256 << 20, 2, 5)
     w0 = synth.make_weights(base, predictor="skip")
     decode_ids = synth.make_decode_ids(base).tolist()
     prompts = {n: synth.make_prompt(base, n).tolist() for n in (128, 2048)}
@@ -513,22 +513,6 @@ def run_sweep(args):
                       "compute_only_ms": {str(k): v for k, v in compute.items()}}), flush=True)
 
 
-def run_probe_fill():
-    """A7 design evidence: pinned H2D bandwidth of copy-engine copies (promoe_measure_h2d) against SM-issued fills
-    (promoe_measure_sm_fill: a kernel reads mapped host memory with 16-byte loads), per copy size and grid."""
-    import torch
-    from paper_2410_22134_b200 import binding as B
-    torch.cuda.set_device(0)
-    Be = 17301504                                     # one c2/c3 expert image
-    ce = {f"{b >> 20}MiB" if b % (1 << 20) == 0 else str(b): round(B.promoe_measure_h2d(b, 1, 5), 2)
-          for b in (1 << 20, 4 << 20, Be, 256 << 20)}
-    sm = []
-    for nbytes in (Be, 256 << 20):
-        for ctas, thr in ((1, 256), (1, 1024), (2, 1024), (4, 1024), (8, 1024), (32, 1024), (148, 1024), (296, 1024)):
-            sm.append({"bytes": nbytes, "ctas": ctas, "threads": thr, "gbs": round(B.promoe_measure_sm_fill(nbytes, ctas, thr, 5), 2)})
-    print(json.dumps({"probe": "h2d fill: copy engine vs SM-issued", "copy_engine_gbs": ce, "sm_fill": sm}))
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -540,18 +524,18 @@ def main():
                     help="skip: training-free MLP weights (default); none: reactive cache; trace: oracle-routing upper bound")
     ap.add_argument("--decode", default="random", choices=["random", "greedy"],
                     help="decode ids: seeded random (locality-neutral, default) or greedy argmax")
-    ap.add_argument("--chunk-mb", type=int, default=8, help="LOW (predicted) fills are issued in chunks of this size")
-    ap.add_argument("--inflight", type=int, default=1, help="LOW chunks kept in flight (bounded preemption delay, P:191)")
+    ap.add_argument("--chunk-kb", type=int, default=0, help="chunk size in KiB: granularity of the ready flags, of LOW copies and of preemption (0 = library default 256)")
+    ap.add_argument("--inflight", type=int, default=0, help="LOW chunks kept in flight (bounded preemption delay, P:191)")
     ap.add_argument("--max-spec-decode", type=int, default=1, help="allocations per PushPredicted in decode (0 = top_k as in Alg. 2, <0 = none); default 1: on a B200 one layer of\n                    compute hides about half an expert copy (profiles/r01_sweep_c2.md)")
     ap.add_argument("--max-spec-prefill", type=int, default=0, help="allocations per PushPredicted in prefill (<=0 = none)")
     ap.add_argument("--low-cap", type=int, default=0, help="a LOW fill stops after this many chunks (0 = no cap)")
+    ap.add_argument("--fetch-ctas", type=int, default=0, help="CTAs of the device-side fetch worker (0 = library default 2)")
     ap.add_argument("--tensor", type=int, default=1, help="prefill GEMMs on tcgen05 (bf16 weights)")
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--decode-steps", type=int, default=0)
     ap.add_argument("--ref-prompt", type=int, default=32, help="oracle sample: prompt tokens")
     ap.add_argument("--ref-decode", type=int, default=3, help="oracle sample: decode tokens")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] grid on the c3 shape (one JSON line per point)")
-    ap.add_argument("--probe-fill", action="store_true", help="copy-engine vs SM-issued H2D fills (one JSON line), then exit")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-allhit", action="store_true")
     ap.add_argument("--variants", type=int, default=1, help="also measure the reactive and oracle-routing context points")
@@ -559,9 +543,6 @@ def main():
 
     if args.sweep:
         run_sweep(args)
-        return
-    if args.probe_fill:
-        run_probe_fill()
         return
     import synth
     over = {}

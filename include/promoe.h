@@ -4,7 +4,8 @@
  * BASELINE.json `north_star`: promoe_create(model shape, cache_slots, stride), promoe_load_experts(host
  * ptrs), promoe_prefill, promoe_decode, promoe_stats.  The remaining calls hand over the always-resident
  * non-expert parameters ("non-expert parameters are always kept on the GPU"), expose traces for
- * parity tests, and micro-entry points for single hot-path steps.
+ * parity tests, and micro-entry points for single hot-path steps.  Measurement hooks used only by bench.py live in
+ * include/promoe_bench.h, not here.
  *
  * Conventions
  *  - every call returns 0 (PROMOE_OK) or a negative PROMOE_E* code; no exception or abort crosses the ABI;
@@ -67,16 +68,20 @@ typedef struct {
 #define PROMOE_F_TRACE 8     /* record routing / permutation / cache traces for promoe_get_trace */
 #define PROMOE_F_NOFUSE 32  /* decode with the unfused per-op kernels (19 launches per layer) instead of the fused 7 */
 #define PROMOE_F_TENSOR 16   /* prefill GEMMs on tcgen05 tensor cores (bf16 weights only); else SIMT fp32 */
+#define PROMOE_F_UNCHUNKED 64 /* ablation (Fig. 12 "+chunk" off): an expert image is copied all or nothing — one LOW
+                                 copy per predicted expert, and a gate that finds a partial image fetches it again from byte 0 */
 
 typedef struct {
   int32_t cache_slots;     /* TOTAL slots; per MoE layer = cache_slots / n_moe_layers (must divide), G14 */
   int32_t stride;          /* predictor at MoE layer m targets MoE layer m+stride; >= 1 */
-  uint64_t chunk_bytes;    /* chunk size: granularity of the per-chunk ready flags and of the LOW (predicted)
-                              copies; a HIGH (precise) fill covers high_group chunks per copy.  0 = default 4 MiB
-                              (profiles/r01_fill_protocol.md); multiple of 256 */
+  uint64_t chunk_bytes;    /* chunk size: granularity of the per-chunk ready flags, of the LOW (predicted) copies and
+                              of preemption.  0 = default 256 KiB (decode fetches on the device, where a chunk costs no host
+                              call: DESIGN.md §6); multiple of 256.  Prefill (copy engines): a HIGH (precise) fill covers
+                              high_group chunks per copy operation */
   int32_t predictor_mode;
   int32_t flags;
-  int32_t max_inflight;    /* LOW chunks kept in flight on the copy stream (P:191 bounded preemption delay); 0 = default 2 */
+  int32_t max_inflight;    /* prefill / unfused decode (copy engines): LOW chunks kept in flight on the copy stream (P:191 bounded
+                              preemption delay); 0 = default 2.  The fused decode step has one LOW chunk per fetch CTA in flight */
   int32_t high_group;      /* chunks per HIGH (precise) copy operation; 0 = the whole remaining fill in ONE copy (measured
                               fastest); ready flags are written behind every operation */
   int32_t max_spec_decode; /* experts of one PushPredicted that may ALLOCATE a slot in a decode step (listed order = most
@@ -85,7 +90,9 @@ typedef struct {
                                an allocation only swaps one needed expert for another (G7) */
   int32_t low_cap_chunks;  /* a LOW (predicted) fill stops after this many chunks; the rest is fetched only if the gate needs
                               the expert (then as HIGH).  0 = no cap.  Physical only: never changes a trace or an output */
-  int32_t reserved;
+  int32_t fetch_ctas;      /* CTAs (one warp each, TMA bulk copies) of the device-side fetch worker of the fused decode step;
+                              0 = default 4 (three reach the SM-side link limit at any chunk size: profiles/r02_fill_probe.md).
+                              Physical only */
   void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
 } promoe_opts_t;
 
@@ -122,6 +129,13 @@ typedef struct {
   uint64_t fetched_at_gate, fetched_at_gate_of;  /* FetchRate numerator / denominator */
   uint64_t registered_host_bytes; /* expert host bytes the library had to cudaHostRegister */
   uint64_t kernel_launches;     /* kernels launched by the library in this process so far (all handles) */
+  /* byte-accurate (physical) view — the logical counters above follow the slot TABLE, these follow the BYTES */
+  uint64_t high_bytes, low_bytes;     /* bytes moved by HIGH (precise) / LOW (predicted) copies; sum = h2d_bytes */
+  uint64_t low_bytes_useful;          /* LOW bytes of fills whose expert was needed at its gate (class B) */
+  uint64_t hits_landed;               /* class A / B accesses whose image had completely landed when the gate was processed */
+  uint64_t owed_bytes_at_gate;        /* bytes the HIGH fills still had to move for the needed experts, summed over gates */
+  uint64_t landed_chunks_at_gate, landed_chunks_of;   /* class-B experts: chunks landed at the gate / chunks per image
+                                         (the partial-fetch form of FetchRate) */
   double copy_busy_ms;          /* copy-stream busy time, from per-chunk events */
   double step_ms;               /* sum of step times (compute-stream events) */
   double last_step_ms;
@@ -169,33 +183,8 @@ PROMOE_API int promoe_reset(promoe_t* h);   /* clears KV cache, cache state (re-
 /* Current logical slot table of MoE layer m: slot_expert_out = host ptr to C int32 (-1 = empty). */
 PROMOE_API int promoe_get_slots(promoe_t* h, int32_t moe_layer, int32_t* slot_expert_out);
 
-/* Measured pinned host->device bandwidth (GB/s) for `bytes`-sized copies at queue depth `depth`
- * (chunk size is chosen from this curve).  Allocates and frees its own buffers. */
-PROMOE_API int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out);
-
-/* Measured bandwidth (GB/s) of an SM-ISSUED fill: a kernel of `ctas` x `threads` reads `bytes` of pinned, mapped
- * host memory with 16-byte loads and stores them into device memory (no copy engine, no host in the loop) — the
- * device-side alternative to the copy-engine fills of A7 (Alg. 1 l.6-10 copies chunk by chunk; who issues
- * the copy is left to the implementation).  DESIGN.md section 7 compares it with promoe_measure_h2d.  Allocates and
- * frees its own buffers; the copied bytes are verified (PROMOE_ECUDA on mismatch).  bytes: multiple of 64; ctas >= 1;
- * threads: multiple of 32 in [32, 1024]; best of `reps` timed launches after one warm-up. */
-PROMOE_API int promoe_measure_sm_fill(size_t bytes, int32_t ctas, int32_t threads, int32_t reps, double* gbs_out);
-
-/* Measured cost of the fill protocol itself:
- * n_fills expert images of expert_bytes each, pinned host -> device, back to back on one stream, every fill bracketed
- * by events as in the engine.  mode 0: one copy + one 32-bit stream write per chunk; 1: ONE copy per fill, then one
- * 32-bit stream write per chunk; 2: one copy per fill + ONE small copy for all its flags; 3: one copy, no flags;
- * 4: one copy + one 4-byte copy per chunk.  Result: sustained GB/s over the whole sequence. */
-PROMOE_API int promoe_measure_fill(size_t expert_bytes, size_t chunk_bytes, int32_t mode, int32_t n_fills, double* gbs_out);
-
-/* Live kernel timing for bench.py's roofline: runs `reps` launches of one hot kernel of the decode step on the
- * compute stream, bracketed by CUDA events, over RESIDENT slots rotating through all layers (working set = the
- * whole slot region, far larger than L2).  which: 0 = A9 gate/up SwiGLU GEMV over top_k experts, 1 = A9 down GEMV
- * over top_k experts.  Outputs the average launch duration and the algorithmic weight bytes one launch streams. */
-PROMOE_API int promoe_kernel_time(promoe_t* h, int32_t which, int32_t reps, double* avg_ms_out, double* bytes_per_launch_out);
-
 /* Micro entry points: single hot-path steps on caller-provided DEVICE buffers (used by kernel-level parity
- * tests and bench.py's per-kernel roofline).  stream = cudaStream_t or NULL (default stream).
+ * tests).  stream = cudaStream_t or NULL (default stream).
  * All are asynchronous on `stream`. */
 /* y[T,N] = x[T,K] . W[N,K]^T ; x,y fp32; W wdtype (0 fp32 / 1 bf16). path: 0 auto, 1 gemv, 2 simt gemm, 3 tcgen05 */
 PROMOE_API int promoe_op_linear(const float* x, const void* w, float* y, int32_t T, int32_t N, int32_t K, int32_t wdtype,
@@ -210,8 +199,7 @@ PROMOE_API int promoe_op_permute(const int32_t* sel, int32_t T, int32_t k, int32
 
 /* expert FFN row A9 on one resident weight set: y[T,H] = Wd.(silu(Wg.x) * (Wu.x)); x [T,H], act_ws [T,I] scratch,
  * prob_ws >= 64 bytes of device scratch (problem record).  path: 0 auto, 1 HBM-streaming GEMV (T == 1),
- * 2 SIMT grouped GEMM, 3 tcgen05 grouped GEMM (bf16 weights), 4 TMA-fed (cp.async.bulk) gate/up GEMV (T == 1, bf16,
- * H <= 2048). */
+ * 2 SIMT grouped GEMM, 3 tcgen05 grouped GEMM (bf16 weights). */
 PROMOE_API int promoe_op_expert_ffn(const float* x, const void* wg, const void* wu, const void* wd, float* act_ws,
                                     float* y, void* prob_ws, int32_t T, int32_t H, int32_t I, int32_t wdtype,
                                     int32_t path, int32_t reserved, void* stream);

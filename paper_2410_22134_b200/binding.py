@@ -23,9 +23,10 @@ TRACE_SEL, TRACE_GATES, TRACE_MARGIN, TRACE_PERM, TRACE_PRECISE, TRACE_PRED, TRA
 EXPORTS = [
     "promoe_create", "promoe_destroy", "promoe_last_error", "promoe_load_dense", "promoe_load_experts",
     "promoe_prefill", "promoe_decode", "promoe_set_prediction_trace", "promoe_stats", "promoe_get_trace",
-    "promoe_reset", "promoe_get_slots", "promoe_measure_h2d", "promoe_op_linear", "promoe_op_route",
-    "promoe_op_permute", "promoe_op_expert_ffn", "promoe_kernel_time", "promoe_measure_fill", "promoe_measure_sm_fill",
+    "promoe_reset", "promoe_get_slots", "promoe_op_linear", "promoe_op_route",
+    "promoe_op_permute", "promoe_op_expert_ffn",
 ]
+BENCH_EXPORTS = ["promoe_bench_h2d", "promoe_bench_kernel_time"]   # include/promoe_bench.h (bench.py only)
 
 
 class promoe_shape_t(C.Structure):
@@ -39,7 +40,7 @@ class promoe_opts_t(C.Structure):
     _fields_ = [("cache_slots", C.c_int32), ("stride", C.c_int32), ("chunk_bytes", C.c_uint64),
                 ("predictor_mode", C.c_int32), ("flags", C.c_int32), ("max_inflight", C.c_int32),
                 ("high_group", C.c_int32), ("max_spec_decode", C.c_int32), ("max_spec_prefill", C.c_int32),
-                ("low_cap_chunks", C.c_int32), ("reserved", C.c_int32),
+                ("low_cap_chunks", C.c_int32), ("fetch_ctas", C.c_int32),
                 ("compute_stream", C.c_void_p)]
 
 
@@ -55,7 +56,8 @@ class promoe_stats_t(C.Structure):
         "steps", "tokens", "accesses", "hits_resident", "hits_prefetch", "misses", "evictions", "predicted",
         "predicted_correct", "pred_allocs", "need_experts", "chunks_issued", "chunks_cancelled", "chunks_high",
         "chunks_low", "h2d_bytes", "fetched_at_gate", "fetched_at_gate_of", "registered_host_bytes",
-        "kernel_launches")] + [
+        "kernel_launches", "high_bytes", "low_bytes", "low_bytes_useful", "hits_landed", "owed_bytes_at_gate",
+        "landed_chunks_at_gate", "landed_chunks_of")] + [
         ("copy_busy_ms", C.c_double), ("step_ms", C.c_double), ("last_step_ms", C.c_double),
         ("timeouts", C.c_int32), ("reserved", C.c_int32)]
 
@@ -93,15 +95,13 @@ def lib() -> C.CDLL:
     L.promoe_get_trace.argtypes = [vp, C.c_int, C.POINTER(vp), C.POINTER(sz)]
     L.promoe_reset.argtypes = [vp]
     L.promoe_get_slots.argtypes = [vp, i32, vp]
-    L.promoe_measure_h2d.argtypes = [sz, i32, i32, C.POINTER(C.c_double)]
+    L.promoe_bench_h2d.argtypes = [sz, i32, i32, C.POINTER(C.c_double)]
     L.promoe_op_linear.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp]
     L.promoe_op_route.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_permute.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_expert_ffn.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
-    L.promoe_measure_fill.argtypes = [sz, sz, i32, i32, C.POINTER(C.c_double)]
-    L.promoe_measure_sm_fill.argtypes = [sz, i32, i32, i32, C.POINTER(C.c_double)]
-    L.promoe_kernel_time.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
-    for n in EXPORTS:
+    L.promoe_bench_kernel_time.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    for n in EXPORTS + BENCH_EXPORTS:
         f = getattr(L, n)
         if n not in ("promoe_destroy", "promoe_last_error"):
             f.restype = C.c_int
@@ -172,27 +172,14 @@ def promoe_get_slots(h, moe_layer: int, n_slots: int) -> np.ndarray:
     return out
 
 
-def promoe_measure_h2d(nbytes: int, depth: int = 2, reps: int = 5) -> float:
+def promoe_bench_h2d(nbytes: int, depth: int = 2, reps: int = 5) -> float:
     g = C.c_double()
-    _check(lib().promoe_measure_h2d(nbytes, depth, reps, C.byref(g)))
+    _check(lib().promoe_bench_h2d(nbytes, depth, reps, C.byref(g)))
     return g.value
 
 
-def promoe_kernel_time(h, which: int, reps: int = 200):
+def promoe_bench_kernel_time(h, which: int, reps: int = 200):
     """(average launch ms, algorithmic bytes per launch) of decode kernel `which` over resident slots."""
     ms, nb = C.c_double(), C.c_double()
-    _check(lib().promoe_kernel_time(h, which, reps, C.byref(ms), C.byref(nb)), h)
+    _check(lib().promoe_bench_kernel_time(h, which, reps, C.byref(ms), C.byref(nb)), h)
     return ms.value, nb.value
-
-
-def promoe_measure_sm_fill(nbytes: int, ctas: int, threads: int = 1024, reps: int = 3) -> float:
-    """GB/s of an SM-issued fill (kernel reads pinned mapped host memory); the copied bytes are verified."""
-    g = C.c_double()
-    _check(lib().promoe_measure_sm_fill(nbytes, ctas, threads, reps, C.byref(g)))
-    return g.value
-
-
-def promoe_measure_fill(expert_bytes: int, chunk_bytes: int, mode: int, n_fills: int = 32) -> float:
-    g = C.c_double()
-    _check(lib().promoe_measure_fill(expert_bytes, chunk_bytes, mode, n_fills, C.byref(g)))
-    return g.value

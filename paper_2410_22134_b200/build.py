@@ -18,9 +18,6 @@ LIB = os.path.join(HERE, "libpromoe.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
          "-Xcompiler", "-fvisibility=hidden"]
-# measurement builds only (e.g. PROMOE_EXTRA_NVCC_FLAGS=-DPROMOE_KNOCKOUT, see step.cu); always combine with --force,
-# and rebuild with --force and the variable unset afterwards
-FLAGS += os.environ.get("PROMOE_EXTRA_NVCC_FLAGS", "").split()
 
 
 def _sources():

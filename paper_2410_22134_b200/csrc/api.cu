@@ -155,11 +155,8 @@ extern "C" int promoe_op_expert_ffn(const float* x, const void* wg, const void* 
   if (cudaMemcpyAsync(prob_ws, &pb, sizeof(pb), cudaMemcpyHostToDevice, st) != cudaSuccess) return PROMOE_ECUDA;
   const FfnProblem* dp = (const FfnProblem*)prob_ws;
   if (path == 0) path = (T == 1) ? 1 : 2;
-  if (path == 1 || path == 4) {     // 4 = TMA-fed gate/up GEMV (bf16, H <= 2048), else register-fed
+  if (path == 1) {
     if (T != 1) return PROMOE_EINVAL;
-    if (path == 4) {
-      if (wdtype != 1 || !launch_ffn_gateup_gemv_tma(x, dp, 1, I, H, act_ws, I, (size_t)1 << 20, nullptr, st)) return PROMOE_EINVAL;
-    } else
     launch_ffn_gateup_gemv(x, dp, 1, I, H, act_ws, I, wdtype, (size_t)1 << 20, nullptr, st);
     launch_ffn_down_gemv(act_ws, I, dp, 1, I, H, y, wdtype, (size_t)1 << 20, nullptr, st);
   } else if (path == 2) {
@@ -189,39 +186,3 @@ extern "C" int promoe_op_expert_ffn(const float* x, const void* wg, const void* 
   return launch_status();
 }
 
-extern "C" int promoe_kernel_time(promoe_t* h, int32_t which, int32_t reps, double* avg_ms_out, double* bytes_out) {
-  if (!h || reps < 1 || !avg_ms_out || !bytes_out || (which != 0 && which != 1)) return PROMOE_EINVAL;
-  if (!h->experts_loaded) { h->err = "kernel_time before load_experts"; return PROMOE_ESTATE; }
-  const promoe_shape_t& s = h->s;
-  const int k = s.top_k, H = s.hidden, I = s.expert_inter, Lm = h->Lm, C = h->C;
-  const size_t hi = (size_t)H * I * h->wb;
-  std::vector<FfnProblem> pb((size_t)Lm * k);
-  for (int m = 0; m < Lm; ++m)
-    for (int i = 0; i < k; ++i) {
-      const uint8_t* img = h->slots + ((size_t)m * C + (i % C)) * h->Be;
-      FfnProblem& p = pb[(size_t)m * k + i];
-      p.wg = img; p.wu = img + hi; p.wd = img + 2 * hi; p.flags = nullptr; p.gen = 0; p.inter = I; p.row0 = i; p.nrows = 1;
-      p.expert = -1; p.pad = 0;
-    }
-  FfnProblem* dp = nullptr;
-  CKA(cudaMalloc((void**)&dp, pb.size() * sizeof(FfnProblem)));
-  CKA(cudaMemcpy(dp, pb.data(), pb.size() * sizeof(FfnProblem), cudaMemcpyHostToDevice));
-  cudaEvent_t a, b;
-  CKA(cudaEventCreate(&a)); CKA(cudaEventCreate(&b));
-  auto launch = [&](int r) {
-    const FfnProblem* q = dp + (size_t)(r % Lm) * k;
-    if (which == 0) launch_ffn_gateup_gemv(h->u, q, k, I, H, h->act, I, s.wdtype, h->chunk_bytes, h->err_dev, h->cs);
-    else launch_ffn_down_gemv(h->act, I, q, k, I, H, h->yexp, s.wdtype, h->chunk_bytes, h->err_dev, h->cs);
-  };
-  for (int r = 0; r < 3; ++r) launch(r);
-  CKA(cudaEventRecord(a, h->cs));
-  for (int r = 0; r < reps; ++r) launch(r + 3);
-  CKA(cudaEventRecord(b, h->cs));
-  CKA(cudaStreamSynchronize(h->cs));
-  float ms = 0.f;
-  CKA(cudaEventElapsedTime(&ms, a, b));
-  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(dp);
-  *avg_ms_out = (double)ms / reps;
-  *bytes_out = (double)k * (which == 0 ? 2.0 : 1.0) * (double)hi;
-  return PROMOE_OK;
-}

@@ -14,7 +14,15 @@ constexpr int kWarp = 32;
 // in front of it has completed and flushed (so at most the prologue overlaps — no data hazard is possible).
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_enter() { pdl_trigger(); pdl_wait(); }
+// Where the trigger sits decides how long the dependent's CTAs sit resident (at griddepcontrol.wait) beside the running
+// kernel.  At the top of the kernel the whole run-ahead queue of the decode step cascades onto the SMs (every kernel
+// triggers its successor as soon as it is resident) and takes registers and thread slots from the one kernel that is
+// actually running; after the main loop only the NEXT kernel overlaps, with the tail of this one.
+#ifndef PMK_PDL_LATE
+#define PMK_PDL_LATE 1
+#endif
+__device__ __forceinline__ void pdl_enter() { if (!PMK_PDL_LATE) pdl_trigger(); pdl_wait(); }
+__device__ __forceinline__ void pdl_done() { if (PMK_PDL_LATE) pdl_trigger(); }
 extern bool g_use_pdl;   // PROMOE_PDL=0 disables (A/B measurements)
 template <typename... KArgs, typename... Args>
 inline void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
@@ -25,6 +33,14 @@ inline void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t sme
   at[0].val.programmaticStreamSerializationAllowed = g_use_pdl ? 1 : 0;
   cfg.attrs = at; cfg.numAttrs = 1;
   cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
+// force the (lazy) load of one kernel; see preload_* in every kernels_*.cu
+inline void preload_fn(const void* f) { cudaFuncAttributes a; (void)cudaFuncGetAttributes(&a, f); }
+void preload_dense(); void preload_attn(); void preload_route(); void preload_slot(); void preload_decode();
+void preload_ffn(); void preload_tc(); void preload_fetch();
+inline void preload_all() {
+  preload_dense(); preload_attn(); preload_route(); preload_slot(); preload_decode(); preload_ffn(); preload_tc(); preload_fetch();
 }
 
 // number of kernels launched by this library (host-side counter, bumped by every launch_* wrapper; promoe_stats)

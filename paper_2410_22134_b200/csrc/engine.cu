@@ -16,7 +16,7 @@ using namespace pmk;
 static std::string g_create_err;
 namespace pmk {
 unsigned long long g_launches = 0;
-bool g_use_pdl = [] { const char* e = getenv("PROMOE_PDL"); return !(e && e[0] == '0'); }();
+bool g_use_pdl = true;
 }
 
 #define CK(call)                                                                                   \
@@ -38,6 +38,7 @@ static cudaError_t dalloc(T** p, size_t n) {
 int promoe_init_cache_state(promoe_t* h, bool copy_warm);  // below
 int ce_retire(promoe_t* h, bool all);
 
+
 extern "C" const char* promoe_last_error(const promoe_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 
 extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, promoe_t** out) {
@@ -58,13 +59,26 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   if (op->stride < 1) return bad("stride must be >= 1");
   if ((size_t)s.max_seq * s.top_k > 16384 * 4) return bad("max_seq*top_k too large for the single-CTA permutation");
 
+  preload_all();      // no kernel of this library may be loaded lazily behind a spinning kernel
+  (void)cudaGetLastError();
   promoe_t* h = new promoe();
   h->s = s; h->o = *op; h->Lm = Lm; h->C = C;
   h->wb = s.wdtype == 0 ? 4 : 2;
   h->Be = (size_t)3 * s.hidden * s.expert_inter * h->wb;
-  h->chunk_bytes = op->chunk_bytes ? (size_t)op->chunk_bytes : ((size_t)4 << 20);
+  h->chunk_bytes = op->chunk_bytes ? (size_t)op->chunk_bytes : ((size_t)256 << 10);
   if (h->chunk_bytes % 256) { delete h; return bad("chunk_bytes must be a multiple of 256"); }
   h->n_chunks = (int)((h->Be + h->chunk_bytes - 1) / h->chunk_bytes);
+  // the pinned ring the flag copies read from must hold the words of every fill that can be in flight (one layer's
+  // HIGH fills) at least twice over
+  if (h->n_chunks > kMaxChunks || (size_t)h->n_chunks * C * 2 > kFlagSrcRing) { delete h; return bad("chunk_bytes too small for this expert size (too many chunks per image)"); }
+  // the fused down+combine kernel cuts (top_k + shared) dot products into pieces of 2048 elements: at most 192 pieces
+  {
+    const int pieces = s.top_k * ((s.expert_inter + 2047) / 2048) + (std::max(s.n_shared_inter, s.dense_inter) + 2047) / 2048;
+    if (pieces > 192) { delete h; return bad("top_k * ceil(expert_inter / 2048) + ceil(shared_inter / 2048) must be <= 192"); }
+  }
+  h->unchunked = (op->flags & PROMOE_F_UNCHUNKED) != 0;
+  cudaGetDevice(&h->dev);
+  h->fetch_ctas = op->fetch_ctas > 0 ? std::min(op->fetch_ctas, 16) : 4;
   h->max_inflight = op->max_inflight > 0 ? op->max_inflight : 2;
   h->high_group = op->high_group > 0 ? op->high_group : 0;
   h->low_cap = op->low_cap_chunks > 0 ? op->low_cap_chunks : 0;
@@ -80,6 +94,7 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     else { CK(cudaStreamCreateWithFlags(&h->cs, cudaStreamNonBlocking)); h->own_cs = true; }
     CK(cudaStreamCreateWithFlags(&h->ps, cudaStreamNonBlocking));
     CK(cudaStreamCreateWithFlags(&h->cs2, cudaStreamNonBlocking));
+    { int lo = 0, hi = 0; CK(cudaDeviceGetStreamPriorityRange(&lo, &hi)); CK(cudaStreamCreateWithPriority(&h->fs, cudaStreamNonBlocking, hi)); }
     CK(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming)); CK(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
     CK(dalloc(&h->x, (size_t)T * H)); CK(dalloc(&h->u1, (size_t)T * H)); CK(dalloc(&h->u, (size_t)T * H));
     CK(dalloc(&h->qkv, (size_t)T * h->qkv_w)); CK(dalloc(&h->attn, (size_t)T * s.n_q_heads * s.head_dim));
@@ -128,13 +143,17 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->tbl.stamp, (size_t)Lm * C)); CK(dalloc(&h->tbl.gen, (size_t)Lm * C));
     CK(dalloc(&h->tbl.origin, (size_t)Lm * C)); CK(dalloc(&h->tbl.clock, (size_t)1));
     h->tbl.Lm = Lm; h->tbl.C = C; h->tbl.E = E;
+    CK(dalloc(&h->claims, (size_t)Lm * C * h->n_chunks)); CK(dalloc(&h->complete, (size_t)Lm * C)); CK(dalloc(&h->alive, (size_t)1));
+    CK(dalloc(&h->fetch_ctr, (size_t)kFetchCounters)); CK(dalloc(&h->src_dev, (size_t)Lm * E));
+    CK(cudaMalloc((void**)&h->cmd_fetch, sizeof(LayerCmd) * Lm)); CK(cudaMemset(h->cmd_fetch, 0, sizeof(LayerCmd) * Lm));
+    CK(cudaHostAlloc((void**)&h->fetch_ctr_pin, sizeof(unsigned long long) * kFetchCounters, cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->cmd_host, sizeof(LayerCmd) * Lm, cudaHostAllocMapped));
     memset((void*)h->cmd_host, 0, sizeof(LayerCmd) * Lm);
     CK(cudaHostGetDevicePointer((void**)&h->cmd_dev, (void*)h->cmd_host, 0));
     CK(cudaHostAlloc((void**)&h->logits_pin, sizeof(float) * (size_t)s.vocab, cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->ids_pin, sizeof(int32_t) * (size_t)T, cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->err_pin, sizeof(int), cudaHostAllocDefault));
-    CK(cudaHostAlloc((void**)&h->flagsrc_host, sizeof(uint32_t) * 65536, cudaHostAllocDefault));
+    CK(cudaHostAlloc((void**)&h->flagsrc_host, sizeof(uint32_t) * kFlagSrcRing, cudaHostAllocDefault));
     h->phys.resize((size_t)Lm * C);
     for (auto& p : h->phys) CK(cudaEventCreateWithFlags(&p.done, cudaEventDisableTiming));
     const int ring = 8192;
@@ -161,7 +180,8 @@ extern "C" void promoe_destroy(promoe_t* h) {
                   h->sgate, h->attn_ws, h->xf, h->logits, h->kcache, h->vcache, h->cos_t, h->sin_t, h->ids, h->sel,
                   h->count, h->offset, h->perm, h->inv, h->gates, h->margin, h->z, h->pred_list, h->trace_precise,
                   h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->attn_cnt, h->slots, h->flags,
-                  h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock};
+                  h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock,
+                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch};
   for (void* b : bufs) if (b) cudaFree(b);
   if (h->xsA) cudaFree(h->xsA);
   if (h->xsG) cudaFree(h->xsG);
@@ -180,6 +200,8 @@ extern "C" void promoe_destroy(promoe_t* h) {
   if (h->step_end) cudaEventDestroy(h->step_end);
   if (h->ps) cudaStreamDestroy(h->ps);
   if (h->cs2) cudaStreamDestroy(h->cs2);
+  if (h->fs) cudaStreamDestroy(h->fs);
+  if (h->fetch_ctr_pin) cudaFreeHost(h->fetch_ctr_pin);
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
   if (h->ev_join) cudaEventDestroy(h->ev_join);
   if (h->own_cs && h->cs) cudaStreamDestroy(h->cs);
@@ -234,7 +256,11 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
       for (int i = 0; i < C; ++i) { se[(size_t)m * C + i] = i; es[(size_t)m * E + i] = i; stamp[(size_t)m * C + i] = (unsigned long long)m * C + i + 1; }
     clock = (unsigned long long)Lm * C;
   }
-  CK(cudaStreamSynchronize(h->cs)); CK(cudaStreamSynchronize(h->ps)); CK(cudaStreamSynchronize(h->cs2));
+  CK(cudaStreamSynchronize(h->cs)); CK(cudaStreamSynchronize(h->ps)); CK(cudaStreamSynchronize(h->cs2)); CK(cudaStreamSynchronize(h->fs));
+  CK(cudaMemset(h->claims, 0, (size_t)Lm * C * h->n_chunks * 4));
+  CK(cudaMemset(h->complete, 0, (size_t)Lm * C * 4));
+  CK(cudaMemset(h->cmd_fetch, 0, sizeof(LayerCmd) * Lm));
+  h->phys_dirty = false;
   CK(cudaMemcpy(h->tbl.slot_expert, se.data(), se.size() * 4, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(h->tbl.expert_slot, es.data(), es.size() * 4, cudaMemcpyHostToDevice));
   CK(cudaMemcpy(h->tbl.stamp, stamp.data(), stamp.size() * 8, cudaMemcpyHostToDevice));
@@ -251,7 +277,9 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
   for (size_t i = 0; i < h->phys.size(); ++i) {
     SlotPhys& p = h->phys[i];
     p.gen = 0; p.expert = se[i]; p.issued = warm ? h->n_chunks : 0; p.flagged = p.issued; p.fill_seq = 0; p.done_valid = false;
+    p.low_chunks = 0; p.low_bytes = 0; p.low_ring.clear();
   }
+
   if (warm && copy_warm && h->experts_loaded)
     for (int m = 0; m < Lm; ++m)
       for (int i = 0; i < C; ++i)
@@ -277,16 +305,29 @@ extern "C" int promoe_load_experts(promoe_t* h, const void* const* host_ptrs, si
     return at.type == cudaMemoryTypeUnregistered;
   };
   if (contiguous && unregistered(host_ptrs[0])) {      // one mapping (e.g. a shared-memory file shared by all ranks)
-    CK(cudaHostRegister((void*)host_ptrs[0], n * expert_bytes, cudaHostRegisterPortable));
+    CK(cudaHostRegister((void*)host_ptrs[0], n * expert_bytes, cudaHostRegisterPortable | cudaHostRegisterMapped));
     h->registered.push_back((void*)host_ptrs[0]);
     h->st.registered_host_bytes += n * expert_bytes;
   } else {
     for (size_t i = 0; i < n; ++i)
       if (unregistered(host_ptrs[i])) {
-        CK(cudaHostRegister((void*)host_ptrs[i], expert_bytes, cudaHostRegisterDefault));
+        CK(cudaHostRegister((void*)host_ptrs[i], expert_bytes, cudaHostRegisterMapped));
         h->registered.push_back((void*)host_ptrs[i]);
         h->st.registered_host_bytes += expert_bytes;
       }
+  }
+  // the device-side fetch worker reads the images through their device-visible addresses (pinned host memory is mapped
+  // into the unified address space); TMA bulk copies need 16-byte alignment
+  {
+    std::vector<unsigned long long> sd(n);
+    for (size_t i = 0; i < n; ++i) {
+      void* dp = nullptr;
+      cudaError_t e = cudaHostGetDevicePointer(&dp, (void*)host_ptrs[i], 0);
+      if (e != cudaSuccess || !dp) { (void)cudaGetLastError(); h->err = "load_experts: expert image is not device-accessible pinned host memory"; return PROMOE_EINVAL; }
+      if (((uintptr_t)dp & 15) || ((uintptr_t)host_ptrs[i] & 15)) { h->err = "load_experts: expert images must be 16-byte aligned"; return PROMOE_EINVAL; }
+      sd[i] = (unsigned long long)(uintptr_t)dp;
+    }
+    CK(cudaMemcpy(h->src_dev, sd.data(), n * 8, cudaMemcpyHostToDevice));
   }
   h->experts_loaded = true;
   return promoe_init_cache_state(h, true);
@@ -316,146 +357,3 @@ extern "C" int promoe_stats(promoe_t* h, promoe_stats_t* out) {
   return PROMOE_OK;
 }
 
-// Pinned H2D bandwidth for `bytes`-sized copies with `depth` copies kept in flight (chunk size choice).
-extern "C" int promoe_measure_h2d(size_t bytes, int32_t depth, int32_t reps, double* gbs_out) {
-  if (!bytes || depth < 1 || reps < 1 || !gbs_out) return PROMOE_EINVAL;
-  void *hbuf = nullptr, *dbuf = nullptr;
-  cudaStream_t st = nullptr;
-  cudaEvent_t a = nullptr, b = nullptr;
-  const size_t total = bytes * (size_t)depth;
-  int rc = PROMOE_ECUDA;
-  if (cudaHostAlloc(&hbuf, total, cudaHostAllocDefault) == cudaSuccess && cudaMalloc(&dbuf, total) == cudaSuccess &&
-      cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess && cudaEventCreate(&a) == cudaSuccess &&
-      cudaEventCreate(&b) == cudaSuccess) {
-    memset(hbuf, 1, total);
-    double best = 0.0;
-    for (int r = 0; r < reps + 1; ++r) {
-      cudaEventRecord(a, st);
-      for (int i = 0; i < depth; ++i)
-        cudaMemcpyAsync((char*)dbuf + (size_t)i * bytes, (char*)hbuf + (size_t)i * bytes, bytes, cudaMemcpyHostToDevice, st);
-      cudaEventRecord(b, st);
-      if (cudaStreamSynchronize(st) != cudaSuccess) break;
-      float ms = 0.f;
-      cudaEventElapsedTime(&ms, a, b);
-      if (r > 0 && ms > 0.f) best = std::max(best, (double)total / (ms * 1e6));
-    }
-    *gbs_out = best;
-    rc = best > 0.0 ? PROMOE_OK : PROMOE_ECUDA;
-  }
-  if (a) cudaEventDestroy(a);
-  if (b) cudaEventDestroy(b);
-  if (st) cudaStreamDestroy(st);
-  if (dbuf) cudaFree(dbuf);
-  if (hbuf) cudaFreeHost(hbuf);
-  return rc;
-}
-
-// SM-issued fill (pinned mapped host → device, 16-byte loads, 4 in flight per thread): device-side alternative to the
-// copy-engine fills, measured for DESIGN.md section 7.
-__global__ void sm_fill_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, size_t n16) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t st = (size_t)gridDim.x * blockDim.x;
-  for (; i + 3 * st < n16; i += 4 * st) {
-    const uint4 a = __ldcs(src + i), b = __ldcs(src + i + st), c = __ldcs(src + i + 2 * st), d = __ldcs(src + i + 3 * st);
-    dst[i] = a; dst[i + st] = b; dst[i + 2 * st] = c; dst[i + 3 * st] = d;
-  }
-  for (; i < n16; i += st) dst[i] = __ldcs(src + i);
-}
-extern "C" int promoe_measure_sm_fill(size_t bytes, int32_t ctas, int32_t threads, int32_t reps, double* gbs_out) {
-  if (!bytes || bytes % 64 || ctas < 1 || threads < 32 || threads > 1024 || threads % 32 || reps < 1 || !gbs_out) return PROMOE_EINVAL;
-  void *hbuf = nullptr, *dbuf = nullptr, *hdev = nullptr;
-  cudaStream_t st = nullptr;
-  cudaEvent_t a = nullptr, b = nullptr;
-  int rc = PROMOE_ECUDA;
-  if (cudaHostAlloc(&hbuf, bytes, cudaHostAllocMapped) == cudaSuccess && cudaHostGetDevicePointer(&hdev, hbuf, 0) == cudaSuccess &&
-      cudaMalloc(&dbuf, bytes) == cudaSuccess && cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess &&
-      cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
-    uint32_t* hw = (uint32_t*)hbuf;
-    for (size_t i = 0; i < bytes / 4; ++i) hw[i] = (uint32_t)i * 2654435761u + 12345u;
-    cudaMemsetAsync(dbuf, 0, bytes, st);
-    double best = 0.0;
-    for (int r = 0; r < reps + 1; ++r) {
-      cudaEventRecord(a, st);
-      sm_fill_kernel<<<ctas, threads, 0, st>>>((const uint4*)hdev, (uint4*)dbuf, bytes / 16);
-      cudaEventRecord(b, st);
-      if (cudaStreamSynchronize(st) != cudaSuccess) break;
-      float ms = 0.f;
-      cudaEventElapsedTime(&ms, a, b);
-      if (r > 0 && ms > 0.f) best = std::max(best, (double)bytes / (ms * 1e6));
-    }
-    std::vector<uint32_t> back(bytes / 4);
-    const bool same = cudaMemcpy(back.data(), dbuf, bytes, cudaMemcpyDeviceToHost) == cudaSuccess &&
-                      memcmp(back.data(), hbuf, bytes) == 0;
-    *gbs_out = best;
-    rc = (best > 0.0 && same) ? PROMOE_OK : PROMOE_ECUDA;
-  }
-  if (a) cudaEventDestroy(a);
-  if (b) cudaEventDestroy(b);
-  if (st) cudaStreamDestroy(st);
-  if (dbuf) cudaFree(dbuf);
-  if (hbuf) cudaFreeHost(hbuf);
-  return rc;
-}
-
-typedef CUresult (*mf_write32_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
-extern "C" int promoe_measure_fill(size_t Be, size_t chunk, int32_t mode, int32_t n_fills, double* gbs_out) {
-  if (!Be || !chunk || n_fills < 1 || mode < 0 || mode > 4 || !gbs_out) return PROMOE_EINVAL;
-  const int nslot = 8, nch = (int)((Be + chunk - 1) / chunk);
-  void *hbuf = nullptr, *dbuf = nullptr;
-  uint32_t *flags = nullptr, *fsrc = nullptr;
-  cudaStream_t st = nullptr;
-  std::vector<cudaEvent_t> ev(3 * (size_t)n_fills + 2, nullptr);
-  void* fn = nullptr;
-  cudaDriverEntryPointQueryResult qr;
-  if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &fn, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess) fn = nullptr;
-  int rc = PROMOE_ECUDA;
-  bool ok = cudaHostAlloc(&hbuf, Be * nslot, cudaHostAllocDefault) == cudaSuccess && cudaMalloc(&dbuf, Be * nslot) == cudaSuccess &&
-            cudaMalloc((void**)&flags, (size_t)nslot * nch * 4) == cudaSuccess &&
-            cudaHostAlloc((void**)&fsrc, (size_t)nch * 4, cudaHostAllocDefault) == cudaSuccess &&
-            cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess;
-  for (auto& e : ev) ok = ok && cudaEventCreate(&e) == cudaSuccess;
-  if (ok && ((mode == 0 || mode == 1) && !fn)) ok = false;
-  if (ok) {
-    memset(hbuf, 1, Be * nslot);
-    for (int c = 0; c < nch; ++c) fsrc[c] = 7;
-    double best = 0.0;
-    for (int rep = 0; rep < 2; ++rep) {
-      cudaEventRecord(ev[3 * (size_t)n_fills], st);
-      for (int f = 0; f < n_fills; ++f) {
-        const int sl = f % nslot;
-        char* d = (char*)dbuf + (size_t)sl * Be;
-        const char* s = (const char*)hbuf + (size_t)sl * Be;
-        uint32_t* fl = flags + (size_t)sl * nch;
-        cudaEventRecord(ev[3 * (size_t)f], st);
-        if (mode == 0 || mode == 4) {
-          for (int c = 0; c < nch; ++c) {
-            const size_t off = (size_t)c * chunk, len = std::min(chunk, Be - off);
-            cudaMemcpyAsync(d + off, s + off, len, cudaMemcpyHostToDevice, st);
-            if (mode == 0) ((mf_write32_fn)fn)((CUstream)st, (CUdeviceptr)(uintptr_t)(fl + c), 7, 0);
-            else cudaMemcpyAsync(fl + c, fsrc + c, 4, cudaMemcpyHostToDevice, st);
-          }
-        } else {
-          cudaMemcpyAsync(d, s, Be, cudaMemcpyHostToDevice, st);
-          if (mode == 1) for (int c = 0; c < nch; ++c) ((mf_write32_fn)fn)((CUstream)st, (CUdeviceptr)(uintptr_t)(fl + c), 7, 0);
-          if (mode == 2) cudaMemcpyAsync(fl, fsrc, (size_t)nch * 4, cudaMemcpyHostToDevice, st);
-        }
-        cudaEventRecord(ev[3 * (size_t)f + 1], st);
-        cudaEventRecord(ev[3 * (size_t)f + 2], st);
-      }
-      cudaEventRecord(ev[3 * (size_t)n_fills + 1], st);
-      if (cudaStreamSynchronize(st) != cudaSuccess) break;
-      float ms = 0.f;
-      cudaEventElapsedTime(&ms, ev[3 * (size_t)n_fills], ev[3 * (size_t)n_fills + 1]);
-      if (ms > 0.f) best = std::max(best, (double)Be * n_fills / (ms * 1e6));
-    }
-    *gbs_out = best;
-    rc = best > 0.0 ? PROMOE_OK : PROMOE_ECUDA;
-  }
-  for (auto e : ev) if (e) cudaEventDestroy(e);
-  if (st) cudaStreamDestroy(st);
-  if (dbuf) cudaFree(dbuf);
-  if (flags) cudaFree(flags);
-  if (hbuf) cudaFreeHost(hbuf);
-  if (fsrc) cudaFreeHost(fsrc);
-  return rc;
-}

@@ -30,7 +30,12 @@ struct SlotPhys {
   size_t fill_seq = 0;          // ring sequence of the last copy operation of this slot
   cudaEvent_t done = nullptr;   // recorded after the last chunk of the current generation
   bool done_valid = false;
+  int low_chunks = 0;           // chunks of the current generation that were moved by LOW (predicted) copies
+  size_t low_bytes = 0;         // their bytes, not yet attributed to useful / wasted
+  std::vector<size_t> low_ring; // ring sequence of each of them (landed once the ring tail has passed it)
 };
+constexpr size_t kFlagSrcRing = 1u << 20;   // words in the pinned ring the flag copies read their generation values from
+constexpr int kMaxChunks = 8192;            // chunks per expert image (promoe_create rejects smaller chunk sizes)
 
 }  // namespace pmk
 
@@ -112,6 +117,16 @@ struct promoe {
   std::vector<std::vector<int32_t>> pending_pred;  // per target layer
   std::vector<int32_t> trace_pred_host_lists;      // predictor_mode TRACE input [Lm*(1+E)]
   promoe_stats_t st{};
+  bool unchunked = false;             // ablation: a fill is all or nothing (no resume from ready_chunk, "without chunking")
+  int dev = 0;
+  // device-side fetch worker of the fused decode step (kernels_fetch.cu)
+  cudaStream_t fs = nullptr;              // its stream (highest priority)
+  pmk::LayerCmd* cmd_fetch = nullptr;     // device copy of the command ring [Lm]
+  uint32_t *claims = nullptr, *complete = nullptr, *alive = nullptr;
+  unsigned long long *fetch_ctr = nullptr, *fetch_ctr_pin = nullptr;   // device counters / pinned host copy
+  unsigned long long* src_dev = nullptr;  // [Lm*E] device-visible addresses of the host expert images
+  int fetch_ctas = 4;
+  bool phys_dirty = false;                // the device path has moved bytes since the host's SlotPhys was last synced
   int pos = 0;
   uint32_t step_seq = 0;
   int last_T = 0;

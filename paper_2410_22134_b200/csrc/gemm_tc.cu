@@ -334,4 +334,13 @@ bool tc_launch(TcContext* c, const TcGemm& g, cudaStream_t st, std::string* err)
   return true;
 }
 
+// Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every
+// running kernel to finish: a first launch behind a kernel that spins on a flag (an expert kernel waiting for its bytes,
+// the fetch worker waiting for a gate) would dead-lock until the spinner times out (profiles/r02_spin_probe.md).
+void preload_tc() {
+  preload_fn((const void*)gemm_tc_kernel<true>);
+  preload_fn((const void*)gemm_tc_kernel<false>);
+  preload_fn((const void*)split_rows_kernel);
+}
+
 }  // namespace pmk

@@ -9,7 +9,11 @@
 namespace pmk {
 
 // A0 embedding lookup: x[t,:] = Emb[ids[t],:] widened to fp32.
-void launch_embed(const int32_t* ids, const void* emb, float* x, int T, int H, int wdtype, cudaStream_t st);
+// alive != nullptr (fused decode): thread 0 first waits until *alive == alive_want, i.e. until the fetch kernel of this
+// step (kernels_fetch.cu) is resident — every later kernel of the step is ordered behind this one, so no flag-gated
+// kernel can occupy the GPU before the worker that feeds it runs.
+void launch_embed(const int32_t* ids, const void* emb, float* x, int T, int H, int wdtype, cudaStream_t st,
+                  const uint32_t* alive = nullptr, uint32_t alive_want = 0, int* err = nullptr);
 // A1 RMSNorm: y = x * rsqrt(mean(x^2)+eps) * w   (one warp-group per row).
 void launch_rmsnorm(const float* x, const float* w, float* y, int T, int H, float eps, cudaStream_t st);
 
@@ -73,12 +77,31 @@ struct LayerCmd {
 // One thread block (one warp) runs PushPrecise(m) then PushPredicted(m+stride) (Alg. 2) and writes:
 //  problems[i] for the needed experts in launch order (row ranges from offset[] when T > 1),
 //  dec_order[j] (decode: launch position -> j), the trace records and the host command.
+// cmd_dev2: second copy of the command in DEVICE memory for the fetch kernel (fused decode), or nullptr.
 void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int32_t* sel, int T, int k, const int32_t* offset,
                        const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* j_of_problem, LayerCmd* cmd,
                        uint32_t seq, int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st,
-                       const RouteFuse* fuse = nullptr);
+                       const RouteFuse* fuse = nullptr, LayerCmd* cmd_dev2 = nullptr);
+
+// A7 (fused decode): the device-side prefetch worker (kernels_fetch.cu).
+struct FetchArgs {
+  const LayerCmd* cmd;         // device ring [Lm] written by the slot-table kernel
+  const unsigned long long* src;   // [Lm*E] device-visible addresses of the pinned host expert images
+  uint8_t* slots;              // slot region [Lm, C, Be]
+  unsigned long long Be, chunk_bytes;
+  uint32_t* flags;             // [Lm, C, n_chunks]  generation whose chunk has landed (Alg. 1 l.10 ready_chunk)
+  uint32_t* claims;            // [Lm, C, n_chunks]  (generation << 1 | by_LOW) of the copy that took the chunk
+  uint32_t* complete;          // [Lm, C]            generation whose whole image is known to have landed
+  unsigned long long* ctr;     // FC_N counters (kernels_fetch.cu), zeroed by the host before the launch
+  int* err;                    // device error word (shared with the expert kernels)
+  uint32_t* alive;             // ← step once the worker runs
+  uint32_t step;
+  int Lm, C, E, n_chunks, preempt, unchunked, low_cap;
+};
+constexpr int kFetchCounters = 16;
+cudaError_t launch_fetch(const FetchArgs& a, int ctas, cudaStream_t st);
 
 // A9 decode expert FFN (GEMV, T == 1) over a problem list in launch order.
 //  gateup: act[p, i] = silu(Wg_p[i,:].u) * (Wu_p[i,:].u)     down: y[p, h] = Wd_p[h,:].act[p,:]
@@ -86,9 +109,6 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
 void launch_ffn_gateup_gemv(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
                             int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st,
                             int static_table = 0);   // 1: records written at load time → early L2 prefetch under PDL
-// TMA-fed variant (bf16 weights, H <= 2048, H % 256 == 0); false = shape unsupported, nothing launched
-bool launch_ffn_gateup_gemv_tma(const float* u, const FfnProblem* probs, int n_probs, int inter, int H, float* act,
-                                int act_stride, size_t chunk_bytes, int* err, cudaStream_t st);
 void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int max_inter,
                           int H, float* y, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st, int static_table = 0);
 // A9 prefill grouped SwiGLU FFN, SIMT fp32: problems [p0, p0+np) each with its row range; x rows are gathered

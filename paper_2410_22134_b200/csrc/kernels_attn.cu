@@ -265,4 +265,16 @@ void launch_attn_prefill(const float* qkv, const float* kcache, const float* vca
   }
 }
 
+// Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every
+// running kernel to finish: a first launch behind a kernel that spins on a flag (an expert kernel waiting for its bytes,
+// the fetch worker waiting for a gate) would dead-lock until the spinner times out (profiles/r02_spin_probe.md).
+void preload_attn() {
+  preload_fn((const void*)rope_append_kernel);
+  preload_fn((const void*)attn_decode_kernel<128>);
+  preload_fn((const void*)attn_decode_kernel<64>);
+  preload_fn((const void*)attn_decode_merge_kernel);
+  preload_fn((const void*)attn_prefill_kernel<128>);
+  preload_fn((const void*)attn_prefill_kernel<64>);
+}
+
 }  // namespace pmk

@@ -88,6 +88,7 @@ __global__ void __launch_bounds__(256, 6) norm_multi_gemv_kernel(NormGemvArgs a)
       if (lane == 0) a.act[rr] = silu(g) * v;
     }
   }
+  pdl_done();
 }
 void launch_norm_multi_gemv(const NormGemvArgs& a_in, int wdtype, cudaStream_t st) {
   ++g_launches;
@@ -196,6 +197,7 @@ __global__ void __launch_bounds__(128) attn_decode_fused_kernel(const float* __r
       m = mn;
     }
   }
+  pdl_done();
   // merge the 16 key groups of this CTA (fixed order)
   if (sub == 0) { sm_m[grp] = m; sm_l[grp] = l; }
 #pragma unroll
@@ -336,6 +338,7 @@ __global__ void __launch_bounds__(256, 4) ffn_down_combine_kernel(const float* _
                                                  : row_dot<WT>(wr, it_x[it] + it_off[it], len, lane);
     if (lane == 0) part[rr][it] = v;
   }
+  pdl_done();
   __syncthreads();
   if (threadIdx.x < DC_ROWS && r0 + threadIdx.x < H) {
     const int rr = threadIdx.x;
@@ -364,6 +367,18 @@ void launch_ffn_down_combine(const float* act, int act_stride, const FfnProblem*
   const int blocks = (H + DC_ROWS - 1) / DC_ROWS;
   if (wdtype == 0) launch_pdl(ffn_down_combine_kernel<float>, dim3(blocks), dim3(256), 0, st, act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
   else launch_pdl(ffn_down_combine_kernel<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, act, act_stride, probs, row_of, gates, k, shared, sact, sgate_logit, shared_y, H, x, chunk_bytes, err);
+}
+
+// Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every
+// running kernel to finish: a first launch behind a kernel that spins on a flag (an expert kernel waiting for its bytes,
+// the fetch worker waiting for a gate) would dead-lock until the spinner times out (profiles/r02_spin_probe.md).
+void preload_decode() {
+  preload_fn((const void*)norm_multi_gemv_kernel<float>);
+  preload_fn((const void*)norm_multi_gemv_kernel<__nv_bfloat16>);
+  preload_fn((const void*)attn_decode_fused_kernel<128>);
+  preload_fn((const void*)attn_decode_fused_kernel<64>);
+  preload_fn((const void*)ffn_down_combine_kernel<float>);
+  preload_fn((const void*)ffn_down_combine_kernel<__nv_bfloat16>);
 }
 
 }  // namespace pmk

@@ -8,15 +8,26 @@ namespace pmk {
 // A0 embedding lookup
 template <typename WT>
 __global__ void embed_kernel(const int32_t* __restrict__ ids, const WT* __restrict__ emb, float* __restrict__ x,
-                             int H) {
+                             int H, const uint32_t* alive, uint32_t alive_want, int* err) {
+  if (alive) {      // fused decode: the step starts only once its fetch worker is resident (kernels.h)
+    if (threadIdx.x == 0) {
+      const unsigned long long t0 = globaltimer_ns();
+      while (ld_acquire_sys(alive) != alive_want) {
+        if (globaltimer_ns() - t0 > kFlagTimeoutNs) { atomicExch(err, 1); break; }
+        __nanosleep(200);
+      }
+    }
+    __syncthreads();
+  }
   const int t = blockIdx.x;
   const WT* row = emb + (size_t)ids[t] * H;
   for (int i = threadIdx.x; i < H; i += blockDim.x) x[(size_t)t * H + i] = wload1(row + i);
 }
-void launch_embed(const int32_t* ids, const void* emb, float* x, int T, int H, int wdtype, cudaStream_t st) {
+void launch_embed(const int32_t* ids, const void* emb, float* x, int T, int H, int wdtype, cudaStream_t st,
+                  const uint32_t* alive, uint32_t alive_want, int* err) {
   ++g_launches;
-  if (wdtype == 0) embed_kernel<float><<<T, 256, 0, st>>>(ids, (const float*)emb, x, H);
-  else embed_kernel<__nv_bfloat16><<<T, 256, 0, st>>>(ids, (const __nv_bfloat16*)emb, x, H);
+  if (wdtype == 0) embed_kernel<float><<<T, 256, 0, st>>>(ids, (const float*)emb, x, H, alive, alive_want, err);
+  else embed_kernel<__nv_bfloat16><<<T, 256, 0, st>>>(ids, (const __nv_bfloat16*)emb, x, H, alive, alive_want, err);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -62,6 +73,7 @@ __global__ void __launch_bounds__(256) gemv_kernel(const float* __restrict__ x, 
       y[n] = v;
     }
   }
+  pdl_done();
 }
 void launch_gemv(const float* x, const void* w, float* y, int N, int K, int wdtype, int flags, cudaStream_t st) {
   ++g_launches;
@@ -169,6 +181,22 @@ __global__ void add_kernel(const float* __restrict__ a, const float* __restrict_
 void launch_add(const float* a, const float* b, float* out, size_t n, cudaStream_t st) {
   ++g_launches;
   add_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, b, out, n);
+}
+
+// Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every
+// running kernel to finish: a first launch behind a kernel that spins on a flag (an expert kernel waiting for its bytes,
+// the fetch worker waiting for a gate) would dead-lock until the spinner times out (profiles/r02_spin_probe.md).
+void preload_dense() {
+  preload_fn((const void*)embed_kernel<float>);
+  preload_fn((const void*)embed_kernel<__nv_bfloat16>);
+  preload_fn((const void*)rmsnorm_kernel);
+  preload_fn((const void*)gemv_kernel<float>);
+  preload_fn((const void*)gemv_kernel<__nv_bfloat16>);
+  preload_fn((const void*)linear_small_n_kernel<float>);
+  preload_fn((const void*)linear_small_n_kernel<__nv_bfloat16>);
+  preload_fn((const void*)gemm_simt_kernel<float>);
+  preload_fn((const void*)gemm_simt_kernel<__nv_bfloat16>);
+  preload_fn((const void*)add_kernel);
 }
 
 }  // namespace pmk

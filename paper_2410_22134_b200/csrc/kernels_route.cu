@@ -223,4 +223,20 @@ void launch_combine(const float* hres, const float* yexp, const int32_t* row_of,
   combine_kernel<<<T, 256, 0, st>>>(hres, yexp, row_of, gates, k, H, shared, sgate_logit, out);
 }
 
+// Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every
+// running kernel to finish: a first launch behind a kernel that spins on a flag (an expert kernel waiting for its bytes,
+// the fetch worker waiting for a gate) would dead-lock until the spinner times out (profiles/r02_spin_probe.md).
+void preload_route() {
+  preload_fn((const void*)topk_gate_kernel<1>);
+  preload_fn((const void*)topk_gate_kernel<2>);
+  preload_fn((const void*)topk_gate_kernel<4>);
+  preload_fn((const void*)topk_gate_kernel<8>);
+  preload_fn((const void*)pred_list_kernel<1>);
+  preload_fn((const void*)pred_list_kernel<2>);
+  preload_fn((const void*)pred_list_kernel<4>);
+  preload_fn((const void*)pred_list_kernel<8>);
+  preload_fn((const void*)permute_kernel);
+  preload_fn((const void*)combine_kernel);
+}
+
 }  // namespace pmk

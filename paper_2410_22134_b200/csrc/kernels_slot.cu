@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
                                                          int inter, int wbytes, FfnProblem* problems,
                                                          int32_t* n_problems, int32_t* row_of, LayerCmd* cmd,
                                                          uint32_t seq, int32_t* trace_precise,
-                                                         int32_t* trace_pred, RouteFuse rf) {
+                                                         int32_t* trace_pred, RouteFuse rf, LayerCmd* cmd2) {
   __shared__ uint8_t needed[kMaxE];
   __shared__ uint8_t prot[kMaxE];
   __shared__ int16_t order[kMaxE];
@@ -197,12 +197,18 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   }
   __syncthreads();
   // first publication (posted writes to mapped pinned memory; every writer fences its own stores; seq last)
-  for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
-  if (threadIdx.x == 0) cmd->n_needed = s_n;
+  // (fused decode: a second copy in device memory feeds the fetch kernel, kernels_fetch.cu — the host copy is only read
+  // after the step, for the statistics)
+  for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) { cmd->need[i] = rec[i]; if (cmd2) cmd2->need[i] = rec[i]; }
+  if (threadIdx.x == 0) { cmd->n_needed = s_n; if (cmd2) cmd2->n_needed = s_n; }
   __threadfence_system();
   __syncthreads();
-  if (threadIdx.x == 0) { volatile uint32_t* sq = &cmd->seq; *sq = seq; }
+  if (threadIdx.x == 0) {
+    if (cmd2) { volatile uint32_t* s2 = &cmd2->seq; *s2 = seq; }
+    volatile uint32_t* sq = &cmd->seq; *sq = seq;
+  }
 
+  pdl_done();      // the expert kernels may take their places while the predictor half runs
   // ================= phase 2: predictor W2 + list (fused decode only) + PushPredicted(m + stride) =================
   if (rf.zraw && rf.pred_out) {
     const int nwarps = blockDim.x >> 5;
@@ -286,11 +292,17 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   }
   __syncthreads();
   // second publication
-  for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) cmd->pred[i] = prec[i];
-  if (threadIdx.x == 0) { cmd->n_pred = s_np; cmd->pred_target = m + stride; }
+  for (int i = threadIdx.x; i < 5 * s_np; i += blockDim.x) { cmd->pred[i] = prec[i]; if (cmd2) cmd2->pred[i] = prec[i]; }
+  if (threadIdx.x == 0) {
+    cmd->n_pred = s_np; cmd->pred_target = m + stride;
+    if (cmd2) { cmd2->n_pred = s_np; cmd2->pred_target = m + stride; }
+  }
   __threadfence_system();
   __syncthreads();
-  if (threadIdx.x == 0) { volatile uint32_t* sq = &cmd->seq_pred; *sq = seq; }
+  if (threadIdx.x == 0) {
+    if (cmd2) { volatile uint32_t* s2 = &cmd2->seq_pred; *s2 = seq; }
+    volatile uint32_t* sq = &cmd->seq_pred; *sq = seq;
+  }
   // write the staged rows back
   for (int i = threadIdx.x; i < C; i += blockDim.x) {
     tbl.slot_expert[(size_t)m * C + i] = t_se[0][i]; tbl.stamp[(size_t)m * C + i] = t_stamp[0][i];
@@ -311,14 +323,21 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
-                       int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf) {
+                       int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf, LayerCmd* cmd_dev2) {
   ++g_launches;
   (void)reorder;
   RouteFuse f{};
   if (rf) f = *rf;
   launch_pdl(slot_table_kernel, dim3(1), dim3((rf && T == 1) ? 1024 : 256), 0, st, tbl, m, stride, max_spec, sel, T, k, offset, pred_list,
              slot_base, slot_bytes, flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of, cmd, seq,
-             trace_precise, trace_pred, f);
+             trace_precise, trace_pred, f, cmd_dev2);
+}
+
+// Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every
+// running kernel to finish: a first launch behind a kernel that spins on a flag (an expert kernel waiting for its bytes,
+// the fetch worker waiting for a gate) would dead-lock until the spinner times out (profiles/r02_spin_probe.md).
+void preload_slot() {
+  preload_fn((const void*)slot_table_kernel);
 }
 
 }  // namespace pmk

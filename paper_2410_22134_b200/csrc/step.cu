@@ -17,6 +17,7 @@
 #include "engine.h"
 #include "gemm_tc.h"
 
+#include <cstdio>
 #include <cstring>
 
 using namespace pmk;
@@ -26,6 +27,9 @@ int ce_pump_low(promoe_t* h);
 int ce_wait_cmd(promoe_t* h, int m, uint32_t seq, int part);
 int ce_process_cmd(promoe_t* h, int m, std::vector<int>* deferred, int parts);
 int ce_issue_deferred(promoe_t* h, int m, int i, cudaEvent_t after);
+void ce_account_cmd(promoe_t* h, int m);
+int ce_sync_phys_from_device(promoe_t* h);
+int ce_flush_flags(promoe_t* h);
 
 #define CKS(call)                                                                                  \
   do {                                                                                             \
@@ -106,17 +110,6 @@ static int expert_batch(promoe_t* h, const int32_t* perm, int i, int j, int max_
 
 #define RC(expr) do { int rc_ = (expr); if (rc_ != PROMOE_OK) return rc_; } while (0)
 
-// Knock-out timing (measurement builds only, -DPROMOE_KNOCKOUT; never compiled into the product): the environment
-// variable PROMOE_KNOCKOUT is a bit mask of decode kernels NOT to launch (bit 0 K1, 1 K2, 2 K3, 3 K4, 4 shared expert,
-// 6 K6, 7 K7).  Results are then meaningless; the drop in all-resident decode time is that kernel's in-situ cost on
-// the critical path.  K5 cannot be knocked out: the host waits for its command.
-#ifdef PROMOE_KNOCKOUT
-static const int g_knockout = [] { const char* e = getenv("PROMOE_KNOCKOUT"); return e ? atoi(e) : 0; }();
-#define KO(bit) (g_knockout & (1 << (bit)))
-#else
-#define KO(bit) 0
-#endif
-
 // One layer of the batch-1 decode step with the fused kernels of kernels_decode.cu (7 launches instead of 19).
 static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   const promoe_shape_t& s = h->s;
@@ -127,10 +120,10 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   NormGemvArgs a{};                                                                      // K1
   a.x = h->x; a.gain = h->ln1[l]; a.eps = s.rms_eps; a.K = H;
   a.seg[0] = GemvSeg{h->wqkv[l], h->qkv, h->qkv_w, 0}; a.nseg = 1;
-  if (!KO(0)) launch_norm_multi_gemv(a, wd, cs);
-  if (!KO(1)) launch_attn_decode_fused(h->qkv, h->cos_t, h->sin_t, h->kcache + (size_t)l * kv_layer, h->vcache + (size_t)l * kv_layer,   // K2
+  launch_norm_multi_gemv(a, wd, cs);
+  launch_attn_decode_fused(h->qkv, h->cos_t, h->sin_t, h->kcache + (size_t)l * kv_layer, h->vcache + (size_t)l * kv_layer,   // K2
                            h->attn_ws, h->attn, h->attn_cnt, pos0, nq, nkv, d, s.max_seq, h->nsplit, cs);
-  if (!KO(2)) launch_gemv(h->attn, h->wo[l], h->x, H, nq * d, wd, LIN_ACC, cs);          // K3
+  launch_gemv(h->attn, h->wo[l], h->x, H, nq * d, wd, LIN_ACC, cs);          // K3
   NormGemvArgs b{};                                                                      // K4
   b.x = h->x; b.gain = h->ln2[l]; b.eps = s.rms_eps; b.K = H; b.u_out = h->u;
   if (l < s.n_dense_layers) {
@@ -148,7 +141,7 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   b.seg[b.nseg++] = GemvSeg{h->router[l], h->zraw, E, 0};
   if (mlp) b.seg[b.nseg++] = GemvSeg{h->pred_w1[l], h->p1, s.pred_hidden, LIN_RELU};
   if (s.n_shared_inter && s.shared_gate) b.seg[b.nseg++] = GemvSeg{h->shared_gate_w[l], h->sgate, 1, 0};
-  if (!KO(3)) launch_norm_multi_gemv(b, wd, cs);
+  launch_norm_multi_gemv(b, wd, cs);
   // The shared expert (resident weights, needs only u) runs on a side stream BESIDE the single-CTA slot-table kernel
   // and the host hand-over instead of behind them; K7 joins it.  (Ordering of sact / sy / u across layers: the fork
   // event of the next layer is recorded after this layer's K7, which has waited for the join event.)
@@ -156,10 +149,8 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
     if (cudaEventRecord(h->ev_fork, cs) != cudaSuccess || cudaStreamWaitEvent(h->cs2, h->ev_fork, 0) != cudaSuccess) {
       h->err = "fork of the shared-expert stream failed"; return PROMOE_ECUDA;
     }
-    if (!KO(4)) {
-      launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
-      launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
-    }
+    launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, s.n_shared_inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
+    launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, s.n_shared_inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs2, 1);
     if (cudaEventRecord(h->ev_join, h->cs2) != cudaSuccess) { h->err = "join event failed"; return PROMOE_ECUDA; }
   }
   int32_t* plist = (mlp || h->o.predictor_mode == PROMOE_PRED_TRACE) ? h->pred_list + (size_t)m * (1 + E) : nullptr;
@@ -171,24 +162,20 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   launch_slot_table(h->tbl, m, h->o.stride, h->max_spec_decode, sel, 1, k, nullptr, plist,
                     (h->o.flags & PROMOE_F_REORDER) != 0, h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb, h->problems,
                     h->n_prob, h->row_of, h->cmd_dev + m, seq, h->trace_precise + (size_t)m * (1 + 5 * E),
-                    (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf);
-  // The flag-gated kernels K6/K7 must NOT be enqueued before the copies they wait for: when the driver multiplexes
-  // the streams onto one hardware queue a resident spinning kernel starves the copy (seen on B200: 4 s flag
-  // time-outs), so copies always go first.
-  RC(ce_wait_cmd(h, m, seq, 1));                                                         // A7: needed list → HIGH fills
-  RC(ce_process_cmd(h, m, nullptr, 1));
-  if (!KO(6)) launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
+                    (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf, h->cmd_fetch + m);
+  // A7 runs beside this stream: the fetch worker (kernels_fetch.cu, resident since the start of the step) sees the
+  // command K5 publishes in device memory and pulls the missing chunks over the link; the flag-gated kernels K6/K7 are
+  // enqueued right away and wait (ld.acquire.sys on the chunk flags, __nanosleep between polls) for exactly the bytes
+  // they read.  The host is not in the layer loop at all.
+  launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
   if (s.n_shared_inter && cudaStreamWaitEvent(cs, h->ev_join, 0) != cudaSuccess) { h->err = "join of the shared-expert stream failed"; return PROMOE_ECUDA; }
-  if (!KO(7))
-    launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,               // K7
+  launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,               // K7
                             (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, s.n_shared_inter ? h->sy : nullptr, H, h->x,
                             wd, h->chunk_bytes, h->err_dev, cs);
-  // the predicted list is published by the second half of the slot-table kernel, which runs while the host issues
-  // the HIGH copies above: LOW jobs are queued as soon as it is there
-  RC(ce_wait_cmd(h, m, seq, 2));
-  RC(ce_process_cmd(h, m, nullptr, 2));
   return PROMOE_OK;
 }
+
+static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fused);
 
 static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_out) {
   const promoe_shape_t& s = h->s;
@@ -211,19 +198,110 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     }
   for (auto& v : h->pending_pred) v.clear();
 
+  const bool fused = T == 1 && !(h->o.flags & PROMOE_F_NOFUSE);
   h->want_done_events = T > 1;
+  if (!fused) RC(ce_sync_phys_from_device(h));      // the copy-engine path tracks slots on the host
   if (T > 1) RC(ce_retire(h, true));   // prefill orders compute after fills with events: start from a drained copy stream
   memcpy(h->ids_pin, ids_host, (size_t)T * 4);
   CKS(cudaMemcpyAsync(h->ids, h->ids_pin, (size_t)T * 4, cudaMemcpyHostToDevice, cs));
-  CKS(cudaEventRecord(h->step_start, cs));
-  if (h->o.flags & PROMOE_F_TRACE) {
-    CKS(cudaMemsetAsync(h->trace_pred, 0, (size_t)Lm * (1 + 4 * E) * 4, cs));
-    if (h->o.predictor_mode == PROMOE_PRED_NONE) CKS(cudaMemsetAsync(h->pred_list, 0, (size_t)Lm * (1 + E) * 4, cs));
+  if (fused) {     // A7 of this step: the device-side fetch worker, resident before anything that may wait for it
+    CKS(cudaMemsetAsync(h->fetch_ctr, 0, sizeof(unsigned long long) * kFetchCounters, h->fs));
+    FetchArgs fa{};
+    fa.cmd = h->cmd_fetch; fa.src = h->src_dev; fa.slots = h->slots; fa.Be = h->Be; fa.chunk_bytes = h->chunk_bytes;
+    fa.flags = h->flags; fa.claims = h->claims; fa.complete = h->complete; fa.ctr = h->fetch_ctr; fa.err = h->err_dev;
+    fa.alive = h->alive; fa.step = step_seq; fa.Lm = Lm; fa.C = C; fa.E = E; fa.n_chunks = h->n_chunks;
+    fa.preempt = (h->o.flags & PROMOE_F_PREEMPT) != 0; fa.unchunked = h->unchunked; fa.low_cap = h->low_cap;
+    // nothing may be queued BEHIND the worker on its stream, and no copy may be submitted behind a kernel that waits:
+    // a pending operation behind a spinning kernel blocks later copy submissions (profiles/r02_spin_probe.md)
+    CKS(launch_fetch(fa, h->fetch_ctas, h->fs));
   }
-  launch_embed(h->ids, h->emb, h->x, T, H, wd, cs);
+  cudaError_t e_end = cudaEventRecord(h->step_start, cs);
+  if (e_end == cudaSuccess && (h->o.flags & PROMOE_F_TRACE)) {
+    e_end = cudaMemsetAsync(h->trace_pred, 0, (size_t)Lm * (1 + 4 * E) * 4, cs);
+    if (e_end == cudaSuccess && h->o.predictor_mode == PROMOE_PRED_NONE) e_end = cudaMemsetAsync(h->pred_list, 0, (size_t)Lm * (1 + E) * 4, cs);
+  }
+  int rc_layers = PROMOE_OK;
+  if (e_end == cudaSuccess) {
+    launch_embed(h->ids, h->emb, h->x, T, H, wd, cs, fused ? h->alive : nullptr, step_seq, h->err_dev);
+    rc_layers = run_layers(h, T, step_seq, pos0, fused);
+  }
+  if (rc_layers == PROMOE_OK && e_end == cudaSuccess) {   // ---- last token: final norm + lm_head
+    NormGemvArgs f{};
+    f.x = h->x + (size_t)(T - 1) * H; f.gain = h->final_norm; f.eps = s.rms_eps; f.K = H;
+    f.seg[0] = GemvSeg{h->lm_head, h->logits, s.vocab, 0}; f.nseg = 1;
+    launch_norm_multi_gemv(f, wd, cs);
+    e_end = cudaEventRecord(h->step_end, cs);
+    if (e_end == cudaSuccess && logits_out) e_end = cudaMemcpyAsync(h->logits_pin, h->logits, (size_t)s.vocab * 4, cudaMemcpyDeviceToHost, cs);
+    if (e_end == cudaSuccess) e_end = cudaMemcpyAsync(h->err_pin, h->err_dev, 4, cudaMemcpyDeviceToHost, cs);
+  }
+  const bool failed = rc_layers != PROMOE_OK || e_end != cudaSuccess;
+  if (fused) {
+    // a step that could not be enqueued completely: raise the error word so that the worker (and any kernel waiting for
+    // it) gives up at once instead of running into its time-out
+    if (failed) { const int one = 1; cudaMemcpy(h->err_dev, &one, 4, cudaMemcpyHostToDevice); }
+#ifdef PMK_FETCH_TRACE
+    fprintf(stderr, "[host] step %u enqueued, sync cs\n", step_seq);
+    cudaError_t e1 = cudaStreamSynchronize(cs);
+    fprintf(stderr, "[host] cs done (%d), sync fs\n", (int)e1);
+    cudaError_t e2 = cudaStreamSynchronize(h->fs);
+    fprintf(stderr, "[host] fs done (%d)\n", (int)e2);
+#else
+    cudaError_t e1 = cudaStreamSynchronize(cs), e2 = cudaStreamSynchronize(h->fs);
+#endif
+    if (failed) cudaMemset(h->err_dev, 0, 4);
+    if (!failed && e1 != cudaSuccess) e_end = e1;
+    if (!failed && e_end == cudaSuccess && e2 != cudaSuccess) e_end = e2;
+    if (!failed && e_end == cudaSuccess)
+      e_end = cudaMemcpy(h->fetch_ctr_pin, h->fetch_ctr, sizeof(unsigned long long) * kFetchCounters, cudaMemcpyDeviceToHost);
+    h->phys_dirty = true;
+  } else if (!failed) {
+    // keep feeding LOW chunks while the tail of the step drains (no-preempt mode may leave some queued)
+    while (cudaStreamQuery(cs) == cudaErrorNotReady) {
+      int rc = ce_pump_low(h);
+      if (rc) return rc;
+    }
+    RC(ce_flush_flags(h));
+  }
+  if (rc_layers != PROMOE_OK) return rc_layers;
+  if (e_end != cudaSuccess) { h->err = std::string("step: ") + cudaGetErrorString(e_end); return PROMOE_ECUDA; }
+  CKS(cudaStreamSynchronize(cs));
+  const int err_host = *h->err_pin;
+  if (logits_out) memcpy(logits_out, h->logits_pin, (size_t)s.vocab * 4);
+  float ms = 0.f;
+  CKS(cudaEventElapsedTime(&ms, h->step_start, h->step_end));
+  if (fused) {     // statistics: logical from the command ring, physical from the worker's counters
+    for (int m = 0; m < Lm; ++m) ce_account_cmd(h, m);
+    const unsigned long long* c = h->fetch_ctr_pin;
+    promoe_stats_t& st = h->st;
+    st.high_bytes += c[0]; st.low_bytes += c[1]; st.h2d_bytes += c[0] + c[1]; st.low_bytes_useful += c[2]; st.hits_landed += c[3];
+    st.owed_bytes_at_gate += c[4]; st.landed_chunks_at_gate += c[5]; st.landed_chunks_of += c[6];
+    st.fetched_at_gate += c[7]; st.fetched_at_gate_of += c[8]; st.chunks_high += c[9]; st.chunks_low += c[10];
+    st.chunks_issued += c[9] + c[10]; st.chunks_cancelled += c[11]; st.copy_busy_ms += (double)c[12] * 1e-6;
+  } else {
+    int rc = ce_retire(h, false);
+    if (rc) return rc;
+  }
+  h->st.steps++; h->st.tokens += (uint64_t)T;
+  h->st.step_ms += ms; h->st.last_step_ms = ms;
+  h->pos += T;
+  h->last_T = T;
+  if (err_host) {
+    h->st.timeouts++;
+    CKS(cudaMemsetAsync(h->err_dev, 0, 4, cs));
+    h->err = "a kernel timed out waiting for a chunk-ready flag or for the fetch worker (device error word " + std::to_string(err_host) + ")";
+    return PROMOE_ETIMEOUT;
+  }
+  return PROMOE_OK;
+}
+
+// The layer loop of one step on the compute stream.
+static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fused) {
+  const promoe_shape_t& s = h->s;
+  const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter;
+  const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = s.wdtype;
+  cudaStream_t cs = h->cs;
   const size_t kv_layer = (size_t)nkv * s.max_seq * d;
   std::vector<int> deferred;
-  const bool fused = T == 1 && !(h->o.flags & PROMOE_F_NOFUSE);
   for (int l = 0; l < s.n_layers; ++l) {
     if (fused) { RC(decode_layer_fused(h, l, step_seq, pos0)); continue; }
     // ---- attention block (A1-A3)
@@ -333,38 +411,6 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
       }
       launch_combine(h->x, h->yexp, inv, gates, T, k, H, shared, sgate, h->x, cs);
     }
-  }
-  // ---- last token: final norm + lm_head
-  {
-    NormGemvArgs f{};
-    f.x = h->x + (size_t)(T - 1) * H; f.gain = h->final_norm; f.eps = s.rms_eps; f.K = H;
-    f.seg[0] = GemvSeg{h->lm_head, h->logits, s.vocab, 0}; f.nseg = 1;
-    launch_norm_multi_gemv(f, wd, cs);
-  }
-  CKS(cudaEventRecord(h->step_end, cs));
-  if (logits_out) CKS(cudaMemcpyAsync(h->logits_pin, h->logits, (size_t)s.vocab * 4, cudaMemcpyDeviceToHost, cs));
-  CKS(cudaMemcpyAsync(h->err_pin, h->err_dev, 4, cudaMemcpyDeviceToHost, cs));
-  // keep feeding LOW chunks while the tail of the step drains (no-preempt mode may leave some queued)
-  while (cudaStreamQuery(cs) == cudaErrorNotReady) {
-    int rc = ce_pump_low(h);
-    if (rc) return rc;
-  }
-  CKS(cudaStreamSynchronize(cs));
-  const int err_host = *h->err_pin;
-  if (logits_out) memcpy(logits_out, h->logits_pin, (size_t)s.vocab * 4);
-  float ms = 0.f;
-  CKS(cudaEventElapsedTime(&ms, h->step_start, h->step_end));
-  int rc = ce_retire(h, false);
-  if (rc) return rc;
-  h->st.steps++; h->st.tokens += (uint64_t)T;
-  h->st.step_ms += ms; h->st.last_step_ms = ms;
-  h->pos += T;
-  h->last_T = T;
-  if (err_host) {
-    h->st.timeouts++;
-    CKS(cudaMemsetAsync(h->err_dev, 0, 4, cs));
-    h->err = "an expert kernel timed out waiting for a chunk-ready flag";
-    return PROMOE_ETIMEOUT;
   }
   return PROMOE_OK;
 }

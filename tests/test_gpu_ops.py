@@ -202,34 +202,3 @@ def test_op_expert_ffn_tcgen05(B, T, H, I):
     ref = swiglu_ffn(x.double(), wg, wu, wdn)
     err = (y.cpu().double() - ref).abs().max().item()
     assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
-
-
-@pytest.mark.parametrize("H,I", [(256, 512), (2048, 1408), (1024, 264 * 8)])
-def test_op_expert_ffn_tma_gemv(B, H, I):
-    """Decode gate/up GEMV fed by cp.async.bulk through a shared-memory ring (path 4)."""
-    from oracle.forward import swiglu_ffn
-    x = _w((1, H), torch.float32, 7, 1.0)
-    wg, wu, wdn = _w((I, H), torch.bfloat16, 8), _w((I, H), torch.bfloat16, 9), _w((H, I), torch.bfloat16, 10)
-    xd, wgd, wud, wdd = x.cuda(), wg.cuda(), wu.cuda(), wdn.cuda()
-    act = torch.empty((1, I), device="cuda"); y = torch.full((1, H), float("nan"), device="cuda")
-    ws = torch.zeros(64, dtype=torch.uint8, device="cuda")
-    rc = B.lib().promoe_op_expert_ffn(xd.data_ptr(), wgd.data_ptr(), wud.data_ptr(), wdd.data_ptr(), act.data_ptr(),
-                                      y.data_ptr(), ws.data_ptr(), 1, H, I, 1, 4, 0, None)
-    assert rc == 0
-    torch.cuda.synchronize()
-    ref = swiglu_ffn(x.double(), wg, wu, wdn)
-    err = (y.cpu().double() - ref).abs().max().item()
-    assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
-
-
-def test_measure_sm_fill(B):
-    """SM-issued fill (promoe.h): copied bytes are verified inside the call; ragged 64-byte tail; bad arguments."""
-    L = B.lib()
-    import ctypes as C
-    g = C.c_double()
-    assert L.promoe_measure_sm_fill(0, 1, 256, 1, C.byref(g)) == B.PROMOE_EINVAL
-    assert L.promoe_measure_sm_fill(100, 1, 256, 1, C.byref(g)) == B.PROMOE_EINVAL          # not a multiple of 64
-    assert L.promoe_measure_sm_fill(1 << 20, 1, 100, 1, C.byref(g)) == B.PROMOE_EINVAL      # threads not a warp multiple
-    assert L.promoe_measure_sm_fill(1 << 20, 1, 256, 1, None) == B.PROMOE_EINVAL
-    for nbytes, ctas, thr in [(64, 1, 32), ((1 << 20) + 64, 3, 96), (17301504, 4, 1024), (64 << 20, 148, 256)]:
-        assert B.promoe_measure_sm_fill(nbytes, ctas, thr, 2) > 0.0
