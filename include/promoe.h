@@ -204,6 +204,20 @@ PROMOE_API int promoe_op_expert_ffn(const float* x, const void* wg, const void* 
                                     float* y, void* prob_ws, int32_t T, int32_t H, int32_t I, int32_t wdtype,
                                     int32_t path, int32_t reserved, void* stream);
 
+/* The same batch-1 expert FFN (A9 decode path, T == 1: y[H] = Wd.(silu(Wg.x) * (Wu.x))) for callers that may NOT allocate —
+ * code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The [I] activation vector and the
+ * problem record live in ONE file-scope device array of the library (64.25 KiB per GPU that loads the library, held until
+ * the process exits); the call itself performs no cudaMalloc / cudaFree and calls no allocating library routine.
+ * x [H], y [H] fp32 DEVICE ptrs, weights as above (DEVICE, borrowed for the call).  Limit: I <= 16384
+ * (promoe_op_expert_ffn_static_max_inter()); larger I, H or I not a multiple of 16, or a NULL pointer → PROMOE_EINVAL.
+ * Asynchronous on `stream`.  Every call on a device SHARES the array: calls that overlap on the GPU (different streams,
+ * no ordering between them) race on it; calls on one stream are ordered.  Nothing in it must start at zero (each call
+ * overwrites what it reads), so the previous call's contents never matter.  Same kernels as promoe_op_expert_ffn path 1:
+ * the result is bit-identical. */
+PROMOE_API int promoe_op_expert_ffn_static(const float* x, const void* wg, const void* wu, const void* wd, float* y,
+                                           int32_t H, int32_t I, int32_t wdtype, void* stream);
+PROMOE_API int promoe_op_expert_ffn_static_max_inter(void);
+
 #ifdef __cplusplus
 }
 #endif
