@@ -134,9 +134,9 @@ def run_reference(args, cfg, rank):
         return
     import synth
     weights = synth.make_weights(cfg, predictor="skip")
-    pl, ds = args.ref_prompt, args.ref_decode
-    for _ in range(args.warmup):
-        oracle_sample(cfg, weights, pl, ds)
+    pl, ds = ref_sample(args, cfg)
+    for _ in range(args.warmup):          # warm-up of a CPU program: page in the weights, start the thread pool
+        oracle_sample(cfg, weights, min(pl, 32), 1)
     t0 = time.perf_counter()
     dec, pre, cores = [], [], 0
     for _ in range(args.steps):
@@ -144,15 +144,31 @@ def run_reference(args, cfg, rank):
         dec.append(r["decode_tok_s"]); pre.append(r["prefill_tok_s"]); cores = r["cores"]
     dt = time.perf_counter() - t0
     v = len(dec) / sum(1.0 / x for x in dec)
-    sample = f"per step: prefill {pl} + {ds} decode tokens of {cfg.name} (of {cfg.prompt_len} + {cfg.decode_steps})"
+    sample = ref_sample_text(cfg, pl, ds)
+    conf = workload_config(cfg, args)
+    conf["reference_sample"] = {"prompt_tokens": pl, "decode_tokens": ds, "decode_positions": [pl, pl + ds - 1],
+                                "of_prompt": cfg.prompt_len, "of_decode": cfg.decode_steps}
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "tokens/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(cfg, args), "prefill_tokens_per_s": len(pre) / sum(1.0 / x for x in pre),
+            "config": conf, "prefill_tokens_per_s": len(pre) / sum(1.0 / x for x in pre),
             "cpu_baseline": {"value": v, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def ref_sample(args, cfg):
+    """Bounded oracle sample at the GPU arm's own token positions: the whole prompt when it is at most 512 tokens (so
+    that the decode tokens sit at the positions the GPU arm decodes at), then a few decode tokens."""
+    pl = args.ref_prompt if args.ref_prompt > 0 else min(cfg.prompt_len, 512)
+    return pl, args.ref_decode
+
+
+def ref_sample_text(cfg, pl, ds):
+    same = "the GPU arm's positions" if pl == cfg.prompt_len else f"SHORTER than the GPU arm's prompt of {cfg.prompt_len}"
+    return (f"per step: prefill {pl} tokens ({same}) + {ds} decode tokens at positions {pl}..{pl + ds - 1} of {cfg.name} "
+            f"(GPU arm: {cfg.prompt_len} + {cfg.decode_steps})")
 
 
 METRIC = "decode tokens/s at fixed expert-cache budget (prefill tokens/s and % of per-step roofline alongside)"
@@ -236,6 +252,32 @@ def run_request(eng, cfg, prompt, decode_ids, greedy: bool, record=None, inject=
             "pre": {k: d(s0, s1, k) for k in s0}, "dec": {k: d(s1, s2, k) for k in s1}}
 
 
+def replica_weights(cfg, pred_kind, local, world, dist, tag=None):
+    """Weights of one replica.  world > 1: the replicas of a node share ONE host copy of the routed experts — a /dev/shm
+    mapping drawn by local rank 0 and mapped by the others (every rank's library registers it with cudaHostRegister);
+    8 private pinned copies of 25-90 GB would not fit the host."""
+    import torch
+    import synth
+    if world <= 1:
+        return synth.make_weights(cfg, predictor=pred_kind)
+    s = cfg.shape
+    n_moe = s.n_layers - s.n_dense_layers
+    per = 3 * s.hidden * s.expert_inter
+    dt = torch.float32 if s.wdtype == 0 else torch.bfloat16
+    path = f"/dev/shm/promoe_experts_{tag or os.environ.get('MASTER_PORT', '0')}_{cfg.name}"
+    if local == 0:
+        buf = torch.from_file(path, shared=True, size=n_moe * s.n_experts * per, dtype=dt).view(n_moe, s.n_experts, per)
+        weights = synth.make_weights(cfg, predictor=pred_kind, experts_buf=buf, fill_experts=True)
+    dist.barrier()
+    if local != 0:
+        buf = torch.from_file(path, shared=True, size=n_moe * s.n_experts * per, dtype=dt).view(n_moe, s.n_experts, per)
+        weights = synth.make_weights(cfg, predictor=pred_kind, experts_buf=buf, fill_experts=False)
+    dist.barrier()
+    if local == 0:
+        os.unlink(path)          # the mappings keep the memory alive until the processes exit
+    return weights
+
+
 def run_ours(args, cfg, rank, world, dist):
     import numpy as np
     import torch
@@ -248,25 +290,7 @@ def run_ours(args, cfg, rank, world, dist):
     peaks = load_peaks()
     s = cfg.shape
     pred_kind = "skip" if args.predictor in ("none", "trace") else args.predictor
-    if world > 1:
-        # replicas share ONE host copy of the routed experts (a /dev/shm mapping drawn by local rank 0; every rank's
-        # library registers it with cudaHostRegister) — 8 private pinned copies of 25-90 GB would not fit the host
-        n_moe = s.n_layers - s.n_dense_layers
-        per = 3 * s.hidden * s.expert_inter
-        dt = torch.float32 if s.wdtype == 0 else torch.bfloat16
-        path = f"/dev/shm/promoe_experts_{os.environ.get('MASTER_PORT', '0')}_{cfg.name}"
-        if local == 0:
-            buf = torch.from_file(path, shared=True, size=n_moe * s.n_experts * per, dtype=dt).view(n_moe, s.n_experts, per)
-            weights = synth.make_weights(cfg, predictor=pred_kind, experts_buf=buf, fill_experts=True)
-        dist.barrier()
-        if local != 0:
-            buf = torch.from_file(path, shared=True, size=n_moe * s.n_experts * per, dtype=dt).view(n_moe, s.n_experts, per)
-            weights = synth.make_weights(cfg, predictor=pred_kind, experts_buf=buf, fill_experts=False)
-        dist.barrier()
-        if local == 0:
-            os.unlink(path)          # the mappings keep the memory alive until the processes exit
-    else:
-        weights = synth.make_weights(cfg, predictor=pred_kind)
+    weights = replica_weights(cfg, pred_kind, local, world, dist)
     wb = 4 if s.wdtype == 0 else 2
     Be = 3 * s.hidden * s.expert_inter * wb
     h2d_gbs = B.promoe_bench_h2d(256 << 20, 2, 5)
@@ -329,6 +353,10 @@ def run_ours(args, cfg, rank, world, dist):
     roof_pre = phase_roof("pre", cfg.prompt_len, 1, 0)
     roof_dec["frac"] = roof_dec["t_roof_s"] / dec_s
     roof_pre["frac"] = roof_pre["t_roof_s"] / pre_s
+    # `frac` takes B_need from THIS run's cache state, which a prefetching run pollutes with its own mispredictions;
+    # `frac_vs_reactive_need` (filled in below from the reactive pass over the same routing) uses the B_need of a plain
+    # LRU cache — a function of routing and budget only (re-fetches caused by pollution are overhead)
+    roof_dec["frac_vs_reactive_need"] = roof_pre["frac_vs_reactive_need"] = None
 
     def cache_stats(key):
         a = {k: sum(r[key][k] for r in reqs) for k in reqs[0][key]}
@@ -357,6 +385,8 @@ def run_ours(args, cfg, rank, world, dist):
     if os.path.exists(prof):
         try:
             kernel_roof["traffic"] = json.load(open(prof)).get(cfg.name, {}).get("ffn_gateup_gemv_kernel")
+            kernel_roof["traffic_source"] = ("stored constant: dram__bytes_read.sum + dram__bytes_write.sum per launch from the "
+                                             "ncu --set full capture named in profiles/README.md (not measured in this run)")
         except Exception:
             pass
     eng.close()
@@ -398,6 +428,13 @@ def run_ours(args, cfg, rank, world, dist):
             r = run_request(v, cfg, prompt, decode_ids, greedy, inject=inj)
             v.close()
             need_d, need_p = r["dec"]["need_experts"] * Be, r["pre"]["need_experts"] * Be
+            if pm == B.PRED_NONE:       # pollution-free B_need of the same requests → the headline fraction
+                for roof, need, t_meas, key in ((roof_dec, need_d, dec_s, "dec"), (roof_pre, need_p, pre_s, "pre")):
+                    t_r, bound_r, _ = roofline_time(need * K, roof["b_hbm_bytes"], roof["flops"], h2d_gbs, peaks["hbm_gbs"],
+                                                    peaks["bf16_tflops_sustained"])
+                    roof["b_need_reactive_bytes"] = need * K
+                    roof["frac_vs_reactive_need"] = t_r / t_meas
+                    roof["bound_vs_reactive_need"] = bound_r
             variants[name] = {
                 "decode_tokens_per_s": cfg.decode_steps / (r["decode_ms"] / 1e3),
                 "prefill_tokens_per_s": cfg.prompt_len / (r["prefill_ms"] / 1e3),
@@ -409,10 +446,11 @@ def run_ours(args, cfg, rank, world, dist):
 
     cpu = None
     if rank == 0 and not args.no_cpu:
-        o = oracle_sample(cfg, weights, args.ref_prompt, args.ref_decode)
+        rpl, rds = ref_sample(args, cfg)
+        o = oracle_sample(cfg, weights, rpl, rds)
         cpu = {"value": o["decode_tok_s"], "unit": "tokens/s", "cores": o["cores"], "kind": "oracle",
                "prefill_tokens_per_s": o["prefill_tok_s"], "seconds": o["seconds"],
-               "sample": f"prefill {args.ref_prompt} + {args.ref_decode} decode tokens of {cfg.name} (of {cfg.prompt_len} + {cfg.decode_steps})"}
+               "sample": ref_sample_text(cfg, rpl, rds)}
     if rank != 0:
         return
     line = {"metric": METRIC, "value": g_dec_tok / g_dec_s, "unit": "tokens/s", "n_gpus": world, "steps": K,
@@ -513,6 +551,14 @@ def run_sweep(args):
                       "compute_only_ms": {str(k): v for k, v in compute.items()}}), flush=True)
 
 
+def spawn_command(n_gpus: int, argv):
+    """Command line that runs this script as n_gpus ranks on one node (127.0.0.1 rendezvous, a free port)."""
+    import socket
+    sk = socket.socket(); sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]; sk.close()
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port), os.path.abspath(__file__), *argv]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -533,8 +579,8 @@ def main():
     ap.add_argument("--tensor", type=int, default=1, help="prefill GEMMs on tcgen05 (bf16 weights)")
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--decode-steps", type=int, default=0)
-    ap.add_argument("--ref-prompt", type=int, default=32, help="oracle sample: prompt tokens")
-    ap.add_argument("--ref-decode", type=int, default=3, help="oracle sample: decode tokens")
+    ap.add_argument("--ref-prompt", type=int, default=0, help="oracle sample: prompt tokens (0 = the whole prompt, capped at 512)")
+    ap.add_argument("--ref-decode", type=int, default=2, help="oracle sample: decode tokens")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4] grid on the c3 shape (one JSON line per point)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-allhit", action="store_true")
@@ -551,6 +597,10 @@ def main():
     if args.decode_steps:
         over["decode_steps"] = args.decode_steps
     cfg = synth.get_config(args.config, **over)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # launched as a plain `python bench.py --gpus N`: start the N ranks ourselves, one process per GPU, the way the
+        # driver does (replicas only; NCCL carries the two aggregate all-reduces, nothing on the data path)
+        sys.exit(subprocess.call(spawn_command(args.gpus, sys.argv[1:])))
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, cfg, rank)

@@ -81,3 +81,50 @@ def test_shared_expert_buffer_matches_private_copy(tmp_path):
     wb = synth.make_weights(cfg, pin=False, experts_buf=b, fill_experts=False)
     assert torch.equal(wa.experts, ref.experts) and torch.equal(wb.experts, ref.experts)
     assert all(torch.equal(wb.dense[k], ref.dense[k]) for k in ref.dense)
+
+
+def _replica_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    import synth
+    cfg = synth.get_config("c1b")
+    w = bench.replica_weights(cfg, "skip", rank, world, dist, tag=f"test{port}")
+    # what a replica hands to the engine: the expert images (shared mapping) and its own dense tensors
+    out.put((rank, float(w.experts.double().sum()), float(w.experts[1, 3, 17:4000].double().abs().sum()),
+             float(w.dense["l0.router"].double().sum()), w.experts.data_ptr() % 4096))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_replicas_share_one_expert_copy_two_ranks_gloo():
+    """bench.py --gpus N: two CPU-side ranks go through the /dev/shm path of replica_weights — local rank 0 draws the
+    routed experts into the mapping, rank 1 maps what rank 0 drew; both see the bytes of a private copy."""
+    import synth
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    ps = [ctx.Process(target=_replica_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in range(2))
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    ref = synth.make_weights(synth.get_config("c1b"), pin=False)
+    want = (float(ref.experts.double().sum()), float(ref.experts[1, 3, 17:4000].double().abs().sum()),
+            float(ref.dense["l0.router"].double().sum()))
+    for r in res:
+        assert r[1:4] == want
+        assert r[4] == 0                                   # page-aligned mapping (cudaHostRegister needs that)
+    assert not [f for f in os.listdir("/dev/shm") if f.startswith(f"promoe_experts_test{port}")]   # unlinked after mapping
+
+
+def test_gpus_flag_spawns_one_rank_per_gpu():
+    """`python bench.py --gpus N` without a launcher starts N ranks itself."""
+    import bench
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "2"])
+    assert cmd[1:3] == ["-m", "torch.distributed.run"]
+    assert "--nproc-per-node=4" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and cmd[-5].endswith("bench.py")
