@@ -31,7 +31,20 @@ every touch / alloc sets stamp ← ++clock (LRU = smallest stamp).
        with T > 1 tokens 50-100 % of the experts are needed and a per-layer LRU has no free slot, so
        an allocation only swaps one needed expert for another; predictions then only refresh LRU stamps.
 
-alloc victim (Alg. 1 l.4 `cache.replace_with`): lowest-index EMPTY slot, else smallest stamp among unprotected.
+alloc victim (Alg. 1 l.4 `cache.replace_with`): lowest-index EMPTY slot, else smallest stamp among unprotected
+(equal stamps — only demoted slots, below — → lowest slot index).
+
+Two switches (readings G16, G17), both off the paper's text:
+  reorder=False — the ablation baseline of §7.3 / Fig. 12 WITHOUT reordered inference: the needed experts
+     are processed in ascending id (the order a framework loops over them), each classified AT ITS TURN:
+     holds a slot → class A / B + touch; holds none → class C, alloc with the plain LRU victim over ALL slots
+     ("standard per-layer LRU") — which may be a needed expert whose turn has not come yet: it is then
+     fetched again at its own turn (the cache-unfriendly order §5.3 removes).  If the victim's slot holds an expert
+     that was launched EARLIER in this layer, `dep` = that launch index (its compute must finish before the copy).
+  demote=True — a slot of origin PRED whose expert the gate of its layer did NOT select (a misprediction) gets
+     stamp 0 at that gate, before the class-C allocations: it is the next victim, so a wrong prediction costs the
+     cache one LRU victim (which the next miss would have taken anyway) instead of a most-recently-used slot.
+     The paper keeps mispredicted prefetches as ordinary MRU entries.
 """
 from __future__ import annotations
 
@@ -87,8 +100,10 @@ class CacheStats:
 
 
 class ProMoECacheSim:
-    def __init__(self, n_moe_layers: int, n_experts: int, slots_per_layer: int, warm: bool = True):
+    def __init__(self, n_moe_layers: int, n_experts: int, slots_per_layer: int, warm: bool = True,
+                 reorder: bool = True, demote: bool = False):
         self.L, self.E, self.C = n_moe_layers, n_experts, slots_per_layer
+        self.reorder, self.demote = reorder, demote
         self.slot_expert = [[EMPTY] * self.C for _ in range(self.L)]
         self.stamp = [[0] * self.C for _ in range(self.L)]
         self.origin = [[RESIDENT] * self.C for _ in range(self.L)]
@@ -139,9 +154,48 @@ class ProMoECacheSim:
         self._step_start = [set(x for x in row if x != EMPTY) for row in self.slot_expert]
         self._pending_pred = {}
 
+    def _demote_mispredicted(self, m: int, needed: Sequence[int]) -> None:
+        for s in range(self.C):
+            if self.origin[m][s] == PRED and self.slot_expert[m][s] not in needed:
+                self.stamp[m][s] = 0
+
+    def _push_precise_id_order(self, m: int, needed: List[int]) -> PreciseRecord:
+        st = self.stats
+        rec = PreciseRecord()
+        st.accesses += len(needed)
+        st.need_experts += len([e for e in needed if e not in self._step_start[m]])
+        for i, e in enumerate(needed):
+            s = self.slot_of(m, e)
+            if s >= 0:
+                cls = CLASS_B if self.origin[m][s] == PRED else CLASS_A
+                if cls == CLASS_A:
+                    st.hits_resident += 1
+                else:
+                    st.hits_prefetch += 1
+                self._touch(m, s)
+                rec.expert.append(e); rec.cls.append(cls); rec.slot.append(s); rec.victim.append(-1); rec.dep.append(-1)
+                continue
+            st.misses += 1
+            s = self._victim(m, set())
+            old = self.slot_expert[m][s]
+            dep = needed.index(old) if old in needed[:i] else -1
+            self._install(m, s, e, PRECISE)
+            rec.expert.append(e); rec.cls.append(CLASS_C); rec.slot.append(s); rec.victim.append(old); rec.dep.append(dep)
+        for s in range(self.C):
+            self.origin[m][s] = RESIDENT
+        return rec
+
     def push_precise(self, m: int, needed: Sequence[int]) -> PreciseRecord:
         needed = sorted(set(int(e) for e in needed))
         st = self.stats
+        if m in self._pending_pred:
+            pred = self._pending_pred.pop(m)
+            st.predicted += len(pred)
+            st.predicted_correct += len([e for e in pred if e in needed])
+        if self.demote:
+            self._demote_mispredicted(m, needed)
+        if not self.reorder:
+            return self._push_precise_id_order(m, needed)
         A = [e for e in needed if self.slot_of(m, e) >= 0 and self.origin[m][self.slot_of(m, e)] != PRED]
         B = [e for e in needed if self.slot_of(m, e) >= 0 and self.origin[m][self.slot_of(m, e)] == PRED]
         Cs = [e for e in needed if self.slot_of(m, e) < 0]
@@ -152,10 +206,6 @@ class ProMoECacheSim:
         st.hits_prefetch += len(B)
         st.misses += len(Cs)
         st.need_experts += len([e for e in needed if e not in self._step_start[m]])
-        if m in self._pending_pred:
-            pred = self._pending_pred.pop(m)
-            st.predicted += len(pred)
-            st.predicted_correct += len([e for e in pred if e in needed])
         for e in A + B:
             s = self.slot_of(m, e)
             self._touch(m, s)

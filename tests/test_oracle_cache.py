@@ -250,3 +250,93 @@ def test_max_spec_limits_allocations_in_listed_order():
     a = ProMoECacheSim(1, 8, 4, warm=True); b = ProMoECacheSim(1, 8, 4, warm=True)
     ra = a.push_predicted(0, [5, 6, 1, 7]); rb = b.push_predicted(0, [5, 6, 1, 7], max_spec=4)
     assert ra.as_tuples() == rb.as_tuples() and a.slot_expert == b.slot_expert    # None ≡ no limit
+
+
+# ---- reorder = False: the ID-order ablation baseline (Fig. 12 "Base") ------------------------------------
+@pytest.mark.parametrize("warm", [True, False])
+@pytest.mark.parametrize("T_experts", [3, 9])
+def test_id_order_is_textbook_lru_in_ascending_id(warm, T_experts):
+    """Without reordered inference the table is a standard per-layer LRU accessed in ascending expert id — also
+    in prefill, where |needed| > C and a needed expert may be evicted before its turn and fetched again."""
+    rng = random.Random(7)
+    L, E, C = 2, 16, 6
+    sim = ProMoECacheSim(L, E, C, warm=warm, reorder=False)
+    ref = [TextbookLRU(C, range(C) if warm else []) for _ in range(L)]
+    for step in range(200):
+        needed = [sorted(rng.sample(range(E), T_experts)) for _ in range(L)]
+        out = sim.run_step(needed, [None] * L, stride=1)
+        for m in range(L):
+            rec = out[m][0]
+            assert rec.expert == needed[m]                      # launch order = ascending id
+            for i, e in enumerate(needed[m]):
+                hit, v = ref[m].access(e)
+                assert (rec.cls[i] == CLASS_A) == hit
+                if not hit:
+                    assert rec.victim[i] == (-1 if v is None else v)
+                    # the victim was launched earlier in this layer → its compute must finish first
+                    assert rec.dep[i] == (needed[m].index(v) if v in needed[m][:i] else -1)
+            assert sorted(x for x in sim.slot_expert[m] if x != EMPTY) == sorted(ref[m].d)
+    assert sim.stats.hits + sim.stats.misses == sim.stats.accesses == 200 * L * T_experts
+
+
+def test_id_order_thrashes_where_reorder_does_not():
+    """§5.3: slots {5,6,7,8} hold 5 (oldest) .. 8, the gate needs {1,5,6}.  Reordered: 5, 6 first (touched), then
+    1 evicts 7 → one miss.  ID order: 1 comes first and evicts 5 (the LRU entry, needed later), 5 then misses and evicts 6,
+    6 misses and evicts 7 → three misses for the same access set."""
+    def build(reorder):
+        sim = ProMoECacheSim(1, 16, 4, warm=False, reorder=reorder)
+        sim.begin_step()
+        sim.push_precise(0, [5]); sim.push_precise(0, [6]); sim.push_precise(0, [7]); sim.push_precise(0, [8])
+        sim.begin_step()
+        return sim
+    a = build(True)
+    ra = a.push_precise(0, [1, 5, 6])
+    assert ra.as_tuples() == [(5, CLASS_A, 0, -1, -1), (6, CLASS_A, 1, -1, -1), (1, CLASS_C, 2, 7, -1)]
+    b = build(False)
+    rb = b.push_precise(0, [1, 5, 6])
+    assert rb.as_tuples() == [(1, CLASS_C, 0, 5, -1), (5, CLASS_C, 1, 6, -1), (6, CLASS_C, 2, 7, -1)]
+    assert b.stats.misses - 4 == 3 and a.stats.misses - 4 == 1
+    assert b.stats.need_experts == a.stats.need_experts            # B_need = the reorder-achievable minimum either way
+
+
+# ---- demote = True: a mispredicted prefetch becomes the next victim (DESIGN.md G17) ----------------------------------
+def test_demoted_misprediction_is_the_next_victim():
+    """4 slots hold 0 (oldest), 1, 2, 3.  Prediction {9} for the layer allocates over 0.  The gate then needs {1, 7}:
+    9 was NOT selected.  Paper behaviour (demote off): 9 stays most recently used, the miss 7 evicts 2 (1 was just
+    touched) — two useful experts lost to one wrong guess.  With demotion 9's slot is the victim of 7: only expert 0,
+    the LRU entry the next miss would have taken anyway, is lost."""
+    for demote, want_victim, want_set in ((False, 2, [1, 3, 7, 9]), (True, 9, [1, 2, 3, 7])):
+        sim = ProMoECacheSim(1, 16, 4, warm=True, demote=demote)
+        sim.begin_step()
+        pr = sim.push_predicted(0, [9], max_spec=1)
+        assert pr.as_tuples() == [(9, ACT_ALLOC, 0, 0)]
+        rec = sim.push_precise(0, [1, 7])
+        assert rec.as_tuples() == [(1, CLASS_A, 1, -1, -1), (7, CLASS_C, 0 if demote else 2, want_victim, -1)]
+        assert sorted(sim.slot_expert[0]) == want_set
+        assert sim.stats.predicted == 1 and sim.stats.predicted_correct == 0
+
+
+def test_demotion_leaves_correct_predictions_and_other_layers_alone():
+    """A correct prediction is class B (touched, kept); demotion happens at the slot's OWN gate only; two demoted slots
+    are taken in slot order (equal stamps → lowest slot index)."""
+    sim = ProMoECacheSim(2, 16, 4, warm=True, demote=True)
+    sim.begin_step()
+    sim.push_predicted(1, [9, 10, 11], max_spec=3)                 # layer 1: slots 0,1,2 ← 9,10,11 (PRED)
+    r0 = sim.push_precise(0, [0, 1])                                # the gate of layer 0 does not touch layer 1
+    assert [c for c in r0.cls] == [CLASS_A, CLASS_A]
+    assert sim.slot_expert[1][:3] == [9, 10, 11] and all(sim.stamp[1][s] > 0 for s in range(3))
+    r1 = sim.push_precise(1, [10, 12, 13])                          # 10 was right; 9 and 11 were not
+    assert r1.as_tuples() == [(10, CLASS_B, 1, -1, -1), (12, CLASS_C, 0, 9, -1), (13, CLASS_C, 2, 11, -1)]
+    assert sim.slot_expert[1] == [12, 10, 13, 3]
+    _check_invariants(sim)
+
+
+def test_demotion_never_changes_outputs_of_a_reactive_run():
+    """No predictions → no PRED slots → demotion is a no-op (same records, same tables)."""
+    rng = random.Random(3)
+    a, b = ProMoECacheSim(2, 12, 5), ProMoECacheSim(2, 12, 5, demote=True)
+    for _ in range(100):
+        needed = [sorted(rng.sample(range(12), 3)) for _ in range(2)]
+        ra, rb = a.run_step(needed, [None, None], 1), b.run_step(needed, [None, None], 1)
+        assert [x[0].as_tuples() for x in ra] == [x[0].as_tuples() for x in rb]
+    assert a.slot_expert == b.slot_expert and a.stamp == b.stamp
