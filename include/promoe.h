@@ -62,12 +62,18 @@ typedef struct {
 #define PROMOE_PRED_TRACE 2  /* injected prediction lists (oracle-routing upper bound) */
 /* flags */
 #define PROMOE_F_PREEMPT 1   /* early preemption: drop un-issued LOW chunks of a layer at its gate */
-#define PROMOE_F_REORDER 2   /* reordered inference: cached -> being prefetched -> missing.  ALWAYS ON in this version:
-                                the bit is accepted for ABI stability; the ID-order baseline is a later row */
+#define PROMOE_F_REORDER 2   /* reordered inference: cached -> being prefetched -> missing.  Clear = the ID-order baseline of
+                                the ablation (Fig. 12 "Base"): experts in ascending id, classified at their turn, plain
+                                LRU victim over all slots — a needed expert may be evicted before its turn (G16) */
 #define PROMOE_F_WARM 4      /* warm start: experts 0..C-1 resident in every layer (G4) */
 #define PROMOE_F_TRACE 8     /* record routing / permutation / cache traces for promoe_get_trace */
 #define PROMOE_F_NOFUSE 32  /* decode with the unfused per-op kernels (19 launches per layer) instead of the fused 7 */
 #define PROMOE_F_TENSOR 16   /* prefill GEMMs on tcgen05 tensor cores (bf16 weights only); else SIMT fp32 */
+#define PROMOE_F_DEMOTE 128  /* a predicted (PRED) slot whose expert its gate did not select gets the oldest LRU stamp at that gate: a
+                                misprediction costs one LRU victim instead of a most-recently-used slot (G17; not in the
+                                paper, which keeps mispredicted prefetches as ordinary cache entries) */
+#define PROMOE_F_TRACE_U 256  /* also record u_l, the post-attention RMSNorm output the router and the predictor of every MoE layer
+                                read (G6): PROMOE_TRACE_U — the input side of the predictor's offline training set */
 #define PROMOE_F_UNCHUNKED 64 /* ablation (Fig. 12 "+chunk" off): an expert image is copied all or nothing — one LOW
                                  copy per predicted expert, and a gate that finds a partial image fetches it again from byte 0 */
 
@@ -153,6 +159,7 @@ typedef struct {
 #define PROMOE_TRACE_HIDDEN 6    /* float [T, hidden]     residual stream after the full stack */
 #define PROMOE_TRACE_PREDLIST 7  /* int32 [n_moe, 1 + E]  n, list predicted BY the predictor at layer m (uncapped by G5) */
 #define PROMOE_TRACE_ZLOGITS 8   /* float [n_moe, T, E]   router logits */
+#define PROMOE_TRACE_U 9         /* float [n_moe, T, hidden]  u_l per MoE layer (needs PROMOE_F_TRACE_U) */
 
 PROMOE_API int promoe_create(const promoe_shape_t* shape, const promoe_opts_t* opts, promoe_t** out);
 PROMOE_API void promoe_destroy(promoe_t* h);

@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libpromoe.so")
 PROMOE_OK, PROMOE_EINVAL, PROMOE_ENOMEM, PROMOE_ECUDA, PROMOE_ESTATE, PROMOE_ETIMEOUT = 0, -1, -2, -3, -4, -5
 PRED_NONE, PRED_MLP, PRED_TRACE = 0, 1, 2
 F_PREEMPT, F_REORDER, F_WARM, F_TRACE, F_TENSOR, F_NOFUSE = 1, 2, 4, 8, 16, 32
-TRACE_SEL, TRACE_GATES, TRACE_MARGIN, TRACE_PERM, TRACE_PRECISE, TRACE_PRED, TRACE_HIDDEN, TRACE_PREDLIST, TRACE_ZLOGITS = range(9)
+F_UNCHUNKED, F_DEMOTE, F_TRACE_U = 64, 128, 256
+TRACE_SEL, TRACE_GATES, TRACE_MARGIN, TRACE_PERM, TRACE_PRECISE, TRACE_PRED, TRACE_HIDDEN, TRACE_PREDLIST, TRACE_ZLOGITS, TRACE_U = range(10)
 
 EXPORTS = [
     "promoe_create", "promoe_destroy", "promoe_last_error", "promoe_load_dense", "promoe_load_experts",

@@ -78,6 +78,10 @@ extern "C" int promoe_get_trace(promoe_t* h, int which, const void** data, size_
     case PROMOE_TRACE_PREDLIST:
       n = (size_t)Lm * (1 + E) * 4; h->trace_buf.resize(n);
       CKA(cudaMemcpy(h->trace_buf.data(), h->pred_list, n, cudaMemcpyDeviceToHost)); break;
+    case PROMOE_TRACE_U:
+      if (!h->trace_u) { h->err = "get_trace: PROMOE_TRACE_U needs PROMOE_F_TRACE_U at create"; return PROMOE_ESTATE; }
+      n = (size_t)Lm * T * H * 4; h->trace_buf.resize(n);
+      rc = gather_rows(h, h->trace_u, Lm, (size_t)T * H * 4, mT * H * 4, 0); break;
     case PROMOE_TRACE_HIDDEN:
       n = (size_t)T * H * 4; h->trace_buf.resize(n);
       CKA(cudaMemcpy(h->trace_buf.data(), h->x, n, cudaMemcpyDeviceToHost)); break;

@@ -108,6 +108,7 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->ids, (size_t)T));
     CK(dalloc(&h->sel, (size_t)Lm * T * k)); CK(dalloc(&h->gates, (size_t)Lm * T * k)); CK(dalloc(&h->margin, (size_t)Lm * T));
     CK(dalloc(&h->z, (size_t)Lm * T * E));
+    if (op->flags & PROMOE_F_TRACE_U) CK(dalloc(&h->trace_u, (size_t)Lm * T * H));
     CK(dalloc(&h->count, (size_t)Lm * E)); CK(dalloc(&h->offset, (size_t)Lm * (E + 1)));
     CK(dalloc(&h->perm, (size_t)Lm * T * k)); CK(dalloc(&h->inv, (size_t)Lm * T * k));
     CK(dalloc(&h->pred_list, (size_t)Lm * (1 + E))); CK(dalloc(&h->trace_precise, (size_t)Lm * (1 + 5 * E)));
@@ -181,7 +182,7 @@ extern "C" void promoe_destroy(promoe_t* h) {
                   h->count, h->offset, h->perm, h->inv, h->gates, h->margin, h->z, h->pred_list, h->trace_precise,
                   h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->attn_cnt, h->slots, h->flags,
                   h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock,
-                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch};
+                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch, h->trace_u};
   for (void* b : bufs) if (b) cudaFree(b);
   if (h->xsA) cudaFree(h->xsA);
   if (h->xsG) cudaFree(h->xsG);

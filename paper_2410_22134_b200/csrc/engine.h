@@ -69,6 +69,7 @@ struct promoe {
   // per-MoE-layer routing / permutation buffers (double as traces)
   int32_t *sel = nullptr, *count = nullptr, *offset = nullptr, *perm = nullptr, *inv = nullptr;
   float *gates = nullptr, *margin = nullptr, *z = nullptr;
+  float* trace_u = nullptr;               // [Lm, maxT, H] with PROMOE_F_TRACE_U, else nullptr
   int32_t *pred_list = nullptr, *trace_precise = nullptr, *trace_pred = nullptr, *row_of = nullptr,
           *n_prob = nullptr;
   pmk::FfnProblem *problems = nullptr, *shared_prob = nullptr;

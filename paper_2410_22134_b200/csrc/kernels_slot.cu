@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
                                                          int inter, int wbytes, FfnProblem* problems,
                                                          int32_t* n_problems, int32_t* row_of, LayerCmd* cmd,
                                                          uint32_t seq, int32_t* trace_precise,
-                                                         int32_t* trace_pred, RouteFuse rf, LayerCmd* cmd2) {
+                                                         int32_t* trace_pred, RouteFuse rf, LayerCmd* cmd2, int mode) {
   __shared__ uint8_t needed[kMaxE];
   __shared__ uint8_t prot[kMaxE];
   __shared__ int16_t order[kMaxE];
@@ -123,7 +123,41 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   if (T == 1 && threadIdx.x < k) s_sel1[threadIdx.x] = sel[threadIdx.x];
   for (int i = threadIdx.x; i < T * k; i += blockDim.x) { const int e = sel[i]; needed[e] = 1; prot[e] = 1; }   // same-value writes
   __syncthreads();
-  if (threadIdx.x == 0) {
+  // G17 (mode bit 1): a PRED slot whose expert this gate did not select is a misprediction → stamp 0, the next victim
+  if (mode & 2)
+    for (int i = threadIdx.x; i < C; i += blockDim.x)
+      if (t_org[0][i] == 1 && t_se[0][i] >= 0 && !needed[t_se[0][i]]) t_stamp[0][i] = 0;
+  __syncthreads();
+  int n_built = 0;
+  if (threadIdx.x == 0 && !(mode & 1)) {
+    // G16: ID-order baseline (Fig. 12 "Base"): ascending id, classified at its turn, plain LRU victim over ALL
+    // slots — a needed expert may lose its slot before its turn and is then fetched again (§5.3)
+    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
+    int n = 0;
+    for (int e = 0; e < E; ++e) if (needed[e]) order[n++] = e;
+    if (trace_precise) trace_precise[0] = n;
+    for (int e = 0; e < E; ++e) prot[e] = 0;
+    for (int i = 0; i < n; ++i) {
+      const int e = order[i];
+      int32_t* r = rec + 7 * i;
+      int sl = v.expert_slot[e];
+      if (sl >= 0) {
+        cls[i] = v.origin[sl] == 1 ? 1 : 0;
+        v.touch(sl);
+        r[0] = e; r[1] = cls[i]; r[2] = sl; r[3] = -1; r[4] = -1; r[5] = (int32_t)v.gen[sl];
+      } else {
+        cls[i] = 2;
+        sl = v.victim(prot);
+        const int held = v.slot_expert[sl];
+        int dep = -1;
+        if (held >= 0) for (int q = 0; q < i; ++q) if (order[q] == held) dep = q;
+        const int old = v.install(sl, e, 2);
+        r[0] = e; r[1] = 2; r[2] = sl; r[3] = old; r[4] = dep; r[5] = (int32_t)v.gen[sl];
+      }
+    }
+    n_built = n;        // hand-over to the common tail below
+  }
+  if (threadIdx.x == 0 && (mode & 1)) {
     SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
     // classes A (cached) → B (being prefetched) → C (not begun), ascending id inside
     int n = 0;
@@ -169,6 +203,11 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
       int32_t* r = rec + 7 * i;
       r[0] = e; r[1] = 2; r[2] = sl; r[3] = old; r[4] = dep; r[5] = (int32_t)v.gen[sl];
     }
+    n_built = n;
+  }
+  if (threadIdx.x == 0) {
+    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
+    const int n = n_built;
     for (int sl = 0; sl < C; ++sl) v.origin[sl] = 0;
     // problem table + decode row map + trace
     const size_t hi = (size_t)H * inter * wbytes;
@@ -325,12 +364,12 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
                        int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf, LayerCmd* cmd_dev2) {
   ++g_launches;
-  (void)reorder;
+  const int mode = reorder;     // bit 0: reordered inference / 0 = ID order (G16); bit 1: demote mispredictions (G17)
   RouteFuse f{};
   if (rf) f = *rf;
   launch_pdl(slot_table_kernel, dim3(1), dim3((rf && T == 1) ? 1024 : 256), 0, st, tbl, m, stride, max_spec, sel, T, k, offset, pred_list,
              slot_base, slot_bytes, flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of, cmd, seq,
-             trace_precise, trace_pred, f, cmd_dev2);
+             trace_precise, trace_pred, f, cmd_dev2, mode);
 }
 
 // Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every

@@ -142,6 +142,9 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   if (mlp) b.seg[b.nseg++] = GemvSeg{h->pred_w1[l], h->p1, s.pred_hidden, LIN_RELU};
   if (s.n_shared_inter && s.shared_gate) b.seg[b.nseg++] = GemvSeg{h->shared_gate_w[l], h->sgate, 1, 0};
   launch_norm_multi_gemv(b, wd, cs);
+  if (h->trace_u && cudaMemcpyAsync(h->trace_u + (size_t)m * h->maxT * H, h->u, (size_t)H * 4, cudaMemcpyDeviceToDevice, cs) != cudaSuccess) {
+    h->err = "trace copy of u failed"; return PROMOE_ECUDA;
+  }
   // The shared expert (resident weights, needs only u) runs on a side stream BESIDE the single-CTA slot-table kernel
   // and the host hand-over instead of behind them; K7 joins it.  (Ordering of sact / sy / u across layers: the fork
   // event of the next layer is recorded after this layer's K7, which has waited for the join event.)
@@ -160,7 +163,7 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   rf.p1 = h->p1; rf.pred_w2 = mlp ? h->pred_w2[l] : nullptr; rf.ph = s.pred_hidden; rf.wdtype = wd;
   rf.pred_out = mlp ? plist : nullptr; rf.k = k; rf.cap = C;
   launch_slot_table(h->tbl, m, h->o.stride, h->max_spec_decode, sel, 1, k, nullptr, plist,
-                    (h->o.flags & PROMOE_F_REORDER) != 0, h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb, h->problems,
+                    ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb, h->problems,
                     h->n_prob, h->row_of, h->cmd_dev + m, seq, h->trace_precise + (size_t)m * (1 + 5 * E),
                     (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf, h->cmd_fetch + m);
   // A7 runs beside this stream: the fetch worker (kernels_fetch.cu, resident since the start of the step) sees the
@@ -323,6 +326,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     }
     // ---- MoE block
     const int m = l - s.n_dense_layers;
+    if (h->trace_u) CKS(cudaMemcpyAsync(h->trace_u + (size_t)m * h->maxT * H, h->u, (size_t)T * H * 4, cudaMemcpyDeviceToDevice, cs));
     const uint32_t seq = step_seq * 4096u + (uint32_t)m + 1u;
     int32_t* sel = h->sel + (size_t)m * h->maxT * k;
     float* gates = h->gates + (size_t)m * h->maxT * k;
@@ -351,7 +355,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     }
     if (T > 1) launch_permute(sel, T, k, E, h->count + (size_t)m * E, offset, perm, inv, cs);   // A8
     launch_slot_table(h->tbl, m, h->o.stride, T == 1 ? h->max_spec_decode : h->max_spec_prefill, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
-                      (h->o.flags & PROMOE_F_REORDER) != 0, h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb,
+                      ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb,
                       h->problems, h->n_prob, h->row_of, h->cmd_dev + m, seq,
                       h->trace_precise + (size_t)m * (1 + 5 * E),
                       (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs);

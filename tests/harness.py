@@ -33,7 +33,8 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
                  max_spec_decode=max_spec_decode, max_spec_prefill=max_spec_prefill)
     use_pred = predictor_mode == B.PRED_MLP
     ora = OracleModel(weights, stride=stride, slots_per_layer=C, use_predictor=use_pred)
-    sim = ProMoECacheSim(n_moe, s.n_experts, C, warm=bool(flags & B.F_WARM))
+    sim = ProMoECacheSim(n_moe, s.n_experts, C, warm=bool(flags & B.F_WARM), reorder=bool(flags & B.F_REORDER),
+                         demote=bool(flags & B.F_DEMOTE))
     rep = ParityReport()
     # library defaults (include/promoe.h): decode top_k allocations per push, prefill none
     ms_dec = s.top_k if max_spec_decode == 0 else max(0, max_spec_decode)

@@ -93,6 +93,33 @@ def test_config1b_tcgen05():
     assert out["report"].max_hidden_ratio <= 1.0
 
 
+@pytest.mark.parametrize("name,T", [("c1", 32), ("c1b", 32), ("c4-mini", 40), ("c2-mini", 64)])
+@pytest.mark.parametrize("mode", ["id_order", "id_order_reactive", "demote", "unchunked", "no_preempt", "demote_spec_all"])
+def test_ablation_modes(name, T, mode):
+    """SURVEY N2 / PAPER.md §7.3: every rung of the ablation ladder is a runtime mode whose traces are still
+    bit-exact against O3 driven the same way — ID-order LRU without reordered inference (G16; c4-mini: |needed| > C, so a
+    needed expert is evicted before its turn and fetched again), un-chunked prefetch, no early preemption — and the
+    demotion of mispredicted prefetches (G17)."""
+    from paper_2410_22134_b200 import binding as B
+    from synth.configs import mini
+    cfg = mini(name[:-5]) if name.endswith("-mini") else synth.get_config(name)
+    w = synth.make_weights(cfg, predictor="skip")
+    base = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | (B.F_TENSOR if cfg.shape.wdtype == 1 else 0)
+    flags, pm, ms = {
+        "id_order": (base & ~B.F_REORDER, B.PRED_MLP, 0),
+        "id_order_reactive": (base & ~B.F_REORDER, B.PRED_NONE, 0),
+        "demote": (base | B.F_DEMOTE, B.PRED_MLP, 1),
+        "demote_spec_all": (base | B.F_DEMOTE, B.PRED_MLP, 0),
+        "unchunked": (base | B.F_UNCHUNKED, B.PRED_MLP, 0),
+        "no_preempt": (base & ~B.F_PREEMPT, B.PRED_MLP, 0),
+    }[mode]
+    ids = synth.make_decode_ids(cfg, 8).tolist()
+    out = run_parity(cfg, w, synth.make_prompt(cfg, T), 8, flags=flags, predictor_mode=pm, decode_ids=ids,
+                     max_spec_decode=ms, max_spec_prefill=2 if mode.startswith("demote") else 0)
+    _report(f"{name}/{mode}", out)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+
+
 def test_injected_prediction_trace():
     """predictor_mode TRACE with the true routing of layer m+stride (oracle-routing upper bound): no class-C
     miss in layers >= stride during decode when C >= k."""
@@ -183,7 +210,10 @@ def test_outputs_independent_of_cache_parameters():
     variants = [dict(cache_slots=4), dict(cache_slots=8, stride=2), dict(cache_slots=8, chunk_bytes=1 << 14),
                 dict(cache_slots=12, predictor_mode=B.PRED_NONE), dict(cache_slots=8, flags=B.F_REORDER | B.F_TRACE),
                 dict(cache_slots=4, chunk_bytes=1 << 18, max_inflight=1), dict(cache_slots=8, chunk_bytes=1 << 16, high_group=2),
-                dict(cache_slots=8, chunk_bytes=1 << 16, low_cap_chunks=2, max_inflight=1)]
+                dict(cache_slots=8, chunk_bytes=1 << 16, low_cap_chunks=2, max_inflight=1),
+                dict(cache_slots=8, flags=B.F_PREEMPT | B.F_WARM | B.F_TRACE),                       # ID order (no reorder)
+                dict(cache_slots=4, flags=B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TRACE | B.F_DEMOTE),
+                dict(cache_slots=8, flags=B.F_REORDER | B.F_WARM | B.F_TRACE | B.F_UNCHUNKED)]
     for kw in variants:
         out = run_gpu_only(cfg, w, prompt, ids, **kw)
         for a, b in zip(base["logits"], out["logits"]):

@@ -296,3 +296,30 @@ def test_random_predictor_accuracy_near_chance_and_skip_beats_it():
         acc[variant] = sim.stats.predicted_correct / sim.stats.predicted
     assert abs(acc["random"] - 2 / 8) < 0.12        # ≈ k/E
     assert acc["skip"] > acc["random"] + 0.15
+
+
+def test_fit_predictor_improves_on_its_start_point_cpu():
+    """paper_2410_22134_b200/fit_predictor.py (P:159-161, 9:1 split): on synthetic traces whose target routing is a FIXED
+    linear map of u that differs from the start point's, the fitted MLP must beat the start point on the held-out split,
+    and the weights it returns must reproduce the accuracy it reports (rounded to bf16, as the GPU sees them)."""
+    from paper_2410_22134_b200.fit_predictor import fit_layer, topk_accuracy
+    g = torch.Generator().manual_seed(5)
+    N, H, E, k, ph = 3000, 64, 16, 2, 64
+    u = torch.randn(N, H, generator=g)
+    R = torch.randn(E, H, generator=g) * H ** -0.5              # what the start point ("skip") assumes
+    M = torch.eye(H) + 0.8 * torch.randn(H, H, generator=g) * H ** -0.5
+    z = (u @ M.T) @ R.T                                          # what the target layer really computes
+    sel = z.topk(k, dim=1).indices
+    w1 = torch.zeros(ph, H); w1[:E] = R; w1[E:2 * E] = -R
+    w2 = torch.zeros(E, ph); w2[:, :E] = torch.eye(E); w2[:, E:2 * E] = -torch.eye(E)
+    r = fit_layer(u, sel, w1, w2, E, k, 1, seed=1, steps=200, lr=2e-3)
+    assert r["kept"] == "fitted" and r["acc_test_fitted"] > r["acc_test_skip"] + 0.05
+    assert r["n_train"] == 2700 and r["n_test"] == 300
+    tgt = torch.zeros(N, E); tgt.scatter_(1, sel, 1.0)
+    assert abs(topk_accuracy(u, w1, w2, tgt, k) - (0.9 * r["acc_train_skip"] + 0.1 * r["acc_test_skip"])) < 1e-6
+    # returned weights are already bf16-representable
+    assert torch.equal(r["w1"], r["w1"].to(torch.bfloat16).float())
+    # a start point that is already exact cannot be beaten: the layer keeps it
+    sel0 = (u @ R.T).topk(k, dim=1).indices
+    r0 = fit_layer(u, sel0, w1, w2, E, k, 0, seed=2, steps=40, lr=1e-4)
+    assert r0["acc_test_skip"] == 1.0 and r0["kept"] == "skip" and torch.equal(r0["w1"], w1)
