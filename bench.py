@@ -181,7 +181,7 @@ def workload_config(cfg, args):
                         f"prompt {cfg.prompt_len} + {cfg.decode_steps} decode",
             "cache_slots": cfg.cache_slots, "cache_fraction": cfg.slots_per_layer / s.n_experts, "stride": cfg.stride,
             "predictor": args.predictor, "decode_ids": args.decode, "chunk_bytes": args.chunk_kb << 10, "max_spec_decode": args.max_spec_decode,
-            "max_spec_prefill": args.max_spec_prefill, "low_cap_chunks": args.low_cap, "max_inflight": args.inflight, "fetch_ctas": args.fetch_ctas,
+            "max_spec_prefill": args.max_spec_prefill, "low_cap_chunks": args.low_cap, "max_inflight": args.inflight, "fetch_ctas": args.fetch_ctas, "demote": args.demote,
             "l2": "inputs larger than L2 (each request streams >> 126 MB of expert weights)"}
 
 
@@ -289,7 +289,7 @@ def run_ours(args, cfg, rank, world, dist):
     torch.cuda.set_device(local)
     peaks = load_peaks()
     s = cfg.shape
-    pred_kind = "skip" if args.predictor in ("none", "trace") else args.predictor
+    pred_kind = "skip" if args.predictor in ("none", "trace", "fitted") else args.predictor
     weights = replica_weights(cfg, pred_kind, local, world, dist)
     wb = 4 if s.wdtype == 0 else 2
     Be = 3 * s.hidden * s.expert_inter * wb
@@ -297,7 +297,12 @@ def run_ours(args, cfg, rank, world, dist):
     prompt = synth.make_prompt(cfg).tolist()
     decode_ids = synth.make_decode_ids(cfg).tolist()
     greedy = args.decode == "greedy"
-    flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | (B.F_TENSOR if args.tensor else 0)
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | (B.F_TENSOR if args.tensor else 0) | (B.F_DEMOTE if args.demote else 0)
+    fit_report = None
+    if args.predictor == "fitted":     # N1: the offline step of §4.3 on the model's own traces, before any timing
+        from paper_2410_22134_b200.fit_predictor import fit_predictor
+        fit_report = fit_predictor(weights, cfg, cfg.stride, n_prompts=args.fit_prompts, steps=args.fit_steps)
+        fit_report.pop("per_layer")
     inject = None
     if args.predictor == "trace":      # pass 0: reactive run that records the routing of every step
         rec_eng = ProMoE(weights, cache_slots=cfg.cache_slots, stride=cfg.stride, predictor_mode=B.PRED_NONE,
@@ -365,6 +370,11 @@ def run_ours(args, cfg, rank, world, dist):
                 "miss_rate": a["misses"] / acc,
                 "predictor_accuracy": a["predicted_correct"] / max(1, a["predicted"]),
                 "fetch_rate": a["fetched_at_gate"] / max(1, a["fetched_at_gate_of"]),
+                # partial-fetch form: chunks of the class-B images that had landed at their gate / chunks per image
+                "fetch_rate_chunks": a["landed_chunks_at_gate"] / max(1, a["landed_chunks_of"]),
+                "good_pred": a["predicted_correct"] / max(1, a["predicted"]) * a["fetched_at_gate"] / max(1, a["fetched_at_gate_of"]),
+                "good_pred_chunks": a["predicted_correct"] / max(1, a["predicted"]) * a["landed_chunks_at_gate"] / max(1, a["landed_chunks_of"]),
+                "pred_allocs": a["pred_allocs"], "low_bytes": a["low_bytes"], "low_bytes_useful": a["low_bytes_useful"],
                 "h2d_bytes_moved": a["h2d_bytes"], "h2d_bytes_needed": a["need_experts"] * Be,
                 "byte_efficiency": a["need_experts"] * Be / max(1, a["h2d_bytes"]),
                 "copy_busy_ms": a["copy_busy_ms"], "link_utilisation": a["h2d_bytes"] / 1e6 / max(1e-9, a["copy_busy_ms"]) / h2d_gbs,
@@ -467,7 +477,7 @@ def run_ours(args, cfg, rank, world, dist):
             "step_roofline": {"h2d_gbs_measured": h2d_gbs, "hbm_gbs": peaks["hbm_gbs"], "bf16_tflops": peaks["bf16_tflops_sustained"],
                               "peaks": peaks["source"], "decode": roof_dec, "prefill": roof_pre},
             "cache": {"decode": cs_dec, "prefill": cs_pre, "hidden_copy_fraction_decode": hidden},
-            "all_resident": allhit, "variants": variants, "cpu_baseline": cpu}
+            "all_resident": allhit, "variants": variants, "predictor_fit": fit_report, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
 
 
@@ -551,6 +561,88 @@ def run_sweep(args):
                       "compute_only_ms": {str(k): v for k, v in compute.items()}}), flush=True)
 
 
+def run_modes(args):
+    """--ladder: PAPER.md §7.3 / Fig. 12 — Base (LRU, ID order, no prefetch) → +prefetch (un-chunked, no early
+    preemption) → +chunked → +early preemption → +reordered inference, and this build's own additions (demotion of
+    mispredictions, the fitted predictor).  --goodpred: §4.1 Accuracy, FetchRate, GoodPred of the `skip` and the
+    fitted predictor at strides 1-3.  One request (after one warm-up request) per row, one JSON line per row."""
+    import dataclasses
+    import torch
+    import synth
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+    from paper_2410_22134_b200.fit_predictor import fit_predictor
+    torch.cuda.set_device(0)
+    over = {}
+    if args.prompt_len:
+        over["prompt_len"] = args.prompt_len
+    if args.decode_steps:
+        over["decode_steps"] = args.decode_steps
+    base = synth.get_config(args.config, **over)
+    s = base.shape
+    Be = 3 * s.hidden * s.expert_inter * (4 if s.wdtype == 0 else 2)
+    h2d = B.promoe_bench_h2d(256 << 20, 2, 5)
+    prompt = synth.make_prompt(base).tolist()
+    decode_ids = synth.make_decode_ids(base).tolist()
+    wcache = {}
+
+    def weights_for(stride, kind):
+        key = (stride, kind)
+        if key not in wcache:
+            cfg = dataclasses.replace(base, stride=stride)
+            first = next(iter(wcache.values()))[0] if wcache else None
+            w = synth.make_weights(cfg, predictor="skip", experts_buf=first.experts if first is not None else None,
+                                   fill_experts=first is None)
+            rep = None
+            if kind == "fitted":
+                rep = fit_predictor(w, cfg, stride, n_prompts=args.fit_prompts, steps=args.fit_steps)
+                rep.pop("per_layer")
+            wcache[key] = (w, rep)
+        return wcache[key]
+
+    P, R, D, U, TN, W = B.F_PREEMPT, B.F_REORDER, B.F_DEMOTE, B.F_UNCHUNKED, (B.F_TENSOR if args.tensor else 0), B.F_WARM
+    if args.ladder:
+        st = base.stride
+        rows = [("base: LRU, ID order, no prefetch", "none", st, W | TN, 0),
+                ("+prefetch (un-chunked, no preemption)", "skip", st, W | TN | U, args.max_spec_decode),
+                ("+chunked", "skip", st, W | TN, args.max_spec_decode),
+                ("+early preemption", "skip", st, W | TN | P, args.max_spec_decode),
+                ("+reordered inference (= ProMoE)", "skip", st, W | TN | P | R, args.max_spec_decode),
+                ("reordered, no prefetch (reactive)", "none", st, W | TN | P | R, 0),
+                ("ProMoE + demotion (G17)", "skip", st, W | TN | P | R | D, args.max_spec_decode),
+                ("ProMoE + demotion + fitted predictor", "fitted", st, W | TN | P | R | D, args.max_spec_decode)]
+    else:
+        rows = [(f"{kind} stride {st}", kind, st, W | TN | P | R | (D if args.demote else 0), args.max_spec_decode)
+                for st in (1, 2, 3) for kind in ("skip", "fitted")]
+    for label, kind, stride, flags, ms in rows:
+        w, rep = weights_for(stride, "fitted" if kind == "fitted" else "skip")
+        cfg = dataclasses.replace(base, stride=stride)
+        eng = ProMoE(w, cache_slots=cfg.cache_slots, stride=stride, chunk_bytes=args.chunk_kb << 10,
+                     predictor_mode=B.PRED_NONE if kind == "none" else B.PRED_MLP, flags=flags, max_inflight=args.inflight,
+                     max_spec_decode=ms, max_spec_prefill=args.max_spec_prefill, fetch_ctas=args.fetch_ctas)
+        run_request(eng, cfg, prompt, decode_ids, False)
+        r = run_request(eng, cfg, prompt, decode_ids, False)
+        eng.close()
+        d, p = r["dec"], r["pre"]
+        dec_s, pre_s = r["decode_ms"] / 1e3, r["prefill_ms"] / 1e3
+        acc = d["predicted_correct"] / max(1, d["predicted"])
+        fr = d["fetched_at_gate"] / max(1, d["fetched_at_gate_of"])
+        frc = d["landed_chunks_at_gate"] / max(1, d["landed_chunks_of"])
+        row = {"mode": label, "config": cfg.name, "stride": stride, "predictor": kind,
+               "decode_tokens_per_s": cfg.decode_steps / dec_s, "prefill_tokens_per_s": cfg.prompt_len / pre_s,
+               "decode_roofline_frac": d["need_experts"] * Be / (h2d * 1e9) / dec_s,
+               "prefill_roofline_frac": p["need_experts"] * Be / (h2d * 1e9) / pre_s,
+               "hit_rate": (d["hits_resident"] + d["hits_prefetch"]) / max(1, d["accesses"]),
+               "miss_rate_prefill": p["misses"] / max(1, p["accesses"]),
+               "accuracy": acc, "fetch_rate": fr, "fetch_rate_chunks": frc, "good_pred": acc * fr, "good_pred_chunks": acc * frc,
+               "need_mb_per_token": d["need_experts"] * Be / 1e6 / cfg.decode_steps,
+               "moved_mb_per_token": d["h2d_bytes"] / 1e6 / cfg.decode_steps,
+               "prefill_moved_gb": p["h2d_bytes"] / 1e9, "prefill_need_gb": p["need_experts"] * Be / 1e9,
+               "fit": rep}
+        print(json.dumps(row), flush=True)
+    print(json.dumps({"modes": "ladder" if args.ladder else "goodpred", "rows": len(rows), "h2d_gbs": h2d}), flush=True)
+
+
 def spawn_command(n_gpus: int, argv):
     """Command line that runs this script as n_gpus ranks on one node (127.0.0.1 rendezvous, a free port)."""
     import socket
@@ -566,8 +658,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c2")
-    ap.add_argument("--predictor", default="skip", choices=["skip", "random", "none", "trace"],
-                    help="skip: training-free MLP weights (default); none: reactive cache; trace: oracle-routing upper bound")
+    ap.add_argument("--predictor", default="skip", choices=["skip", "fitted", "random", "none", "trace"],
+                    help="skip: training-free MLP weights; fitted: the MLP fitted offline on the model's own traces (fit_predictor.py); "
+                         "none: reactive cache; trace: oracle-routing upper bound")
+    ap.add_argument("--demote", type=int, default=0, help="PROMOE_F_DEMOTE: a mispredicted prefetch becomes the next LRU victim (G17)")
+    ap.add_argument("--fit-prompts", type=int, default=16, help="--predictor fitted: prompts of prompt_len tokens to collect traces from")
+    ap.add_argument("--fit-steps", type=int, default=240, help="--predictor fitted: optimiser steps per layer")
+    ap.add_argument("--ladder", action="store_true", help="ablation ladder of PAPER.md §7.3 / Fig. 12 (one JSON line per rung)")
+    ap.add_argument("--goodpred", action="store_true", help="Accuracy / FetchRate / GoodPred of skip vs fitted at strides 1-3 (one JSON line per row)")
     ap.add_argument("--decode", default="random", choices=["random", "greedy"],
                     help="decode ids: seeded random (locality-neutral, default) or greedy argmax")
     ap.add_argument("--chunk-kb", type=int, default=0, help="chunk size in KiB: granularity of the ready flags, of LOW copies and of preemption (0 = library default 256)")
@@ -589,6 +687,9 @@ def main():
 
     if args.sweep:
         run_sweep(args)
+        return
+    if args.ladder or args.goodpred:
+        run_modes(args)
         return
     import synth
     over = {}

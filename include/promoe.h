@@ -204,6 +204,16 @@ PROMOE_API int promoe_op_route(const float* u, const void* router, const float* 
 PROMOE_API int promoe_op_permute(const int32_t* sel, int32_t T, int32_t k, int32_t E, int32_t* count, int32_t* offset,
                       int32_t* perm, int32_t* inv, void* stream);
 
+/* attention rows A2 + A3 on caller-provided DEVICE buffers: rotate-half RoPE on q and k (tables cos_t / sin_t
+ * [max_seq, d/2] fp32, angle = pos * theta^(-2i/d), G11), KV append at positions pos0 .. pos0+T-1, then causal attention of
+ * the T new rows over cache positions 0 .. pos0+t.  qkv [T, (nq + 2 nkv) d] fp32 (rows: q heads | k heads | v heads; q and k
+ * are rotated in place when T > 1); kcache / vcache [nkv, max_seq, d] fp32; out [T, nq d].  T == 1 runs the fused decode
+ * kernel of the step and needs ws (nq * 16 * (d + 2) floats) and counters (nq int32, zero on entry, left zero); T > 1 runs the
+ * prefill kernels (ws / counters may be NULL).  d in {64, 128}; nq a multiple of nkv (GQA). */
+PROMOE_API int promoe_op_attention(float* qkv, const float* cos_t, const float* sin_t, float* kcache, float* vcache,
+                                   float* out, float* ws, int32_t* counters, int32_t T, int32_t pos0, int32_t nq,
+                                   int32_t nkv, int32_t d, int32_t max_seq, void* stream);
+
 /* expert FFN row A9 on one resident weight set: y[T,H] = Wd.(silu(Wg.x) * (Wu.x)); x [T,H], act_ws [T,I] scratch,
  * prob_ws >= 64 bytes of device scratch (problem record).  path: 0 auto, 1 HBM-streaming GEMV (T == 1),
  * 2 SIMT grouped GEMM, 3 tcgen05 grouped GEMM (bf16 weights). */

@@ -31,6 +31,7 @@ from typing import Dict, List, Optional, Tuple
 import torch
 
 from .predictor import predict_experts, predictor_scores, topk_desc
+from .quant import dequant_expert
 
 F64 = torch.float64
 
@@ -156,7 +157,10 @@ class OracleModel:
             for j, e in enumerate(sel[t]):
                 by_expert.setdefault(e, []).append((t, j))
         for e, pairs in sorted(by_expert.items()):
-            wg, wu, wd = self.w.expert_views(m, e)
+            if s.wdtype == 2:      # INT4 experts: dequantise, then the plain definition
+                wg, wu, wd = dequant_expert(self.w.experts[m, e], s.hidden, s.expert_inter)
+            else:
+                wg, wu, wd = self.w.expert_views(m, e)
             rows = torch.tensor([t for t, _ in pairs])
             out = swiglu_ffn(u[rows], wg, wu, wd)
             for i, (t, j) in enumerate(pairs):

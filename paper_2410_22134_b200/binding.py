@@ -26,6 +26,7 @@ EXPORTS = [
     "promoe_prefill", "promoe_decode", "promoe_set_prediction_trace", "promoe_stats", "promoe_get_trace",
     "promoe_reset", "promoe_get_slots", "promoe_op_linear", "promoe_op_route",
     "promoe_op_permute", "promoe_op_expert_ffn", "promoe_op_expert_ffn_static", "promoe_op_expert_ffn_static_max_inter",
+    "promoe_op_attention",
 ]
 BENCH_EXPORTS = ["promoe_bench_h2d", "promoe_bench_kernel_time"]   # include/promoe_bench.h (bench.py only)
 
@@ -101,6 +102,7 @@ def lib() -> C.CDLL:
     L.promoe_op_route.argtypes = [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_permute.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
     L.promoe_op_expert_ffn.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
+    L.promoe_op_attention.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp]
     L.promoe_op_expert_ffn_static.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, vp]
     L.promoe_op_expert_ffn_static_max_inter.argtypes = []
     L.promoe_bench_kernel_time.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]

@@ -190,3 +190,21 @@ extern "C" int promoe_op_expert_ffn(const float* x, const void* wg, const void* 
   return launch_status();
 }
 
+
+// A2 + A3 on caller buffers: RoPE on q and k (rotate-half), KV append at positions pos0 .. pos0+T-1, attention over the
+// cache.  T == 1 runs the fused decode kernel of the step (split over positions, last-CTA merge), T > 1 the prefill kernels.
+extern "C" int promoe_op_attention(float* qkv, const float* cos_t, const float* sin_t, float* kcache, float* vcache,
+                                   float* out, float* ws, int32_t* counters, int32_t T, int32_t pos0, int32_t nq,
+                                   int32_t nkv, int32_t d, int32_t max_seq, void* stream) {
+  if (!qkv || !cos_t || !sin_t || !kcache || !vcache || !out || T < 1 || pos0 < 0 || pos0 + T > max_seq) return PROMOE_EINVAL;
+  if ((d != 64 && d != 128) || nq < 1 || nkv < 1 || nq % nkv) return PROMOE_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (T == 1) {
+    if (!ws || !counters) return PROMOE_EINVAL;
+    launch_attn_decode_fused(qkv, cos_t, sin_t, kcache, vcache, ws, out, counters, pos0, nq, nkv, d, max_seq, 16, st);
+  } else {
+    launch_rope_append(qkv, cos_t, sin_t, kcache, vcache, T, pos0, nq, nkv, d, max_seq, st);
+    launch_attn_prefill(qkv, kcache, vcache, out, T, pos0, nq, nkv, d, max_seq, st);
+  }
+  return launch_status();
+}

@@ -30,7 +30,7 @@ class Shape:
     dense_inter: int = 0
     router_bias: int = 0        # c3: per-expert logit bias
     pred_hidden: int = 128
-    wdtype: int = 1             # 0 fp32 (c1), 1 bf16
+    wdtype: int = 1             # 0 fp32 (c1), 1 bf16, 2 bf16 with INT4 group-quantised routed experts
     rope_theta: float = 10000.0
     rms_eps: float = 1e-6
 
@@ -60,7 +60,12 @@ def expert_elems(s: Shape) -> int:
     return 3 * s.hidden * s.expert_inter
 
 
+INT4_GROUP = 128   # elements per quantisation group (along the reduction dimension)
+
+
 def expert_bytes(s: Shape) -> int:
+    if s.wdtype == 2:   # 4-bit codes, two per byte, + one bf16 scale per group of 128
+        return expert_elems(s) // 2 + expert_elems(s) // INT4_GROUP * 2
     return expert_elems(s) * (4 if s.wdtype == 0 else 2)
 
 

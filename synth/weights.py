@@ -17,6 +17,14 @@ Each routed expert is ONE contiguous image [Wgate (I×H) | Wup (I×H) | Wdown (H
 all images live in one [n_moe_layers, E, 3·H·I] host tensor, pinned when CUDA is present ("routed experts live in
 pinned host memory", BASELINE.json configs[1]).
 
+INT4 experts (shape.wdtype == 2, PAPER.md P:313 / §7.6 P:417-433 — the paper's QW-2 and Mixt run GPTQ-style
+4-bit experts): the routed experts are drawn as above (bf16) and then packed by `pack_int4` — the stand-in for the
+offline quantiser, an input-preparation step: per row, groups of 128 consecutive elements of the reduction dimension share
+one bf16 scale = max|w| / 7 of the group (1 for an all-zero group); code = clamp(round_half_even(w / scale), −8, 7) + 8,
+two codes per byte (even element in the low nibble).  Image = [gate codes | up codes | down codes | gate scales | up
+scales | down scales] (uint8).  The dense weights of such a model stay bf16.  Dequantisation — value = (code − 8)·scale —
+is method arithmetic and lives on the two sides separately (oracle/quant.py; csrc/kernels_q4.cu).
+
 Large tensors are drawn with torch's CUDA Philox generator when a GPU is present (25-90 GB of normals are too slow
 on the host); small configs always use the CPU generator so CPU-only tests see the same values everywhere.
 """
@@ -29,7 +37,7 @@ from typing import Dict, List, Optional
 
 import torch
 
-from .configs import RunConfig, Shape, expert_elems, moe_layer_ids
+from .configs import INT4_GROUP, RunConfig, Shape, expert_bytes, expert_elems, moe_layer_ids
 
 _GPU_GEN_THRESHOLD = 1 << 26   # tensors above 64 Mi elements are drawn on the GPU when there is one
 
@@ -57,6 +65,21 @@ def _normal(seed: int, name: str, shape, std: float, dtype: torch.dtype, out: Op
     return t.cpu()
 
 
+def pack_int4(w: torch.Tensor, group: int = 128):
+    """w [..., N, K] float (K a multiple of `group`) → (codes uint8 [..., N, K/2], scales bf16 [..., N, K/group])."""
+    shp = w.shape
+    K = shp[-1]
+    assert K % group == 0
+    g = w.to(torch.float32).reshape(*shp[:-1], K // group, group)
+    amax = g.abs().amax(dim=-1, keepdim=True)
+    scale = (amax / 7.0).to(torch.bfloat16)
+    scale = torch.where(scale.to(torch.float32) == 0, torch.ones_like(scale), scale)
+    code = torch.clamp(torch.round(g / scale.to(torch.float32)), -8, 7).to(torch.int16) + 8
+    code = code.reshape(*shp[:-1], K // 2, 2)
+    packed = (code[..., 0] | (code[..., 1] << 4)).to(torch.uint8)
+    return packed, scale.reshape(*shp[:-1], K // group)
+
+
 @dataclass
 class Weights:
     shape: Shape
@@ -66,8 +89,11 @@ class Weights:
     stride: int = 1
 
     def expert_views(self, m: int, e: int):
-        """(Wgate [I,H], Wup [I,H], Wdown [H,I]) views of routed expert e of MoE layer m."""
+        """(Wgate [I,H], Wup [I,H], Wdown [H,I]) views of routed expert e of MoE layer m (fp32 / bf16 images; an INT4
+        image is raw bytes — the oracle unpacks it itself, oracle/quant.py)."""
         s = self.shape
+        if s.wdtype == 2:
+            raise TypeError("INT4 expert images have no tensor views: unpack self.experts[m, e] (uint8)")
         img = self.experts[m, e]
         hi = s.hidden * s.expert_inter
         return (img[:hi].view(s.expert_inter, s.hidden),
@@ -81,7 +107,7 @@ def make_weights(cfg: RunConfig, predictor: str = "skip", pin: Optional[bool] = 
     node); fill_experts=False: the buffer already holds the values (another rank drew them)."""
     s = cfg.shape
     seed = cfg.seed
-    dt = torch.float32 if s.wdtype == 0 else torch.bfloat16
+    dt = torch.float32 if s.wdtype == 0 else torch.bfloat16     # dense weights (wdtype 2: bf16 dense, INT4 experts)
     H, d = s.hidden, s.head_dim
     nq, nkv = s.n_q_heads, s.n_kv_heads
     D: Dict[str, torch.Tensor] = {}
@@ -144,19 +170,30 @@ def make_weights(cfg: RunConfig, predictor: str = "skip", pin: Optional[bool] = 
 
     # routed experts: one contiguous host tensor, pinned if possible
     n_moe = s.n_moe_layers
-    per = expert_elems(s)
+    q4 = s.wdtype == 2
+    per = expert_bytes(s) if q4 else expert_elems(s)
+    edt = torch.uint8 if q4 else dt
     if pin is None:
         pin = torch.cuda.is_available()
     if experts_buf is not None:
-        assert tuple(experts_buf.shape) == (n_moe, E, per) and experts_buf.dtype == dt
+        assert tuple(experts_buf.shape) == (n_moe, E, per) and experts_buf.dtype == edt
         experts = experts_buf
     else:
-        experts = torch.empty((n_moe, E, per), dtype=dt, pin_memory=bool(pin))
+        experts = torch.empty((n_moe, E, per), dtype=edt, pin_memory=bool(pin))
     hi = H * s.expert_inter
     for mi, l in enumerate(moe_ids if fill_experts else []):
         # gate/up rows have fan-in H, down rows fan-in I; one draw per (layer, matrix) over all experts
         for k, (name, std) in enumerate((("gate", H ** -0.5), ("up", H ** -0.5), ("down", s.expert_inter ** -0.5))):
-            _normal(seed, f"l{l}.experts.{name}", (E, hi), std, dt, out=experts[mi, :, k * hi:(k + 1) * hi])
+            if not q4:
+                _normal(seed, f"l{l}.experts.{name}", (E, hi), std, dt, out=experts[mi, :, k * hi:(k + 1) * hi])
+                continue
+            dev = "cuda" if torch.cuda.is_available() and E * hi >= _GPU_GEN_THRESHOLD else "cpu"
+            w = _normal(seed, f"l{l}.experts.{name}", (E, hi), std, dt).to(dev)
+            kdim = H if k < 2 else s.expert_inter
+            codes, scales = pack_int4(w.view(E, hi // kdim, kdim), INT4_GROUP)
+            experts[mi, :, k * (hi // 2):(k + 1) * (hi // 2)].copy_(codes.reshape(E, hi // 2))
+            so = 3 * (hi // 2) + k * (hi // INT4_GROUP) * 2
+            experts[mi, :, so:so + (hi // INT4_GROUP) * 2].copy_(scales.reshape(E, hi // INT4_GROUP).contiguous().view(torch.uint8).reshape(E, -1))
     return Weights(shape=s, dense=D, experts=experts, predictor=predictor, stride=cfg.stride)
 
 

@@ -202,3 +202,49 @@ def test_op_expert_ffn_tcgen05(B, T, H, I):
     ref = swiglu_ffn(x.double(), wg, wu, wdn)
     err = (y.cpu().double() - ref).abs().max().item()
     assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
+
+
+# ---- A2 + A3: RoPE + KV append + attention, op level, against OracleModel._attention -------------------------------
+@pytest.mark.parametrize("nq,nkv,d,T0,n_dec", [(4, 4, 64, 70, 3),          # c1 head shape, two query tiles
+                                               (16, 16, 128, 900, 4),      # c2/c3 heads; decode beyond 768 positions (multi-round key loop)
+                                               (8, 2, 128, 2110, 3),       # GQA (c4 ratio); decode at positions 2110+ (c5's longest prompts)
+                                               (4, 4, 128, 1, 2)])         # T0 = 1: a one-token prefill, then decode at positions 1, 2
+def test_op_attention(B, nq, nkv, d, T0, n_dec):
+    """promoe_op_attention against the oracle's attention block: a T0-token causal prefill (several 64-row query tiles, a
+    ragged tail), then n_dec single-token steps through the fused decode kernel at positions T0, T0+1, ... — the paths
+    bench.py's prompt lengths reach (position > 768: the carried-(m, l) multi-round loop of the decode kernel)."""
+    import types
+    from oracle.forward import OracleModel
+    H = nq * d
+    qkv_w = (nq + 2 * nkv) * d
+    max_seq = T0 + n_dec
+    wqkv = _w((qkv_w, H), torch.float32, 31)
+    shape = types.SimpleNamespace(n_q_heads=nq, n_kv_heads=nkv, head_dim=d, n_layers=1, n_experts=1, rope_theta=10000.0)
+    weights = types.SimpleNamespace(shape=shape, dense={"l0.wqkv": wqkv, "l0.wo": torch.eye(H)})
+    ora = OracleModel(weights)
+    half = d // 2
+    ang = torch.arange(max_seq, dtype=torch.float64)[:, None] * (10000.0 ** (-2.0 * torch.arange(half, dtype=torch.float64) / d))[None, :]
+    cos_t, sin_t = torch.cos(ang).float().cuda(), torch.sin(ang).float().cuda()
+    kc = torch.zeros(nkv, max_seq, d, device="cuda"); vc = torch.zeros(nkv, max_seq, d, device="cuda")
+    ws = torch.zeros(nq * 16 * (d + 2), device="cuda"); cnt = torch.zeros(nq, dtype=torch.int32, device="cuda")
+    L = B.lib()
+    pos = 0
+    for step, T in enumerate([T0] + [1] * n_dec):
+        u1 = _w((T, H), torch.float32, 40 + step, 1.0)
+        qkv = (u1.double() @ wqkv.double().T).float().cuda()        # the projection is not under test here
+        out = torch.full((T, H), float("nan"), device="cuda")
+        rc = L.promoe_op_attention(qkv.data_ptr(), cos_t.data_ptr(), sin_t.data_ptr(), kc.data_ptr(), vc.data_ptr(),
+                                   out.data_ptr(), ws.data_ptr(), cnt.data_ptr(), T, pos, nq, nkv, d, max_seq, None)
+        assert rc == 0
+        torch.cuda.synchronize()
+        ref = ora._attention(0, u1.double())
+        ora.pos += T
+        pos += T
+        err = (out.cpu().double() - ref).abs().max().item()
+        assert err <= 2e-5 * max(1.0, ref.abs().max().item()), (step, err)
+        assert int(cnt.abs().sum()) == 0                             # the arrival counters are left zero
+    # the cache holds the rotated keys / raw values of every position
+    kref = torch.stack([ora.kcache[0][:, g, :] for g in range(nkv)])
+    assert (kc[:, :pos].cpu().double() - kref).abs().max().item() <= 1e-5 * max(1.0, kref.abs().max().item())
+    assert L.promoe_op_attention(qkv.data_ptr(), cos_t.data_ptr(), sin_t.data_ptr(), kc.data_ptr(), vc.data_ptr(), out.data_ptr(),
+                                 ws.data_ptr(), cnt.data_ptr(), 1, max_seq, nq, nkv, d, max_seq, None) == B.PROMOE_EINVAL

@@ -120,6 +120,28 @@ def test_ablation_modes(name, T, mode):
     assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
 
 
+def test_fitted_predictor_parity():
+    """the stride predictor fitted offline on the model's own traces (PROMOE_TRACE_U +
+    selections, 9:1 split) is at least as accurate as its `skip` start point on held-out tokens, and the step that runs
+    with the fitted weights is still bit-exact against the oracle given the same weights (demotion on, as bench.py runs it)."""
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.fit_predictor import fit_predictor
+    from synth.configs import mini
+    cfg = mini("c2")
+    w = synth.make_weights(cfg, predictor="skip")
+    rep = fit_predictor(w, cfg, cfg.stride, n_prompts=6, prompt_len=128, steps=80)
+    print({k: v for k, v in rep.items() if k != "per_layer"})
+    assert w.predictor == "fitted" and rep["tokens"] == 6 * 128 and rep["layers"] == cfg.shape.n_moe_layers - cfg.stride
+    assert rep["acc_test_fitted"] >= rep["acc_test_skip"] - 1e-9 or rep["layers_kept_fitted"] == 0
+    for r in rep["per_layer"]:
+        assert max(r["acc_test_fitted"], r["acc_test_skip"]) > 2.0 * cfg.shape.top_k / cfg.shape.n_experts   # far above chance
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR | B.F_DEMOTE
+    ids = synth.make_decode_ids(cfg, 8).tolist()
+    out = run_parity(cfg, w, synth.make_prompt(cfg, 64), 8, flags=flags, decode_ids=ids, max_spec_decode=1)
+    _report("c2-mini/fitted", out)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+
+
 def test_injected_prediction_trace():
     """predictor_mode TRACE with the true routing of layer m+stride (oracle-routing upper bound): no class-C
     miss in layers >= stride during decode when C >= k."""
@@ -284,3 +306,59 @@ def test_top_k_equals_n_experts():
     out = run_parity(cfg, w, synth.make_prompt(cfg, 21), 5)
     _report("c1 k=E", out)
     assert out["stats"]["misses"] == 0 and out["stats"]["h2d_bytes"] == 0
+
+
+# ---- parity at the sizes and in the kernel paths bench.py runs ("parity sizes do not reach the bench") ----
+def _long_cfg(name, n_layers, max_seq, **over):
+    from dataclasses import replace
+    from synth.configs import mini
+    cfg = mini(name)
+    shape = replace(cfg.shape, n_layers=n_layers, max_seq=max_seq)
+    per = over.pop("slots_per_layer", cfg.slots_per_layer)
+    return replace(cfg, shape=shape, cache_slots=per * shape.n_moe_layers, **over)
+
+
+@pytest.mark.parametrize("name,T,n_layers", [("c2", 512, 3), ("c3", 2048, 3)])
+def test_prefill_at_bench_prompt_lengths(name, T, n_layers):
+    """Prefill at the bench's own prompt lengths on the c2 / c3 layer shapes (reduced depth so the oracle stays under a
+    minute): T = 512 → 34 rows per expert, T = 2048 → 192 rows per expert, i.e. grouped tcgen05 launches with several
+    64-row tiles per problem (blockIdx.y > 0) and ragged last tiles; 8 / 32 query tiles in the prefill attention; the
+    permutation at T·k = 2048 / 12288; the slot table with every expert needed (|needed| > C: in-layer recycling)."""
+    from paper_2410_22134_b200 import binding as B
+    cfg = _long_cfg(name, n_layers, T + 8)
+    w = synth.make_weights(cfg, predictor="skip")
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR
+    ids = synth.make_decode_ids(cfg, 2).tolist()
+    out = run_parity(cfg, w, synth.make_prompt(cfg, T), 2, flags=flags, decode_ids=ids, max_spec_decode=1)
+    _report(f"{name} prefill T={T}", out)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+
+
+@pytest.mark.parametrize("name,T0", [("c2", 800), ("c2", 1296), ("c3", 2100)])
+def test_decode_at_long_positions(name, T0):
+    """Decode at positions 800+, 1296+ and 2100+ (bench: c2 512-640, c3 1024-1280, c5 up to 2304) on a 2-layer model whose
+    KV cache is seeded by a long prefill: the fused decode attention runs its multi-round key loop (n_pos > 768) and
+    every split carries (m, l) across rounds."""
+    from paper_2410_22134_b200 import binding as B
+    cfg = _long_cfg(name, 2, T0 + 8)
+    w = synth.make_weights(cfg, predictor="skip")
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR
+    ids = synth.make_decode_ids(cfg, 5).tolist()
+    out = run_parity(cfg, w, synth.make_prompt(cfg, T0), 5, flags=flags, decode_ids=ids, max_spec_decode=1)
+    _report(f"{name} decode at {T0}+", out)
+    assert out["report"].steps == 6 and out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+
+
+@pytest.mark.parametrize("budget,stride", [(0.25, 2), (0.25, 3), (0.75, 2), (0.75, 3), (0.5, 1)])
+def test_c5_budgets_and_strides_on_c3_shape(budget, stride):
+    """BASELINE.json configs[4]: the c3 layer shape at 25 % / 75 % budget (16 / 48 slots of 64) with strides 2 and 3 —
+    6 layers (1 dense + 5 MoE) so that stride 3 still has two predicted layers; 128-token prompt + 8 decode steps."""
+    from paper_2410_22134_b200 import binding as B
+    cfg = _long_cfg("c3", 6, 160, slots_per_layer=int(64 * budget), stride=stride)
+    w = synth.make_weights(cfg, predictor="skip")
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR
+    ids = synth.make_decode_ids(cfg, 8).tolist()
+    out = run_parity(cfg, w, synth.make_prompt(cfg, 128), 8, flags=flags, decode_ids=ids, stride=stride, max_spec_decode=1)
+    _report(f"c3-shape budget {budget} stride {stride}", out)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+    assert out["stats"]["pred_allocs"] > 0
