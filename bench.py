@@ -662,7 +662,7 @@ def main():
                     help="skip: training-free MLP weights; fitted: the MLP fitted offline on the model's own traces (fit_predictor.py); "
                          "none: reactive cache; trace: oracle-routing upper bound")
     ap.add_argument("--demote", type=int, default=0, help="PROMOE_F_DEMOTE: a mispredicted prefetch becomes the next LRU victim (G17)")
-    ap.add_argument("--fit-prompts", type=int, default=16, help="--predictor fitted: prompts of prompt_len tokens to collect traces from")
+    ap.add_argument("--fit-prompts", type=int, default=20, help="--predictor fitted: prompts of prompt_len tokens to collect traces from")
     ap.add_argument("--fit-steps", type=int, default=240, help="--predictor fitted: optimiser steps per layer")
     ap.add_argument("--ladder", action="store_true", help="ablation ladder of PAPER.md §7.3 / Fig. 12 (one JSON line per rung)")
     ap.add_argument("--goodpred", action="store_true", help="Accuracy / FetchRate / GoodPred of skip vs fitted at strides 1-3 (one JSON line per row)")

@@ -52,7 +52,10 @@ typedef struct {
   int32_t dense_inter;
   int32_t router_bias;     /* 1 = per-expert logit bias (c3) */
   int32_t pred_hidden;     /* predictor MLP hidden width ("2-layer MLP") */
-  int32_t wdtype;          /* 0 fp32 (c1), 1 bf16 */
+  int32_t wdtype;          /* 0 fp32 (c1), 1 bf16, 2 = bf16 dense weights + INT4 group-quantised routed experts:
+                              per matrix 4-bit codes (two per byte, even element in the low nibble) then, behind the three code
+                              blocks, one bf16 scale per 128 consecutive elements of a row; value = (code - 8) * scale; image =
+                              [gate codes | up codes | down codes | gate scales | up scales | down scales] (G18) */
   float rope_theta, rms_eps;
 } promoe_shape_t;
 
@@ -216,7 +219,8 @@ PROMOE_API int promoe_op_attention(float* qkv, const float* cos_t, const float* 
 
 /* expert FFN row A9 on one resident weight set: y[T,H] = Wd.(silu(Wg.x) * (Wu.x)); x [T,H], act_ws [T,I] scratch,
  * prob_ws >= 64 bytes of device scratch (problem record).  path: 0 auto, 1 HBM-streaming GEMV (T == 1),
- * 2 SIMT grouped GEMM, 3 tcgen05 grouped GEMM (bf16 weights). */
+ * 2 SIMT grouped GEMM, 3 tcgen05 grouped GEMM (bf16 weights).  wdtype 2: wg = DEVICE ptr to one INT4 expert image (format at
+ * promoe_shape_t.wdtype; wu / wd ignored), T == 1 and path 0 / 1 only. */
 PROMOE_API int promoe_op_expert_ffn(const float* x, const void* wg, const void* wu, const void* wd, float* act_ws,
                                     float* y, void* prob_ws, int32_t T, int32_t H, int32_t I, int32_t wdtype,
                                     int32_t path, int32_t reserved, void* stream);

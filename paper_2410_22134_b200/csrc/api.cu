@@ -152,8 +152,17 @@ extern "C" int promoe_op_expert_ffn(const float* x, const void* wg, const void* 
                                     float* y, void* prob_ws, int32_t T, int32_t H, int32_t I, int32_t wdtype,
                                     int32_t path, int32_t reserved, void* stream) {
   (void)reserved;
-  if (!x || !wg || !wu || !wd || !act_ws || !y || !prob_ws || T < 1 || H % 16 || I % 16 || (wdtype != 0 && wdtype != 1)) return PROMOE_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
+  if (wdtype == 2) {     // INT4 image [gate codes | up codes | down codes | scales] at wg (wu / wd ignored); GEMV path only
+    if (!x || !wg || !act_ws || !y || !prob_ws || T != 1 || path > 1 || H % 128 || I % 128) return PROMOE_EINVAL;
+    FfnProblem q{};
+    q.wg = wg; q.wu = nullptr; q.wd = nullptr; q.flags = nullptr; q.gen = 0; q.inter = I; q.row0 = 0; q.nrows = 1; q.expert = -1;
+    if (cudaMemcpyAsync(prob_ws, &q, sizeof(q), cudaMemcpyHostToDevice, st) != cudaSuccess) return PROMOE_ECUDA;
+    launch_ffn_gateup_gemv_q4(x, (const FfnProblem*)prob_ws, 1, I, H, act_ws, I, (size_t)1 << 20, nullptr, st);
+    launch_ffn_down_gemv_q4(act_ws, I, (const FfnProblem*)prob_ws, 1, H, y, (size_t)1 << 20, nullptr, st);
+    return launch_status();
+  }
+  if (!x || !wg || !wu || !wd || !act_ws || !y || !prob_ws || T < 1 || H % 16 || I % 16 || (wdtype != 0 && wdtype != 1)) return PROMOE_EINVAL;
   FfnProblem pb{};
   pb.wg = wg; pb.wu = wu; pb.wd = wd; pb.flags = nullptr; pb.gen = 0; pb.inter = I; pb.row0 = 0; pb.nrows = T; pb.expert = -1;
   if (cudaMemcpyAsync(prob_ws, &pb, sizeof(pb), cudaMemcpyHostToDevice, st) != cudaSuccess) return PROMOE_ECUDA;

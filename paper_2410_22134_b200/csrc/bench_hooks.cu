@@ -56,7 +56,7 @@ extern "C" int promoe_bench_kernel_time(promoe_t* h, int32_t which, int32_t reps
   if (!h->experts_loaded) { h->err = "kernel_time before load_experts"; return PROMOE_ESTATE; }
   const promoe_shape_t& s = h->s;
   const int k = s.top_k, H = s.hidden, I = s.expert_inter, Lm = h->Lm, C = h->C;
-  const size_t hi = (size_t)H * I * h->wb;
+  const size_t hi = h->q4 ? (size_t)H * I / 2 : (size_t)H * I * h->wb;     // INT4: code bytes per matrix (scales follow the codes)
   // problem tables over resident slots, one per layer, so that consecutive launches stream different weights
   std::vector<FfnProblem> pb((size_t)Lm * k);
   for (int m = 0; m < Lm; ++m)
@@ -82,7 +82,10 @@ extern "C" int promoe_bench_kernel_time(promoe_t* h, int32_t which, int32_t reps
   CKA(cudaEventCreate(&a)); CKA(cudaEventCreate(&b));
   auto launch = [&](int r) {
     const FfnProblem* q = dp + (size_t)(r % Lm) * k;
-    if (which == 0) launch_ffn_gateup_gemv(h->u, q, k, I, H, h->act, I, s.wdtype, h->chunk_bytes, h->err_dev, h->cs);
+    if (h->q4) {
+      if (which == 0) launch_ffn_gateup_gemv_q4(h->u, q, k, I, H, h->act, I, h->chunk_bytes, h->err_dev, h->cs);
+      else launch_ffn_down_combine_q4(h->act, I, q, row_of, gates, k, nullptr, nullptr, H, h->yexp, h->chunk_bytes, h->err_dev, h->cs);
+    } else if (which == 0) launch_ffn_gateup_gemv(h->u, q, k, I, H, h->act, I, s.wdtype, h->chunk_bytes, h->err_dev, h->cs);
     else launch_ffn_down_combine(h->act, I, q, row_of, gates, k, nullptr, nullptr, nullptr, nullptr, H, h->yexp, s.wdtype,
                                  h->chunk_bytes, h->err_dev, h->cs);
   };
@@ -95,6 +98,6 @@ extern "C" int promoe_bench_kernel_time(promoe_t* h, int32_t which, int32_t reps
   CKA(cudaEventElapsedTime(&ms, a, b));
   cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(dp); cudaFree(row_of); cudaFree(gates);
   *avg_ms_out = (double)ms / reps;
-  *bytes_out = (double)k * (which == 0 ? 2.0 : 1.0) * (double)hi;
+  *bytes_out = (double)k * (which == 0 ? 2.0 : 1.0) * (double)hi * (h->q4 ? 33.0 / 32.0 : 1.0);   // INT4: + one bf16 scale per 128 codes
   return PROMOE_OK;
 }

@@ -38,9 +38,9 @@ inline void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t sme
 // force the (lazy) load of one kernel; see preload_* in every kernels_*.cu
 inline void preload_fn(const void* f) { cudaFuncAttributes a; (void)cudaFuncGetAttributes(&a, f); }
 void preload_dense(); void preload_attn(); void preload_route(); void preload_slot(); void preload_decode();
-void preload_ffn(); void preload_tc(); void preload_fetch();
+void preload_ffn(); void preload_tc(); void preload_fetch(); void preload_q4();
 inline void preload_all() {
-  preload_dense(); preload_attn(); preload_route(); preload_slot(); preload_decode(); preload_ffn(); preload_tc(); preload_fetch();
+  preload_dense(); preload_attn(); preload_route(); preload_slot(); preload_decode(); preload_ffn(); preload_tc(); preload_fetch(); preload_q4();
 }
 
 // number of kernels launched by this library (host-side counter, bumped by every launch_* wrapper; promoe_stats)

@@ -51,7 +51,8 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   if (s.n_q_heads % s.n_kv_heads) return bad("n_q_heads must be a multiple of n_kv_heads");
   if (s.n_experts > 256 || s.top_k > 16 || s.top_k > s.n_experts) return bad("n_experts <= 256, top_k <= 16");
   if (s.n_shared_inter % 16 || s.dense_inter % 16 || s.pred_hidden % 8) return bad("ffn widths must be multiples of 16");
-  if (s.wdtype != 0 && s.wdtype != 1) return bad("wdtype must be 0 (fp32) or 1 (bf16)");
+  if (s.wdtype != 0 && s.wdtype != 1 && s.wdtype != 2) return bad("wdtype must be 0 (fp32), 1 (bf16) or 2 (bf16 + INT4 routed experts)");
+  if (s.wdtype == 2 && (s.hidden % 128 || s.expert_inter % 128)) return bad("INT4 experts need hidden and expert_inter to be multiples of 128 (the quantisation group)");
   if (op->cache_slots <= 0 || op->cache_slots % Lm) return bad("cache_slots must be a positive multiple of n_moe_layers");
   const int C = op->cache_slots / Lm;
   if (C > s.n_experts) return bad("more slots per layer than experts");
@@ -64,7 +65,10 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   promoe_t* h = new promoe();
   h->s = s; h->o = *op; h->Lm = Lm; h->C = C;
   h->wb = s.wdtype == 0 ? 4 : 2;
+  h->wdd = s.wdtype == 0 ? 0 : 1;
+  h->q4 = s.wdtype == 2;
   h->Be = (size_t)3 * s.hidden * s.expert_inter * h->wb;
+  if (h->q4) h->Be = (size_t)3 * s.hidden * s.expert_inter / 2 + (size_t)3 * s.hidden * s.expert_inter / 128 * 2;   // codes + bf16 scales (G18)
   h->chunk_bytes = op->chunk_bytes ? (size_t)op->chunk_bytes : ((size_t)256 << 10);
   if (h->chunk_bytes % 256) { delete h; return bad("chunk_bytes must be a multiple of 256"); }
   h->n_chunks = (int)((h->Be + h->chunk_bytes - 1) / h->chunk_bytes);
@@ -114,7 +118,8 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->pred_list, (size_t)Lm * (1 + E))); CK(dalloc(&h->trace_precise, (size_t)Lm * (1 + 5 * E)));
     CK(dalloc(&h->trace_pred, (size_t)Lm * (1 + 4 * E))); CK(dalloc(&h->row_of, (size_t)k)); CK(dalloc(&h->n_prob, (size_t)1));
     CK(dalloc(&h->problems, (size_t)E)); CK(dalloc(&h->shared_prob, (size_t)L)); CK(dalloc(&h->err_dev, (size_t)1)); CK(dalloc(&h->attn_cnt, (size_t)s.n_q_heads));
-    if ((op->flags & PROMOE_F_TENSOR) && s.wdtype == 1) {
+    if (h->q4) { CK(dalloc(&h->q4_stage, (size_t)E * 3 * H * s.expert_inter)); CK(dalloc(&h->problems_deq, (size_t)E)); }
+    if ((op->flags & PROMOE_F_TENSOR) && s.wdtype >= 1) {
       h->tc = tc_create(&h->err);
       if (!h->tc) return PROMOE_ECUDA;
       auto up8 = [](size_t v) { return (v + 7) & ~(size_t)7; };
@@ -182,7 +187,7 @@ extern "C" void promoe_destroy(promoe_t* h) {
                   h->count, h->offset, h->perm, h->inv, h->gates, h->margin, h->z, h->pred_list, h->trace_precise,
                   h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->attn_cnt, h->slots, h->flags,
                   h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock,
-                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch, h->trace_u};
+                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch, h->trace_u, h->q4_stage, h->problems_deq};
   for (void* b : bufs) if (b) cudaFree(b);
   if (h->xsA) cudaFree(h->xsA);
   if (h->xsG) cudaFree(h->xsG);

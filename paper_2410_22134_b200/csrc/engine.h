@@ -43,6 +43,10 @@ struct promoe {
   promoe_shape_t s{};
   promoe_opts_t o{};
   int Lm = 0, C = 0, wb = 2, n_chunks = 0, max_inflight = 2;
+  int wdd = 1;                 // dtype of the DENSE weights (0 fp32, 1 bf16); wdtype 2 = bf16 dense + INT4 routed experts
+  bool q4 = false;             // routed experts are INT4 group-quantised images (kernels_q4.cu)
+  float* q4_stage = nullptr;   // prefill: fp32 staging images of the needed experts [E, 3*H*I]
+  pmk::FfnProblem* problems_deq = nullptr;   // records pointing into q4_stage
   size_t Be = 0, chunk_bytes = 0;
   int max_spec_decode = 0, max_spec_prefill = 0;   // allocations allowed per PushPredicted (knob G3)
   int maxT = 0, qkv_w = 0, ffn_w = 0, nsplit = 1;

@@ -119,6 +119,18 @@ void launch_ffn_gateup_gemm_simt(const float* x, const int32_t* row_src, int src
 void launch_ffn_down_gemm_simt(const float* act, int act_stride, const FfnProblem* probs, int p0, int np,
                                int max_rows, int rows_override, int max_inter, int H, float* y, int wdtype, cudaStream_t st);
 
+// A9 with INT4 group-quantised expert images (kernels_q4.cu; G18).  Problem records as above with wg = image base.
+void launch_ffn_gateup_gemv_q4(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
+                               int act_stride, size_t chunk_bytes, int* err, cudaStream_t st);
+void launch_ffn_down_gemv_q4(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int H, float* y,
+                             size_t chunk_bytes, int* err, cudaStream_t st);
+void launch_ffn_down_combine_q4(const float* act, int act_stride, const FfnProblem* probs, const int32_t* row_of,
+                                const float* gates, int k, const float* sgate_logit, const float* shared_y, int H, float* x,
+                                size_t chunk_bytes, int* err, cudaStream_t st);
+// prefill: INT4 images of problems [p0, p0+np) → fp32 staging images + records pointing at them (out_probs[p0 ..])
+void launch_dequant_q4(const FfnProblem* probs, int p0, int np, int H, int max_inter, float* stage,
+                       size_t stage_stride_elems, FfnProblem* out_probs, cudaStream_t st);
+
 // ---- fused decode kernels (kernels_decode.cu) ---------------------------------------------------------------
 struct GemvSeg { const void* w; float* out; int n; int flags; };
 struct NormGemvArgs {

@@ -314,10 +314,19 @@ struct Scout {
       if (r != ACQ_OK) { FTRACE("[scout %d] end %d\n", blockIdx.x, r); if (lane == 0) { __threadfence_block(); fq->end = r; } break; }
       // HIGH chunks may queue up in front of the engine; a LOW chunk only when nothing is waiting (it could not be taken back)
       const unsigned room = c.low ? 1u : (unsigned)kQueue - 1u;
-      {   // every wait of the worker is bounded: a protocol error must surface as PROMOE_ETIMEOUT, never as a hang
+      {   // every wait of the worker is bounded: a protocol error must surface as PROMOE_ETIMEOUT, never as a hang.
+          // Lane 0 alone looks at the queue and the warp follows its verdict: with every lane polling for itself, lane 0
+          // could leave the loop, push the chunk and let the engine take it — head then runs AHEAD of the `pushed` the
+          // slower lanes still hold, `pushed - head` wraps, and they spin until the time-out (seen as 4 s fetch kernels
+          // behind decode steps that had long finished)
         const unsigned long long t0 = globaltimer_ns();
-        while (pushed - fq->head >= room) {
-          if (globaltimer_ns() - t0 > kFlagTimeoutNs) { if (lane == 0) atomicExch(a.err, 2); break; }
+        while (true) {
+          int full = 0;
+          if (lane == 0) {
+            full = pushed - fq->head >= room;
+            if (full && globaltimer_ns() - t0 > kFlagTimeoutNs) { atomicExch(a.err, 2); full = 0; }
+          }
+          if (!__shfl_sync(0xffffffffu, full, 0)) break;
           __nanosleep(40);
         }
       }

@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     const int n = n_built;
     for (int sl = 0; sl < C; ++sl) v.origin[sl] = 0;
     // problem table + decode row map + trace
-    const size_t hi = (size_t)H * inter * wbytes;
+    const size_t hi = wbytes ? (size_t)H * inter * wbytes : (size_t)H * inter / 2;   // wbytes 0: INT4 codes (kernels_q4.cu)
     for (int i = 0; i < n; ++i) {
       const int32_t* r = rec + 7 * i;
       const int e = order[i];

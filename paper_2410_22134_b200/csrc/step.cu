@@ -40,7 +40,7 @@ int ce_flush_flags(promoe_t* h);
     }                                                                                              \
   } while (0)
 
-static bool use_tc(const promoe_t* h, int T) { return T > 1 && h->tc != nullptr && h->s.wdtype == 1; }
+static bool use_tc(const promoe_t* h, int T) { return T > 1 && h->tc != nullptr && h->wdd == 1; }
 
 // fp32 rows of x → bf16 hi/lo planes in xsA (the activation operand of the tcgen05 GEMMs, reading G1)
 static void split_A(promoe_t* h, const float* x, int T, int K) {
@@ -50,9 +50,9 @@ static void split_A(promoe_t* h, const float* x, int T, int K) {
 // y[T,N] (+)= x[T,K]·W^T on the compute stream: GEMV for one token; T > 1: tcgen05 GEMM (bf16 weights) or SIMT.
 // presplit: xsA already holds the hi/lo split of x.
 static int linear(promoe_t* h, const float* x, const void* w, float* y, int T, int N, int K, int flags, bool presplit = false) {
-  if (T == 1) { launch_gemv(x, w, y, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
-  if (N <= 4) { launch_linear_small_n(x, w, y, T, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
-  if (!use_tc(h, T) || N < 16) { launch_gemm_simt(x, w, y, T, N, K, h->s.wdtype, flags, h->cs); return PROMOE_OK; }
+  if (T == 1) { launch_gemv(x, w, y, N, K, h->wdd, flags, h->cs); return PROMOE_OK; }
+  if (N <= 4) { launch_linear_small_n(x, w, y, T, N, K, h->wdd, flags, h->cs); return PROMOE_OK; }
+  if (!use_tc(h, T) || N < 16) { launch_gemm_simt(x, w, y, T, N, K, h->wdd, flags, h->cs); return PROMOE_OK; }
   if (!presplit) split_A(h, x, T, K);
   TcGemm g;
   g.a0 = w; g.a_rows = N; g.b_hi = h->xsA; g.b_lo_off = h->xsA_half; g.b_rows_cap = (int)(h->xsA_half / K);
@@ -63,7 +63,7 @@ static int linear(promoe_t* h, const float* x, const void* w, float* y, int T, i
 // SwiGLU FFN of an always-resident MLP (shared expert / dense layer) for all T rows of u → h->sy.
 // T > 1 with tensor cores: expects the split of u in xsA.
 static int resident_ffn(promoe_t* h, int l, int inter, int T) {
-  const int H = h->s.hidden, wd = h->s.wdtype;
+  const int H = h->s.hidden, wd = h->wdd;
   if (T == 1) {
     launch_ffn_gateup_gemv(h->u, h->shared_prob + l, 1, inter, H, h->sact, h->ffn_w, wd, h->chunk_bytes, h->err_dev, h->cs);
     launch_ffn_down_gemv(h->sact, h->ffn_w, h->shared_prob + l, 1, inter, H, h->sy, wd, h->chunk_bytes, h->err_dev, h->cs);
@@ -88,6 +88,12 @@ static int resident_ffn(promoe_t* h, int l, int inter, int T) {
 static int expert_batch(promoe_t* h, const int32_t* perm, int i, int j, int max_rows) {
   const promoe_shape_t& s = h->s;
   const int H = s.hidden, I = s.expert_inter, k = s.top_k;
+  if (h->q4) {     // INT4 experts: exact fp32 staging images, then the fp32 SIMT grouped GEMM (kernels_q4.cu)
+    launch_dequant_q4(h->problems, i, j - i, H, I, h->q4_stage, (size_t)3 * H * I, h->problems_deq, h->cs);
+    launch_ffn_gateup_gemm_simt(h->u, perm, k, h->problems_deq, i, j - i, max_rows, 0, I, H, h->act, I, 0, h->cs);
+    launch_ffn_down_gemm_simt(h->act, I, h->problems_deq, i, j - i, max_rows, 0, I, H, h->yexp, 0, h->cs);
+    return PROMOE_OK;
+  }
   if (!use_tc(h, 2)) {
     launch_ffn_gateup_gemm_simt(h->u, perm, k, h->problems, i, j - i, max_rows, 0, I, H, h->act, I, s.wdtype, h->cs);
     launch_ffn_down_gemm_simt(h->act, I, h->problems, i, j - i, max_rows, 0, I, H, h->yexp, s.wdtype, h->cs);
@@ -113,7 +119,7 @@ static int expert_batch(promoe_t* h, const int32_t* perm, int i, int j, int max_
 // One layer of the batch-1 decode step with the fused kernels of kernels_decode.cu (7 launches instead of 19).
 static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   const promoe_shape_t& s = h->s;
-  const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter, wd = s.wdtype;
+  const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter, wd = h->wdd;
   const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim;
   cudaStream_t cs = h->cs;
   const size_t kv_layer = (size_t)nkv * s.max_seq * d;
@@ -163,15 +169,21 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   rf.p1 = h->p1; rf.pred_w2 = mlp ? h->pred_w2[l] : nullptr; rf.ph = s.pred_hidden; rf.wdtype = wd;
   rf.pred_out = mlp ? plist : nullptr; rf.k = k; rf.cap = C;
   launch_slot_table(h->tbl, m, h->o.stride, h->max_spec_decode, sel, 1, k, nullptr, plist,
-                    ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb, h->problems,
+                    ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb, h->problems,
                     h->n_prob, h->row_of, h->cmd_dev + m, seq, h->trace_precise + (size_t)m * (1 + 5 * E),
                     (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf, h->cmd_fetch + m);
   // A7 runs beside this stream: the fetch worker (kernels_fetch.cu, resident since the start of the step) sees the
   // command K5 publishes in device memory and pulls the missing chunks over the link; the flag-gated kernels K6/K7 are
   // enqueued right away and wait (ld.acquire.sys on the chunk flags, __nanosleep between polls) for exactly the bytes
   // they read.  The host is not in the layer loop at all.
-  launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
+  if (h->q4) launch_ffn_gateup_gemv_q4(h->u, h->problems, k, I, H, h->act, I, h->chunk_bytes, h->err_dev, cs);      // K6 (INT4)
+  else launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
   if (s.n_shared_inter && cudaStreamWaitEvent(cs, h->ev_join, 0) != cudaSuccess) { h->err = "join of the shared-expert stream failed"; return PROMOE_ECUDA; }
+  if (h->q4) {                                                                                             // K7 (INT4)
+    launch_ffn_down_combine_q4(h->act, I, h->problems, h->row_of, gates, k, (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr,
+                               s.n_shared_inter ? h->sy : nullptr, H, h->x, h->chunk_bytes, h->err_dev, cs);
+    return PROMOE_OK;
+  }
   launch_ffn_down_combine(h->act, I, h->problems, h->row_of, gates, k, nullptr, nullptr,               // K7
                             (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr, s.n_shared_inter ? h->sy : nullptr, H, h->x,
                             wd, h->chunk_bytes, h->err_dev, cs);
@@ -183,7 +195,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
 static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_out) {
   const promoe_shape_t& s = h->s;
   const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter;
-  const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = s.wdtype;
+  const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = h->wdd;
   if (!h->dense_loaded || !h->experts_loaded) { h->err = "step before load_dense / load_experts"; return PROMOE_ESTATE; }
   if (T < 1 || !ids_host) { h->err = "step: no tokens"; return PROMOE_EINVAL; }
   if (h->pos + T > s.max_seq) { h->err = "step: sequence exceeds max_seq"; return PROMOE_ESTATE; }
@@ -301,7 +313,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
 static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fused) {
   const promoe_shape_t& s = h->s;
   const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter;
-  const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = s.wdtype;
+  const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = h->wdd;
   cudaStream_t cs = h->cs;
   const size_t kv_layer = (size_t)nkv * s.max_seq * d;
   std::vector<int> deferred;
@@ -355,7 +367,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     }
     if (T > 1) launch_permute(sel, T, k, E, h->count + (size_t)m * E, offset, perm, inv, cs);   // A8
     launch_slot_table(h->tbl, m, h->o.stride, T == 1 ? h->max_spec_decode : h->max_spec_prefill, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
-                      ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->wb,
+                      ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb,
                       h->problems, h->n_prob, h->row_of, h->cmd_dev + m, seq,
                       h->trace_precise + (size_t)m * (1 + 5 * E),
                       (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs);
@@ -377,11 +389,16 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     const int n = cmd.n_needed;
     // ---- A9 routed experts, launch order
     if (T == 1) {
-      launch_ffn_gateup_gemv(h->u, h->problems, n, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);
-      launch_ffn_down_gemv(h->act, I, h->problems, n, I, H, h->yexp, wd, h->chunk_bytes, h->err_dev, cs);
+      if (h->q4) {
+        launch_ffn_gateup_gemv_q4(h->u, h->problems, n, I, H, h->act, I, h->chunk_bytes, h->err_dev, cs);
+        launch_ffn_down_gemv_q4(h->act, I, h->problems, n, H, h->yexp, h->chunk_bytes, h->err_dev, cs);
+      } else {
+        launch_ffn_gateup_gemv(h->u, h->problems, n, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);
+        launch_ffn_down_gemv(h->act, I, h->problems, n, I, H, h->yexp, wd, h->chunk_bytes, h->err_dev, cs);
+      }
       launch_combine(h->x, h->yexp, h->row_of, gates, 1, k, H, shared, sgate, h->x, cs);
     } else {
-      if (tc) launch_split_rows(h->u, perm, k, T * k, H, h->xsG, h->xsG_half, cs);   // gathered rows, permuted order
+      if (tc && !h->q4) launch_split_rows(h->u, perm, k, T * k, H, h->xsG, h->xsG_half, cs);   // gathered rows, permuted order
       // batches: [all class A] [all class B] then every class C alone (its fill lands in copy order)
       int i = 0;
       size_t dnext = 0;

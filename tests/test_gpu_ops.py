@@ -248,3 +248,31 @@ def test_op_attention(B, nq, nkv, d, T0, n_dec):
     assert (kc[:, :pos].cpu().double() - kref).abs().max().item() <= 1e-5 * max(1.0, kref.abs().max().item())
     assert L.promoe_op_attention(qkv.data_ptr(), cos_t.data_ptr(), sin_t.data_ptr(), kc.data_ptr(), vc.data_ptr(), out.data_ptr(),
                                  ws.data_ptr(), cnt.data_ptr(), 1, max_seq, nq, nkv, d, max_seq, None) == B.PROMOE_EINVAL
+
+
+# ---- A9 with INT4 group-quantised experts (format DESIGN.md G18) ---------------------------------------
+@pytest.mark.parametrize("H,I", [(256, 512), (2048, 1408), (4096, 14336), (128, 128)])
+def test_op_expert_ffn_int4(B, H, I):
+    """promoe_op_expert_ffn with wdtype 2 (decode GEMVs that dequantise in registers) against the oracle's
+    dequantise-then-fp64 FFN on the same packed image; K = 1408 has a ragged last pass, K = 14336 many passes."""
+    from oracle.forward import swiglu_ffn
+    from oracle.quant import dequant_expert
+    from synth.weights import pack_int4
+    mats = [_w((I, H), torch.float32, 8), _w((I, H), torch.float32, 9), _w((H, I), torch.float32, 10)]
+    packed = [pack_int4(m) for m in mats]
+    img = torch.cat([c.reshape(-1) for c, _ in packed] + [s.contiguous().view(torch.uint8).reshape(-1) for _, s in packed])
+    assert img.numel() == 3 * H * I * 33 // 64
+    x = _w((1, H), torch.float32, 7, 1.0)
+    xd, imgd = x.cuda(), img.cuda()
+    act = torch.empty((1, I), device="cuda"); y = torch.full((1, H), float("nan"), device="cuda")
+    ws = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    rc = B.lib().promoe_op_expert_ffn(xd.data_ptr(), imgd.data_ptr(), None, None, act.data_ptr(), y.data_ptr(), ws.data_ptr(),
+                                      1, H, I, 2, 1, 0, None)
+    assert rc == 0
+    torch.cuda.synchronize()
+    wg, wu, wd = dequant_expert(img, H, I)
+    ref = swiglu_ffn(x.double(), wg, wu, wd)
+    err = (y.cpu().double() - ref).abs().max().item()
+    assert err <= 2e-4 * max(1.0, ref.abs().max().item()), err
+    assert B.lib().promoe_op_expert_ffn(xd.data_ptr(), imgd.data_ptr(), None, None, act.data_ptr(), y.data_ptr(), ws.data_ptr(),
+                                        1, H + 64, I, 2, 1, 0, None) == B.PROMOE_EINVAL       # not a multiple of the group
