@@ -72,6 +72,13 @@ class ClockSampler:
 
 
 # ---- algorithmic work of one step -----------------------------
+def expert_image_bytes(s) -> int:
+    """Bytes of one routed expert image (what a slot fill moves): 3·H·I weights at 4 / 2 bytes, or INT4 codes + one
+    bf16 scale per 128 (wdtype 2, G18)."""
+    n = 3 * s.hidden * s.expert_inter
+    return n // 2 + n // 128 * 2 if s.wdtype == 2 else n * (4 if s.wdtype == 0 else 2)
+
+
 def dense_bytes_per_token(s) -> int:
     """Always-resident weight bytes one decode step streams from HBM (each touched once)."""
     wb = 4 if s.wdtype == 0 else 2
@@ -89,7 +96,7 @@ def step_work(s, T: int, pos0: int, distinct_experts: int, need_experts: int):
     """(B_hbm, FLOPs) of one step with T tokens starting at position pos0.  distinct_experts = Σ_layers |needed|,
     need_experts = those not resident at step start (their bytes are also WRITTEN into the slot region)."""
     wb = 4 if s.wdtype == 0 else 2
-    Be = 3 * s.hidden * s.expert_inter * wb
+    Be = expert_image_bytes(s)
     n_moe = s.n_layers - s.n_dense_layers
     kv_read = sum(2 * s.n_layers * s.n_kv_heads * s.head_dim * 4 * (pos0 + t + 1) for t in range(T)) if T == 1 else \
         2 * s.n_layers * s.n_kv_heads * s.head_dim * 4 * (pos0 + T)
@@ -181,7 +188,7 @@ def workload_config(cfg, args):
                         f"prompt {cfg.prompt_len} + {cfg.decode_steps} decode",
             "cache_slots": cfg.cache_slots, "cache_fraction": cfg.slots_per_layer / s.n_experts, "stride": cfg.stride,
             "predictor": args.predictor, "decode_ids": args.decode, "chunk_bytes": args.chunk_kb << 10, "max_spec_decode": args.max_spec_decode,
-            "max_spec_prefill": args.max_spec_prefill, "low_cap_chunks": args.low_cap, "max_inflight": args.inflight, "fetch_ctas": args.fetch_ctas, "demote": args.demote,
+            "max_spec_prefill": args.max_spec_prefill, "low_cap_chunks": args.low_cap, "max_inflight": args.inflight, "fetch_ctas": args.fetch_ctas, "demote": args.demote, "int4_experts": args.int4,
             "l2": "inputs larger than L2 (each request streams >> 126 MB of expert weights)"}
 
 
@@ -262,8 +269,8 @@ def replica_weights(cfg, pred_kind, local, world, dist, tag=None):
         return synth.make_weights(cfg, predictor=pred_kind)
     s = cfg.shape
     n_moe = s.n_layers - s.n_dense_layers
-    per = 3 * s.hidden * s.expert_inter
-    dt = torch.float32 if s.wdtype == 0 else torch.bfloat16
+    per = expert_image_bytes(s) if s.wdtype == 2 else 3 * s.hidden * s.expert_inter
+    dt = {0: torch.float32, 1: torch.bfloat16, 2: torch.uint8}[s.wdtype]
     path = f"/dev/shm/promoe_experts_{tag or os.environ.get('MASTER_PORT', '0')}_{cfg.name}"
     if local == 0:
         buf = torch.from_file(path, shared=True, size=n_moe * s.n_experts * per, dtype=dt).view(n_moe, s.n_experts, per)
@@ -291,8 +298,7 @@ def run_ours(args, cfg, rank, world, dist):
     s = cfg.shape
     pred_kind = "skip" if args.predictor in ("none", "trace", "fitted") else args.predictor
     weights = replica_weights(cfg, pred_kind, local, world, dist)
-    wb = 4 if s.wdtype == 0 else 2
-    Be = 3 * s.hidden * s.expert_inter * wb
+    Be = expert_image_bytes(s)
     h2d_gbs = B.promoe_bench_h2d(256 << 20, 2, 5)
     prompt = synth.make_prompt(cfg).tolist()
     decode_ids = synth.make_decode_ids(cfg).tolist()
@@ -465,7 +471,8 @@ def run_ours(args, cfg, rank, world, dist):
         return
     line = {"metric": METRIC, "value": g_dec_tok / g_dec_s, "unit": "tokens/s", "n_gpus": world, "steps": K,
             "warmup": args.warmup, "ms_per_step": 1e3 * wall / K, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32 activations x bf16 weights, f32 accumulate" if s.wdtype else "f32",
+            "vs_baseline": None, "dtype": {0: "f32", 1: "f32 activations x bf16 weights, f32 accumulate",
+                                          2: "f32 activations x (bf16 dense weights, int4 group-quantised experts), f32 accumulate"}[s.wdtype],
             "data": "synthetic", "config": workload_config(cfg, args),
             "prefill_tokens_per_s": g_pre_tok / g_pre_s, "decode_ms_per_token": 1e3 * g_dec_s / g_dec_tok * world,
             "ttft_ms": 1e3 * pre_s / K,
@@ -578,9 +585,11 @@ def run_modes(args):
         over["prompt_len"] = args.prompt_len
     if args.decode_steps:
         over["decode_steps"] = args.decode_steps
+    if args.int4:
+        over["shape_overrides"] = {"wdtype": 2}
     base = synth.get_config(args.config, **over)
     s = base.shape
-    Be = 3 * s.hidden * s.expert_inter * (4 if s.wdtype == 0 else 2)
+    Be = expert_image_bytes(s)
     h2d = B.promoe_bench_h2d(256 << 20, 2, 5)
     prompt = synth.make_prompt(base).tolist()
     decode_ids = synth.make_decode_ids(base).tolist()
@@ -664,6 +673,9 @@ def main():
     ap.add_argument("--demote", type=int, default=0, help="PROMOE_F_DEMOTE: a mispredicted prefetch becomes the next LRU victim (G17)")
     ap.add_argument("--fit-prompts", type=int, default=20, help="--predictor fitted: prompts of prompt_len tokens to collect traces from")
     ap.add_argument("--fit-steps", type=int, default=240, help="--predictor fitted: optimiser steps per layer")
+    ap.add_argument("--cache-all", type=int, default=0, help="every routed expert resident (compute-only step; with --fetch-ctas -1 "
+                    "this is the configuration ncu can profile: a kernel-serialising profiler cannot run the persistent fetch worker)")
+    ap.add_argument("--int4", type=int, default=0, help="routed experts as INT4 group-quantised images (SURVEY N3; wdtype 2)")
     ap.add_argument("--ladder", action="store_true", help="ablation ladder of PAPER.md §7.3 / Fig. 12 (one JSON line per rung)")
     ap.add_argument("--goodpred", action="store_true", help="Accuracy / FetchRate / GoodPred of skip vs fitted at strides 1-3 (one JSON line per row)")
     ap.add_argument("--decode", default="random", choices=["random", "greedy"],
@@ -697,7 +709,12 @@ def main():
         over["prompt_len"] = args.prompt_len
     if args.decode_steps:
         over["decode_steps"] = args.decode_steps
+    if args.int4:
+        over["shape_overrides"] = {"wdtype": 2}
     cfg = synth.get_config(args.config, **over)
+    if args.cache_all:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, cache_slots=(cfg.shape.n_layers - cfg.shape.n_dense_layers) * cfg.shape.n_experts)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # launched as a plain `python bench.py --gpus N`: start the N ranks ourselves, one process per GPU, the way the
         # driver does (replicas only; NCCL carries the two aggregate all-reduces, nothing on the data path)

@@ -101,7 +101,8 @@ typedef struct {
                               the expert (then as HIGH).  0 = no cap.  Physical only: never changes a trace or an output */
   int32_t fetch_ctas;      /* CTAs (one warp each, TMA bulk copies) of the device-side fetch worker of the fused decode step;
                               0 = default 4 (three reach the SM-side link limit at any chunk size: profiles/r02_fill_probe.md).
-                              Physical only */
+                              < 0 = no worker: legal only when nothing is ever fetched (every expert resident) — for runs under
+                              a profiler that serialises kernels; a needed fetch then ends in PROMOE_ETIMEOUT.  Physical only */
   void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
 } promoe_opts_t;
 

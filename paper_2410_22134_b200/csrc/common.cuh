@@ -241,6 +241,20 @@ __device__ inline bool wait_chunks(const unsigned* flags, int c0, int c1, unsign
   return true;
 }
 
+// Gate word (fused decode): a kernel that needs only the FIRST half of the kernel in front of it waits for the word that
+// kernel publishes (release) behind that half instead of griddepcontrol.wait, which would wait for all of it.
+__device__ inline bool wait_gate_word(const unsigned* word, unsigned want, int* err) {
+  unsigned long long t0 = 0;
+  unsigned v;
+  while (true) {
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(word) : "memory");
+    if (v == want) return true;
+    if (t0 == 0) t0 = globaltimer_ns();
+    if (globaltimer_ns() - t0 > kFlagTimeoutNs || (err && *reinterpret_cast<volatile int*>(err) != 0)) { if (err) atomicExch(err, 1); return false; }
+    __nanosleep(64);
+  }
+}
+
 // One FFN problem = one SwiGLU MLP applied to a row range.  Routed experts: written
 // by the slot-table kernel; shared/dense FFNs: written once at load time.
 struct FfnProblem {
@@ -254,5 +268,15 @@ struct FfnProblem {
   int expert;              // routed expert id, or -1
   int pad;
 };
+static_assert(sizeof(FfnProblem) % 8 == 0, "FfnProblem is read in 8-byte pieces");
+// a record written by a kernel that is still running (gate word): read past L1, 8 bytes at a time (records are 8-byte aligned)
+__device__ __forceinline__ FfnProblem load_problem_cg(const FfnProblem* p) {
+  FfnProblem pb;
+  const unsigned long long* src = reinterpret_cast<const unsigned long long*>(p);
+  unsigned long long* dst = reinterpret_cast<unsigned long long*>(&pb);
+#pragma unroll
+  for (int q = 0; q < (int)(sizeof(FfnProblem) / 8); ++q) dst[q] = __ldcg(src + q);
+  return pb;
+}
 
 }  // namespace pmk

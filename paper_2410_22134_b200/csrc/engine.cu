@@ -82,7 +82,9 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   }
   h->unchunked = (op->flags & PROMOE_F_UNCHUNKED) != 0;
   cudaGetDevice(&h->dev);
-  h->fetch_ctas = op->fetch_ctas > 0 ? std::min(op->fetch_ctas, 16) : 4;
+  // < 0: no fetch worker at all — only for runs in which nothing is ever fetched (every expert resident), e.g. under a
+  // profiler that serialises kernels: a persistent worker would never see the gates of kernels that cannot run beside it
+  h->fetch_ctas = op->fetch_ctas > 0 ? std::min(op->fetch_ctas, 16) : (op->fetch_ctas < 0 ? 0 : 4);
   h->max_inflight = op->max_inflight > 0 ? op->max_inflight : 2;
   h->high_group = op->high_group > 0 ? op->high_group : 0;
   h->low_cap = op->low_cap_chunks > 0 ? op->low_cap_chunks : 0;

@@ -66,6 +66,10 @@ struct SlotTable {
 struct LayerCmd {
   volatile uint32_t seq;     // step_seq * 4096 + layer + 1 once the NEEDED part (PushPrecise) is valid
   volatile uint32_t seq_pred;  // same value once the PREDICTED part (PushPredicted) is valid (published later)
+  volatile uint32_t seq_done;  // same value once the kernel has written the table rows back (device copy only): the next
+                               // layer's slot-table kernel waits for it, because the expert kernels no longer wait for the
+                               // predictor half of this kernel (DESIGN.md §6 "gate word")
+  uint32_t pad_;
   int32_t n_needed;
   int32_t n_pred;            // entries of the push INTO layer (m + stride), 0 if none
   int32_t pred_target;
@@ -83,7 +87,7 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* j_of_problem, LayerCmd* cmd,
                        uint32_t seq, int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st,
-                       const RouteFuse* fuse = nullptr, LayerCmd* cmd_dev2 = nullptr);
+                       const RouteFuse* fuse = nullptr, LayerCmd* cmd_dev2 = nullptr, const LayerCmd* cmd_prev = nullptr);
 
 // A7 (fused decode): the device-side prefetch worker (kernels_fetch.cu).
 struct FetchArgs {
@@ -106,9 +110,11 @@ cudaError_t launch_fetch(const FetchArgs& a, int ctas, cudaStream_t st);
 // A9 decode expert FFN (GEMV, T == 1) over a problem list in launch order.
 //  gateup: act[p, i] = silu(Wg_p[i,:].u) * (Wu_p[i,:].u)     down: y[p, h] = Wd_p[h,:].act[p,:]
 // chunk geometry: image = [gate | up | down], chunk c covers bytes [c*chunk_bytes, (c+1)*chunk_bytes).
+// gate_seq != nullptr (fused decode): the kernel does NOT wait for the kernel in front of it (the slot-table kernel, whose
+// predictor half it does not need) but for *gate_seq == gate_want, the word that kernel publishes behind the problem table.
 void launch_ffn_gateup_gemv(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
                             int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st,
-                            int static_table = 0);   // 1: records written at load time → early L2 prefetch under PDL
+                            int static_table = 0, const uint32_t* gate_seq = nullptr, uint32_t gate_want = 0);
 void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int max_inter,
                           int H, float* y, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st, int static_table = 0);
 // A9 prefill grouped SwiGLU FFN, SIMT fp32: problems [p0, p0+np) each with its row range; x rows are gathered
@@ -121,7 +127,8 @@ void launch_ffn_down_gemm_simt(const float* act, int act_stride, const FfnProble
 
 // A9 with INT4 group-quantised expert images (kernels_q4.cu; G18).  Problem records as above with wg = image base.
 void launch_ffn_gateup_gemv_q4(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
-                               int act_stride, size_t chunk_bytes, int* err, cudaStream_t st);
+                               int act_stride, size_t chunk_bytes, int* err, cudaStream_t st,
+                               const uint32_t* gate_seq = nullptr, uint32_t gate_want = 0);
 void launch_ffn_down_gemv_q4(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int H, float* y,
                              size_t chunk_bytes, int* err, cudaStream_t st);
 void launch_ffn_down_combine_q4(const float* act, int act_stride, const FfnProblem* probs, const int32_t* row_of,

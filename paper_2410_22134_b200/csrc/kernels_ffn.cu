@@ -19,13 +19,23 @@ __global__ void __launch_bounds__(256) ffn_gateup_gemv_kernel(const float* __res
                                                               const FfnProblem* __restrict__ probs,
                                                               const int32_t* __restrict__ n_probs_dev, int tiles,
                                                               int H, float* __restrict__ act, int act_stride,
-                                                              size_t chunk_bytes, int* err, int static_table) {
+                                                              size_t chunk_bytes, int* err, int static_table,
+                                                              const uint32_t* gate_seq, uint32_t gate_want) {
   const int p = blockIdx.x / tiles, tile = blockIdx.x % tiles;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r0 = tile * 8;
   (void)static_table;   // early L2 prefetch of resident rows before the wait was measured slower (2.90 vs 2.81 ms/token)
-  pdl_enter();
-  const FfnProblem pb = probs[p];
+  FfnProblem pb;
+  if (gate_seq) {       // wait for the problem table only, not for the predictor half of the slot-table kernel
+    __shared__ int gate_ok;
+    if (threadIdx.x == 0) gate_ok = wait_gate_word(gate_seq, gate_want, err);
+    __syncthreads();
+    if (!gate_ok) return;
+    pb = load_problem_cg(probs + p);
+  } else {
+    pdl_enter();
+    pb = probs[p];
+  }
   if (n_probs_dev && p >= *n_probs_dev) return;
   if (r0 >= pb.inter) return;
   const int r1 = min(pb.inter, r0 + 8);
@@ -166,12 +176,13 @@ __global__ void __launch_bounds__(256) ffn_gemm_simt_kernel(const float* __restr
 #define WDISPATCH(expr_f32, expr_bf16) do { if (wdtype == 0) { expr_f32; } else { expr_bf16; } } while (0)
 
 void launch_ffn_gateup_gemv(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
-                            int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st, int static_table) {
+                            int act_stride, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st, int static_table,
+                            const uint32_t* gate_seq, uint32_t gate_want) {
   ++g_launches;
   const int tiles = (max_inter + 7) / 8;
   const int32_t* nd = nullptr;
-  WDISPATCH(launch_pdl(ffn_gateup_gemv_kernel<float>, dim3(n_probs * tiles), dim3(256), 0, st, u, probs, nd, tiles, H, act, act_stride, chunk_bytes, err, static_table),
-            launch_pdl(ffn_gateup_gemv_kernel<__nv_bfloat16>, dim3(n_probs * tiles), dim3(256), 0, st, u, probs, nd, tiles, H, act, act_stride, chunk_bytes, err, static_table));
+  WDISPATCH(launch_pdl(ffn_gateup_gemv_kernel<float>, dim3(n_probs * tiles), dim3(256), 0, st, u, probs, nd, tiles, H, act, act_stride, chunk_bytes, err, static_table, gate_seq, gate_want),
+            launch_pdl(ffn_gateup_gemv_kernel<__nv_bfloat16>, dim3(n_probs * tiles), dim3(256), 0, st, u, probs, nd, tiles, H, act, act_stride, chunk_bytes, err, static_table, gate_seq, gate_want));
 }
 void launch_ffn_down_gemv(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int max_inter,
                           int H, float* y, int wdtype, size_t chunk_bytes, int* err, cudaStream_t st, int static_table) {

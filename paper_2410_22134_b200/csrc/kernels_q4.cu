@@ -8,8 +8,8 @@
 // 0.515625 bytes per weight instead of 2, so a slot fill moves 3.88× fewer bytes over the link — the H2D term of the step
 // roofline shrinks by that factor and the HBM / latency terms start to matter.
 //
-// Decode: HBM-streaming GEMVs that dequantise in registers (one 16-byte load = 32 weights per lane and pass; the scale
-// multiplies the group's partial sum once).  Each CTA gates on the chunk-ready flags of exactly the code AND scale bytes it
+// Decode: HBM-streaming GEMVs that dequantise in registers (one 4-byte load = 8 weights per lane and block of 256; the
+// scale multiplies the block's partial sum once).  Each CTA gates on the chunk-ready flags of exactly the code AND scale bytes it
 // reads.  Prefill: the needed experts are dequantised (exactly) into an fp32 staging image and the fp32 SIMT grouped GEMM runs
 // on that; see dequant_q4_kernel for why not bf16 + tcgen05.
 #include <algorithm>
@@ -20,46 +20,64 @@ namespace pmk {
 
 constexpr int kQ4Group = 128;
 
-// Σ_k W[k]·x[k] over one quantised row of K elements (K % 128 == 0); summation order depends on (K, lane) only.
-// pass p: lane handles elements [p·1024 + lane·32, +32) — one 16-byte code load; 4 lanes share a scale.
-__device__ __forceinline__ float q4_dot32(const uint4& c, const float* __restrict__ x) {
-  const uint32_t w[4] = {c.x, c.y, c.z, c.w};
+// Σ_k W[k]·x[k] over quantised rows of K elements (K % 128 == 0); summation order depends on (K, lane) only.
+// Block b of 256 elements: lane handles the 8 elements [256·b + 8·lane, +8) — ONE 4-byte code load (a warp reads 128
+// contiguous bytes) and two float4 loads of x whose addresses are 32 bytes apart across lanes, i.e. the same L1 pattern as
+// the bf16 GEMVs.  (A first version gave each lane 32 consecutive elements per 16-byte load: the x loads of a warp then hit
+// 32 different 128-byte lines per instruction and the kernel ran at 0.49 TB/s, L1-wavefront bound.)  16 lanes share a scale.
+__device__ __forceinline__ float q4_dot8(uint32_t w, const float* __restrict__ x) {
+  const float4 x0 = __ldg(reinterpret_cast<const float4*>(x));
+  const float4 x1 = __ldg(reinterpret_cast<const float4*>(x + 4));
+  const float xv[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
   float acc = 0.f;
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    const float4 x0 = __ldg(reinterpret_cast<const float4*>(x + 8 * q));
-    const float4 x1 = __ldg(reinterpret_cast<const float4*>(x + 8 * q + 4));
-    const float xv[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      // nibble → float without an integer conversion: 2^23 + code as a bit pattern, minus (2^23 + 8)
-      const float v = __uint_as_float(0x4B000000u | ((w[q] >> (4 * i)) & 15u)) - 8388616.0f;
-      acc = fmaf(v, xv[i], acc);
-    }
+  for (int i = 0; i < 8; ++i) {
+    // nibble → float without an integer conversion: 2^23 + code as a bit pattern, minus (2^23 + 8)
+    const float v = __uint_as_float(0x4B000000u | ((w >> (4 * i)) & 15u)) - 8388616.0f;
+    acc = fmaf(v, xv[i], acc);
   }
   return acc;
 }
-template <int NP>
-__device__ __forceinline__ float row_dot_q4(const uint8_t* __restrict__ codes, const __nv_bfloat16* __restrict__ scales,
-                                            const float* __restrict__ x, int K, int lane) {
-  float tot = 0.f;
-  for (int k0 = 0; k0 < K; k0 += NP * 1024) {
-    uint4 c[NP]; float s[NP];
+// NR rows (1: a down row, 2: the gate and the up row of one output) against the same x; U blocks in flight per row.
+template <int NR, int U>
+__device__ __forceinline__ void rows_dot_q4(const uint8_t* const (&codes)[NR], const __nv_bfloat16* const (&scales)[NR],
+                                            const float* __restrict__ x, int K, int lane, float (&out)[NR]) {
+  float tot[NR];
 #pragma unroll
-    for (int p = 0; p < NP; ++p) {
-      const int k = k0 + p * 1024 + lane * 32;
+  for (int r = 0; r < NR; ++r) tot[r] = 0.f;
+  for (int k0 = 0; k0 < K; k0 += U * 256) {
+    uint32_t c[NR][U]; float s[NR][U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int k = k0 + u * 256 + lane * 8;
       if (k < K) {
-        c[p] = __ldcs(reinterpret_cast<const uint4*>(codes + (k >> 1)));
-        s[p] = __bfloat162float(scales[k / kQ4Group]);
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+          c[r][u] = __ldcs(reinterpret_cast<const unsigned int*>(codes[r] + (k >> 1)));
+          s[r][u] = __bfloat162float(scales[r][k / kQ4Group]);
+        }
       }
     }
 #pragma unroll
-    for (int p = 0; p < NP; ++p) {
-      const int k = k0 + p * 1024 + lane * 32;
-      if (k < K) tot = fmaf(s[p], q4_dot32(c[p], x + k), tot);
+    for (int u = 0; u < U; ++u) {
+      const int k = k0 + u * 256 + lane * 8;
+      if (k < K) {
+#pragma unroll
+        for (int r = 0; r < NR; ++r) tot[r] = fmaf(s[r][u], q4_dot8(c[r][u], x + k), tot[r]);
+      }
     }
   }
-  return warp_sum(tot);
+#pragma unroll
+  for (int r = 0; r < NR; ++r) out[r] = warp_sum(tot[r]);
+}
+template <int U>
+__device__ __forceinline__ float row_dot_q4(const uint8_t* codes, const __nv_bfloat16* scales, const float* __restrict__ x,
+                                            int K, int lane) {
+  const uint8_t* const c[1] = {codes};
+  const __nv_bfloat16* const sc[1] = {scales};
+  float o[1];
+  rows_dot_q4<1, U>(c, sc, x, K, lane, o);
+  return o[0];
 }
 
 struct Q4Image {       // byte offsets inside one expert image
@@ -71,14 +89,24 @@ __device__ __forceinline__ int q4_wait(const unsigned* flags, size_t b0, size_t 
 }
 
 // gate/up GEMV: act[p, i] = silu(Wg[i,:]·u) · (Wu[i,:]·u); grid = n_probs · ceil(inter/8), one warp per row
-__global__ void __launch_bounds__(256) ffn_gateup_gemv_q4_kernel(const float* __restrict__ u, const FfnProblem* __restrict__ probs,
+__global__ void __launch_bounds__(256, 5) ffn_gateup_gemv_q4_kernel(const float* __restrict__ u, const FfnProblem* __restrict__ probs,
                                                                  int tiles, int H, float* __restrict__ act, int act_stride,
-                                                                 size_t chunk_bytes, int* err) {
+                                                                 size_t chunk_bytes, int* err, const uint32_t* gate_seq,
+                                                                 uint32_t gate_want) {
   const int p = blockIdx.x / tiles, tile = blockIdx.x % tiles;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int r0 = tile * 8;
-  pdl_enter();
-  const FfnProblem pb = probs[p];
+  FfnProblem pb;
+  if (gate_seq) {       // wait for the problem table only, not for the predictor half of the slot-table kernel
+    __shared__ int gate_ok;
+    if (threadIdx.x == 0) gate_ok = wait_gate_word(gate_seq, gate_want, err);
+    __syncthreads();
+    if (!gate_ok) return;
+    pb = load_problem_cg(probs + p);
+  } else {
+    pdl_enter();
+    pb = probs[p];
+  }
   if (r0 >= pb.inter) return;
   const int r1 = min(pb.inter, r0 + 8);
   const Q4Image im(H, pb.inter);
@@ -98,10 +126,12 @@ __global__ void __launch_bounds__(256) ffn_gateup_gemv_q4_kernel(const float* __
   const int r = r0 + warp;
   if (r >= pb.inter) return;
   const uint8_t* img = (const uint8_t*)pb.wg;
-  const float g = row_dot_q4<2>(img + r * crow, (const __nv_bfloat16*)(img + 3 * im.nc + r * srow), u, H, lane);
-  const float v = row_dot_q4<2>(img + im.nc + r * crow, (const __nv_bfloat16*)(img + 3 * im.nc + im.ns + r * srow), u, H, lane);
+  const uint8_t* const cr[2] = {img + r * crow, img + im.nc + r * crow};
+  const __nv_bfloat16* const sr[2] = {(const __nv_bfloat16*)(img + 3 * im.nc + r * srow), (const __nv_bfloat16*)(img + 3 * im.nc + im.ns + r * srow)};
+  float gv[2];
+  rows_dot_q4<2, 4>(cr, sr, u, H, lane, gv);        // gate and up row: 8 loads in flight per lane
   pdl_done();
-  if (lane == 0) act[(size_t)p * act_stride + r] = silu(g) * v;
+  if (lane == 0) act[(size_t)p * act_stride + r] = silu(gv[0]) * gv[1];
 }
 
 // down GEMV: y[p, h] = Wd[h,:]·act[p,:]
@@ -129,7 +159,7 @@ __global__ void __launch_bounds__(256) ffn_down_gemv_q4_kernel(const float* __re
   const int r = r0 + warp;
   if (r >= H) return;
   const uint8_t* img = (const uint8_t*)pb.wg;
-  const float v = row_dot_q4<2>(img + 2 * im.nc + r * crow, (const __nv_bfloat16*)(img + 3 * im.nc + 2 * im.ns + r * srow),
+  const float v = row_dot_q4<8>(img + 2 * im.nc + r * crow, (const __nv_bfloat16*)(img + 3 * im.nc + 2 * im.ns + r * srow),
                                 act + (size_t)p * act_stride, pb.inter, lane);
   pdl_done();
   if (lane == 0) y[(size_t)p * H + r] = v;
@@ -173,7 +203,7 @@ __global__ void __launch_bounds__(256) ffn_down_combine_q4_kernel(const float* _
     const Q4Image im(H, pb.inter);
     const size_t crow = (size_t)pb.inter / 2, srow = (size_t)pb.inter / kQ4Group * 2;
     const uint8_t* img = (const uint8_t*)pb.wg;
-    const float v = row_dot_q4<2>(img + 2 * im.nc + r * crow, (const __nv_bfloat16*)(img + 3 * im.nc + 2 * im.ns + r * srow),
+    const float v = row_dot_q4<8>(img + 2 * im.nc + r * crow, (const __nv_bfloat16*)(img + 3 * im.nc + 2 * im.ns + r * srow),
                                   s_xv[j], pb.inter, lane);
     if (lane == 0) part[rr][j] = v;
   }
@@ -234,10 +264,12 @@ __global__ void __launch_bounds__(256) dequant_q4_kernel(const FfnProblem* __res
 }
 
 void launch_ffn_gateup_gemv_q4(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
-                               int act_stride, size_t chunk_bytes, int* err, cudaStream_t st) {
+                               int act_stride, size_t chunk_bytes, int* err, cudaStream_t st, const uint32_t* gate_seq,
+                               uint32_t gate_want) {
   ++g_launches;
   const int tiles = (max_inter + 7) / 8;
-  launch_pdl(ffn_gateup_gemv_q4_kernel, dim3(n_probs * tiles), dim3(256), 0, st, u, probs, tiles, H, act, act_stride, chunk_bytes, err);
+  launch_pdl(ffn_gateup_gemv_q4_kernel, dim3(n_probs * tiles), dim3(256), 0, st, u, probs, tiles, H, act, act_stride, chunk_bytes, err,
+             gate_seq, gate_want);
 }
 void launch_ffn_down_gemv_q4(const float* act, int act_stride, const FfnProblem* probs, int n_probs, int H, float* y,
                              size_t chunk_bytes, int* err, cudaStream_t st) {

@@ -74,7 +74,8 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
                                                          int inter, int wbytes, FfnProblem* problems,
                                                          int32_t* n_problems, int32_t* row_of, LayerCmd* cmd,
                                                          uint32_t seq, int32_t* trace_precise,
-                                                         int32_t* trace_pred, RouteFuse rf, LayerCmd* cmd2, int mode) {
+                                                         int32_t* trace_pred, RouteFuse rf, LayerCmd* cmd2, int mode,
+                                                         const LayerCmd* cmd_prev) {
   __shared__ uint8_t needed[kMaxE];
   __shared__ uint8_t prot[kMaxE];
   __shared__ int16_t order[kMaxE];
@@ -109,6 +110,14 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     else if (E <= 64) front_route<2>(rf, E, lane, f_sel[0], f_val[0]);
     else if (E <= 128) front_route<4>(rf, E, lane, f_sel[0], f_val[0]);
     else front_route<8>(rf, E, lane, f_sel[0], f_val[0]);
+  }
+  // The expert kernels of the layer before this one did not wait for the END of that layer's slot-table kernel (gate word),
+  // so nothing in the stream order says its table rows have been written back: wait for its `seq_done`.
+  if (cmd_prev) {
+    __shared__ int prev_ok;
+    if (threadIdx.x == 0) prev_ok = wait_gate_word((const unsigned*)&cmd_prev->seq_done, seq - 1u, nullptr);
+    __syncthreads();
+    (void)prev_ok;      // a time-out here surfaces through the expert kernels' own flag waits
   }
   for (int i = threadIdx.x; i < C; i += blockDim.x) {
     t_se[0][i] = tbl.slot_expert[(size_t)m * C + i]; t_stamp[0][i] = tbl.stamp[(size_t)m * C + i];
@@ -356,20 +365,26 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     if (have_t) tbl.expert_slot[(size_t)mt_ * E + e] = t_es[1][e];
   }
   if (threadIdx.x == 0) *tbl.clock = t_clock;
+  if (cmd2) {           // table rows are back in global memory: the next layer's kernel may read them
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&cmd2->seq_done), "r"(seq) : "memory");
+  }
 }
 
 void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int32_t* sel, int T, int k, const int32_t* offset,
                        const int32_t* pred_list, int reorder, const uint8_t* slot_base, size_t slot_bytes,
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
-                       int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf, LayerCmd* cmd_dev2) {
+                       int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf, LayerCmd* cmd_dev2,
+                       const LayerCmd* cmd_prev) {
   ++g_launches;
   const int mode = reorder;     // bit 0: reordered inference / 0 = ID order (G16); bit 1: demote mispredictions (G17)
   RouteFuse f{};
   if (rf) f = *rf;
   launch_pdl(slot_table_kernel, dim3(1), dim3((rf && T == 1) ? 1024 : 256), 0, st, tbl, m, stride, max_spec, sel, T, k, offset, pred_list,
              slot_base, slot_bytes, flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of, cmd, seq,
-             trace_precise, trace_pred, f, cmd_dev2, mode);
+             trace_precise, trace_pred, f, cmd_dev2, mode, cmd_prev);
 }
 
 // Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every

@@ -171,13 +171,16 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   launch_slot_table(h->tbl, m, h->o.stride, h->max_spec_decode, sel, 1, k, nullptr, plist,
                     ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb, h->problems,
                     h->n_prob, h->row_of, h->cmd_dev + m, seq, h->trace_precise + (size_t)m * (1 + 5 * E),
-                    (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf, h->cmd_fetch + m);
+                    (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf, h->cmd_fetch + m,
+                    m > 0 ? h->cmd_fetch + (m - 1) : nullptr);
   // A7 runs beside this stream: the fetch worker (kernels_fetch.cu, resident since the start of the step) sees the
   // command K5 publishes in device memory and pulls the missing chunks over the link; the flag-gated kernels K6/K7 are
   // enqueued right away and wait (ld.acquire.sys on the chunk flags, __nanosleep between polls) for exactly the bytes
   // they read.  The host is not in the layer loop at all.
-  if (h->q4) launch_ffn_gateup_gemv_q4(h->u, h->problems, k, I, H, h->act, I, h->chunk_bytes, h->err_dev, cs);      // K6 (INT4)
-  else launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs);      // K6
+  // K6 waits for the gate word K5 publishes behind the problem table (not for K5's predictor half)
+  const uint32_t* gate_word = (const uint32_t*)&h->cmd_fetch[m].seq;
+  if (h->q4) launch_ffn_gateup_gemv_q4(h->u, h->problems, k, I, H, h->act, I, h->chunk_bytes, h->err_dev, cs, gate_word, seq);      // K6 (INT4)
+  else launch_ffn_gateup_gemv(h->u, h->problems, k, I, H, h->act, I, wd, h->chunk_bytes, h->err_dev, cs, 0, gate_word, seq);      // K6
   if (s.n_shared_inter && cudaStreamWaitEvent(cs, h->ev_join, 0) != cudaSuccess) { h->err = "join of the shared-expert stream failed"; return PROMOE_ECUDA; }
   if (h->q4) {                                                                                             // K7 (INT4)
     launch_ffn_down_combine_q4(h->act, I, h->problems, h->row_of, gates, k, (s.n_shared_inter && s.shared_gate) ? h->sgate : nullptr,
@@ -219,8 +222,9 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
   if (T > 1) RC(ce_retire(h, true));   // prefill orders compute after fills with events: start from a drained copy stream
   memcpy(h->ids_pin, ids_host, (size_t)T * 4);
   CKS(cudaMemcpyAsync(h->ids, h->ids_pin, (size_t)T * 4, cudaMemcpyHostToDevice, cs));
-  if (fused) {     // A7 of this step: the device-side fetch worker, resident before anything that may wait for it
-    CKS(cudaMemsetAsync(h->fetch_ctr, 0, sizeof(unsigned long long) * kFetchCounters, h->fs));
+  const bool worker = fused && h->fetch_ctas > 0;
+  if (fused) CKS(cudaMemsetAsync(h->fetch_ctr, 0, sizeof(unsigned long long) * kFetchCounters, h->fs));
+  if (worker) {    // A7 of this step: the device-side fetch worker, resident before anything that may wait for it
     FetchArgs fa{};
     fa.cmd = h->cmd_fetch; fa.src = h->src_dev; fa.slots = h->slots; fa.Be = h->Be; fa.chunk_bytes = h->chunk_bytes;
     fa.flags = h->flags; fa.claims = h->claims; fa.complete = h->complete; fa.ctr = h->fetch_ctr; fa.err = h->err_dev;
@@ -237,7 +241,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
   }
   int rc_layers = PROMOE_OK;
   if (e_end == cudaSuccess) {
-    launch_embed(h->ids, h->emb, h->x, T, H, wd, cs, fused ? h->alive : nullptr, step_seq, h->err_dev);
+    launch_embed(h->ids, h->emb, h->x, T, H, wd, cs, worker ? h->alive : nullptr, step_seq, h->err_dev);
     rc_layers = run_layers(h, T, step_seq, pos0, fused);
   }
   if (rc_layers == PROMOE_OK && e_end == cudaSuccess) {   // ---- last token: final norm + lm_head
