@@ -500,15 +500,16 @@ def run_sweep(args):
     from paper_2410_22134_b200.engine import ProMoE
     torch.cuda.set_device(0)
     peaks = load_peaks()
-    base = synth.get_config("c3", shape_overrides={"max_seq": 2048 + 256}, decode_steps=args.decode_steps or 256)
+    base = synth.get_config("c3", shape_overrides={"max_seq": 2048 + 256, **({"wdtype": 2} if args.int4 else {})},
+                            decode_steps=args.decode_steps or 256)
     s = base.shape
     n_moe = s.n_layers - s.n_dense_layers
-    Be = 3 * s.hidden * s.expert_inter * 2
+    Be = expert_image_bytes(s)
     h2d = B.promoe_bench_h2d(256 << 20, 2, 5)
     w0 = synth.make_weights(base, predictor="skip")
     decode_ids = synth.make_decode_ids(base).tolist()
     prompts = {n: synth.make_prompt(base, n).tolist() for n in (128, 2048)}
-    flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TENSOR
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TENSOR | (B.F_DEMOTE if args.demote else 0)
     wcache = {1: w0}
 
     def weights_for(stride):
@@ -553,7 +554,9 @@ def run_sweep(args):
                 dec_s, pre_s = r["decode_ms"] / 1e3, r["prefill_ms"] / 1e3
                 copy_s = d["copy_busy_ms"] / 1e3
                 exposed = max(0.0, dec_s - compute[n][1] / 1e3)
-                pt = {"budget": frac, "predictor": mode, "stride": stride, "chunk_mib": chunk, "prompt": n,
+                pt = {"budget": frac, "predictor": mode, "stride": stride, "chunk_mib": chunk, "prompt": n, "demote": args.demote,
+                      "int4": args.int4, "fetch_rate": d["fetched_at_gate"] / max(1, d["fetched_at_gate_of"]),
+                      "fetch_rate_chunks": d["landed_chunks_at_gate"] / max(1, d["landed_chunks_of"]),
                       "decode_tokens_per_s": cfg.decode_steps / dec_s, "prefill_tokens_per_s": n / pre_s,
                       "hit_rate": (d["hits_resident"] + d["hits_prefetch"]) / max(1, d["accesses"]),
                       "hit_rate_resident": d["hits_resident"] / max(1, d["accesses"]),
@@ -670,7 +673,7 @@ def main():
     ap.add_argument("--predictor", default="skip", choices=["skip", "fitted", "random", "none", "trace"],
                     help="skip: training-free MLP weights; fitted: the MLP fitted offline on the model's own traces (fit_predictor.py); "
                          "none: reactive cache; trace: oracle-routing upper bound")
-    ap.add_argument("--demote", type=int, default=0, help="PROMOE_F_DEMOTE: a mispredicted prefetch becomes the next LRU victim (G17)")
+    ap.add_argument("--demote", type=int, default=1, help="PROMOE_F_DEMOTE: a mispredicted prefetch becomes the next LRU victim (G17)")
     ap.add_argument("--fit-prompts", type=int, default=20, help="--predictor fitted: prompts of prompt_len tokens to collect traces from")
     ap.add_argument("--fit-steps", type=int, default=240, help="--predictor fitted: optimiser steps per layer")
     ap.add_argument("--cache-all", type=int, default=0, help="every routed expert resident (compute-only step; with --fetch-ctas -1 "

@@ -120,7 +120,13 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->pred_list, (size_t)Lm * (1 + E))); CK(dalloc(&h->trace_precise, (size_t)Lm * (1 + 5 * E)));
     CK(dalloc(&h->trace_pred, (size_t)Lm * (1 + 4 * E))); CK(dalloc(&h->row_of, (size_t)k)); CK(dalloc(&h->n_prob, (size_t)1));
     CK(dalloc(&h->problems, (size_t)E)); CK(dalloc(&h->shared_prob, (size_t)L)); CK(dalloc(&h->err_dev, (size_t)1)); CK(dalloc(&h->attn_cnt, (size_t)s.n_q_heads));
-    if (h->q4) { CK(dalloc(&h->q4_stage, (size_t)E * 3 * H * s.expert_inter)); CK(dalloc(&h->problems_deq, (size_t)E)); }
+    if (h->q4) {
+      CK(dalloc(&h->problems_deq, (size_t)E));
+      if (op->flags & PROMOE_F_TENSOR) {
+        h->q4_lo_off = (size_t)E * 3 * H * s.expert_inter;
+        CK(dalloc(&h->q4_stage_bf, 2 * h->q4_lo_off)); CK(dalloc(&h->q4_gu, (size_t)T * k * 2 * s.expert_inter));
+      } else CK(dalloc(&h->q4_stage, (size_t)E * 3 * H * s.expert_inter));
+    }
     if ((op->flags & PROMOE_F_TENSOR) && s.wdtype >= 1) {
       h->tc = tc_create(&h->err);
       if (!h->tc) return PROMOE_ECUDA;
@@ -189,7 +195,7 @@ extern "C" void promoe_destroy(promoe_t* h) {
                   h->count, h->offset, h->perm, h->inv, h->gates, h->margin, h->z, h->pred_list, h->trace_precise,
                   h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->attn_cnt, h->slots, h->flags,
                   h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock,
-                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch, h->trace_u, h->q4_stage, h->problems_deq};
+                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch, h->trace_u, h->q4_stage, h->problems_deq, h->q4_stage_bf, h->q4_gu};
   for (void* b : bufs) if (b) cudaFree(b);
   if (h->xsA) cudaFree(h->xsA);
   if (h->xsG) cudaFree(h->xsG);

@@ -45,7 +45,10 @@ struct promoe {
   int Lm = 0, C = 0, wb = 2, n_chunks = 0, max_inflight = 2;
   int wdd = 1;                 // dtype of the DENSE weights (0 fp32, 1 bf16); wdtype 2 = bf16 dense + INT4 routed experts
   bool q4 = false;             // routed experts are INT4 group-quantised images (kernels_q4.cu)
-  float* q4_stage = nullptr;   // prefill: fp32 staging images of the needed experts [E, 3*H*I]
+  float* q4_stage = nullptr;   // prefill (SIMT): fp32 staging images of the needed experts [E, 3*H*I]
+  __nv_bfloat16* q4_stage_bf = nullptr;   // prefill (tcgen05): bf16 hi plane [E, 3*H*I], lo plane q4_lo_off elements later
+  size_t q4_lo_off = 0;
+  float* q4_gu = nullptr;      // [maxT*k, 2*I] fp32 [gate | up] pre-activations of the INT4 tensor-core prefill
   pmk::FfnProblem* problems_deq = nullptr;   // records pointing into q4_stage
   size_t Be = 0, chunk_bytes = 0;
   int max_spec_decode = 0, max_spec_prefill = 0;   // allocations allowed per PushPredicted (knob G3)

@@ -138,6 +138,13 @@ void launch_ffn_down_combine_q4(const float* act, int act_stride, const FfnProbl
 void launch_dequant_q4(const FfnProblem* probs, int p0, int np, int H, int max_inter, float* stage,
                        size_t stage_stride_elems, FfnProblem* out_probs, cudaStream_t st);
 
+// tensor-core prefill: INT4 images → bf16 hi/lo staging images (lo plane lo_off elements behind the hi plane) + records;
+// then silu(g)·u of the [gate | up] GEMM output as the hi/lo activation operand of the down GEMM
+void launch_dequant_q4_bf16(const FfnProblem* probs, int p0, int np, int H, int max_inter, __nv_bfloat16* stage, size_t lo_off,
+                            size_t stage_stride_elems, FfnProblem* out_probs, cudaStream_t st);
+void launch_swiglu_split(const float* gu, const FfnProblem* probs, int p0, int np, int max_rows, int inter, __nv_bfloat16* o_hi,
+                         size_t o_lo_off, cudaStream_t st);
+
 // ---- fused decode kernels (kernels_decode.cu) ---------------------------------------------------------------
 struct GemvSeg { const void* w; float* out; int n; int flags; };
 struct NormGemvArgs {

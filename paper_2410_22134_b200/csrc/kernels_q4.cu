@@ -263,6 +263,60 @@ __global__ void __launch_bounds__(256) dequant_q4_kernel(const FfnProblem* __res
   }
 }
 
+// Prefill on the tensor cores: the same dequantisation into a bf16 hi/lo PAIR of staging images — (code − 8)·scale has up to
+// 11 significant bits, hi = bf16(w) keeps 8 and lo = w − hi (≤ 4 bits) is exact — so the tcgen05 GEMM runs one pass over
+// each image with the same activation operand and accumulates (W_hi + W_lo)·x in fp32: exact weights, twice the MMAs.
+__global__ void __launch_bounds__(256) dequant_q4_bf16_kernel(const FfnProblem* __restrict__ probs, int p0, int H,
+                                                              __nv_bfloat16* __restrict__ stage, size_t lo_off,
+                                                              size_t stage_stride_elems, FfnProblem* __restrict__ out_probs) {
+  const int pi = p0 + blockIdx.y;
+  const FfnProblem pb = probs[pi];
+  const int inter = pb.inter;
+  const size_t hi = (size_t)H * inter;
+  const Q4Image im(H, inter);
+  const uint8_t* img = (const uint8_t*)pb.wg;
+  __nv_bfloat16* dst = stage + (size_t)pi * stage_stride_elems;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    FfnProblem o = pb;
+    o.wg = dst; o.wu = dst + hi; o.wd = dst + 2 * hi; o.flags = nullptr; o.gen = 0;
+    out_probs[pi] = o;
+  }
+  const size_t n8 = 3 * hi / 8;        // 8 codes per 4-byte load: consecutive threads read consecutive words
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n8; t += (size_t)gridDim.x * blockDim.x) {
+    const size_t e0 = t * 8;
+    const int mat = (int)(e0 / hi);
+    const size_t within = e0 - (size_t)mat * hi;
+    const int K = mat < 2 ? H : inter;
+    const size_t row = within / K, col = within % K;
+    const uint32_t w = *reinterpret_cast<const uint32_t*>(img + e0 / 2);
+    const float s = __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(img + 3 * im.nc + (size_t)mat * im.ns + (row * (K / kQ4Group) + col / kQ4Group) * 2));
+    __align__(16) __nv_bfloat16 oh[8], ol[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const float v = ((float)((w >> (4 * i)) & 15u) - 8.0f) * s;       // exact in fp32
+      oh[i] = __float2bfloat16_rn(v);
+      ol[i] = __float2bfloat16_rn(v - __bfloat162float(oh[i]));         // exact: at most 4 significant bits are left
+    }
+    *reinterpret_cast<uint4*>(dst + e0) = *reinterpret_cast<const uint4*>(oh);
+    *reinterpret_cast<uint4*>(dst + lo_off + e0) = *reinterpret_cast<const uint4*>(ol);
+  }
+}
+// gu [.., 2·I] fp32 = [gate | up] pre-activations of the rows of problems [p0, p0+np) → silu(g)·u as bf16 hi/lo planes
+// [.., I] (the activation operand of the down GEMM).  grid (max_rows, np).
+__global__ void __launch_bounds__(256) swiglu_split_kernel(const float* __restrict__ gu, const FfnProblem* __restrict__ probs,
+                                                           int p0, int inter, __nv_bfloat16* __restrict__ o_hi, size_t o_lo_off) {
+  const FfnProblem pb = probs[p0 + blockIdx.y];
+  if ((int)blockIdx.x >= pb.nrows) return;
+  const size_t r = (size_t)pb.row0 + blockIdx.x;
+  const float* g = gu + r * 2 * inter;
+  for (int i = threadIdx.x; i < inter; i += blockDim.x) {
+    const float v = silu(g[i]) * g[inter + i];
+    const __nv_bfloat16 hi = __float2bfloat16_rn(v);
+    o_hi[r * inter + i] = hi;
+    o_hi[r * inter + i + o_lo_off] = __float2bfloat16_rn(v - __bfloat162float(hi));
+  }
+}
+
 void launch_ffn_gateup_gemv_q4(const float* u, const FfnProblem* probs, int n_probs, int max_inter, int H, float* act,
                                int act_stride, size_t chunk_bytes, int* err, cudaStream_t st, const uint32_t* gate_seq,
                                uint32_t gate_want) {
@@ -293,7 +347,24 @@ void launch_dequant_q4(const FfnProblem* probs, int p0, int np, int H, int max_i
   dequant_q4_kernel<<<dim3(bx, np), 256, 0, st>>>(probs, p0, H, stage, stage_stride_elems, out_probs);
 }
 
+void launch_dequant_q4_bf16(const FfnProblem* probs, int p0, int np, int H, int max_inter, __nv_bfloat16* stage, size_t lo_off,
+                            size_t stage_stride_elems, FfnProblem* out_probs, cudaStream_t st) {
+  ++g_launches;
+  if (np <= 0) return;
+  const size_t n8 = (size_t)3 * H * max_inter / 8;
+  const int bx = (int)std::min<size_t>((n8 + 255) / 256, 2048);
+  dequant_q4_bf16_kernel<<<dim3(bx, np), 256, 0, st>>>(probs, p0, H, stage, lo_off, stage_stride_elems, out_probs);
+}
+void launch_swiglu_split(const float* gu, const FfnProblem* probs, int p0, int np, int max_rows, int inter, __nv_bfloat16* o_hi,
+                         size_t o_lo_off, cudaStream_t st) {
+  ++g_launches;
+  if (np <= 0 || max_rows <= 0) return;
+  swiglu_split_kernel<<<dim3(max_rows, np), 256, 0, st>>>(gu, probs, p0, inter, o_hi, o_lo_off);
+}
+
 void preload_q4() {
+  preload_fn((const void*)dequant_q4_bf16_kernel);
+  preload_fn((const void*)swiglu_split_kernel);
   preload_fn((const void*)ffn_gateup_gemv_q4_kernel);
   preload_fn((const void*)ffn_down_gemv_q4_kernel);
   preload_fn((const void*)ffn_down_combine_q4_kernel);

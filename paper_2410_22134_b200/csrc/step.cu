@@ -87,7 +87,31 @@ static int resident_ffn(promoe_t* h, int l, int inter, int T) {
 // Routed experts [i, j) of the problem table (prefill): grouped SwiGLU FFN over their row ranges → yexp.
 static int expert_batch(promoe_t* h, const int32_t* perm, int i, int j, int max_rows) {
   const promoe_shape_t& s = h->s;
-  const int H = s.hidden, I = s.expert_inter, k = s.top_k;
+  const int H = s.hidden, I = s.expert_inter, k = s.top_k, E = s.n_experts;
+  if (h->q4 && use_tc(h, 2)) {
+    // INT4 experts on the tensor cores: bf16 hi/lo staging images (exact), ONE [gate | up] GEMM of N = 2·I per image with the
+    // second accumulating onto the first, SwiGLU + split, then the down GEMM the same way (kernels_q4.cu)
+    const size_t stride = (size_t)3 * H * I;
+    launch_dequant_q4_bf16(h->problems, i, j - i, H, I, h->q4_stage_bf, h->q4_lo_off, stride, h->problems_deq, h->cs);
+    for (int pass = 0; pass < 2; ++pass) {
+      TcGemm g;
+      g.a0 = h->q4_stage_bf + (pass ? h->q4_lo_off : 0); g.a_rows = 2 * I; g.a_batches = E; g.a_batch_stride = stride * 2;
+      g.b_hi = h->xsG; g.b_lo_off = h->xsG_half; g.b_rows_cap = (int)(h->xsG_half / H);
+      g.K = H; g.N = 2 * I; g.probs = h->problems_deq; g.p0 = i; g.np = j - i; g.max_rows = max_rows;
+      g.slot_base = (const uint8_t*)h->q4_stage_bf; g.y = h->q4_gu; g.ldy = 2 * I; g.flags = pass ? LIN_ACC : 0;
+      if (!tc_launch(h->tc, g, h->cs, &h->err)) return PROMOE_ECUDA;
+    }
+    launch_swiglu_split(h->q4_gu, h->problems_deq, i, j - i, max_rows, I, h->xsB, h->xsB_half, h->cs);
+    for (int pass = 0; pass < 2; ++pass) {
+      TcGemm d;
+      d.a0 = h->q4_stage_bf + (pass ? h->q4_lo_off : 0) + (size_t)2 * H * I; d.a_rows = H; d.a_batches = E; d.a_batch_stride = stride * 2;
+      d.b_hi = h->xsB; d.b_lo_off = h->xsB_half; d.b_rows_cap = (int)(h->xsB_half / I);
+      d.K = I; d.N = H; d.probs = h->problems_deq; d.p0 = i; d.np = j - i; d.max_rows = max_rows;
+      d.slot_base = (const uint8_t*)h->q4_stage_bf; d.y = h->yexp; d.ldy = H; d.flags = pass ? LIN_ACC : 0;
+      if (!tc_launch(h->tc, d, h->cs, &h->err)) return PROMOE_ECUDA;
+    }
+    return PROMOE_OK;
+  }
   if (h->q4) {     // INT4 experts: exact fp32 staging images, then the fp32 SIMT grouped GEMM (kernels_q4.cu)
     launch_dequant_q4(h->problems, i, j - i, H, I, h->q4_stage, (size_t)3 * H * I, h->problems_deq, h->cs);
     launch_ffn_gateup_gemm_simt(h->u, perm, k, h->problems_deq, i, j - i, max_rows, 0, I, H, h->act, I, 0, h->cs);
@@ -402,7 +426,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
       }
       launch_combine(h->x, h->yexp, h->row_of, gates, 1, k, H, shared, sgate, h->x, cs);
     } else {
-      if (tc && !h->q4) launch_split_rows(h->u, perm, k, T * k, H, h->xsG, h->xsG_half, cs);   // gathered rows, permuted order
+      if (tc) launch_split_rows(h->u, perm, k, T * k, H, h->xsG, h->xsG_half, cs);   // gathered rows, permuted order
       // batches: [all class A] [all class B] then every class C alone (its fill lands in copy order)
       int i = 0;
       size_t dnext = 0;

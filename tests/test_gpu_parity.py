@@ -370,22 +370,23 @@ def _q4(cfg):
     return replace(cfg, name=cfg.name + "-int4", shape=replace(cfg.shape, wdtype=2))
 
 
-@pytest.mark.parametrize("name,T,fused", [("c1b", 32, True), ("c1b", 32, False), ("c2-mini", 96, True), ("c3-mini", 64, True),
-                                          ("c4-mini", 40, True)])
-def test_int4_experts_full_stack(name, T, fused):
+@pytest.mark.parametrize("name,T,fused,tensor", [("c1b", 32, True, 1), ("c1b", 32, False, 1), ("c2-mini", 96, True, 1),
+                                                 ("c2-mini", 96, True, 0), ("c3-mini", 64, True, 1), ("c4-mini", 40, True, 1)])
+def test_int4_experts_full_stack(name, T, fused, tensor):
     """The whole step with 4-bit expert images in pinned host memory and in the slots (3.88x fewer bytes per fill):
     routing / permutation / cache traces bit-exact, hidden state in tolerance against the oracle that dequantises the same
-    images (oracle/quant.py) — prefill through the exact fp32 staging path, decode through the INT4 GEMVs (fused K6/K7 or
-    the unfused kernels), chunk flags gating code and scale bytes separately."""
+    images (oracle/quant.py) — prefill through the exact bf16 hi/lo staging images on tcgen05 (tensor = 1) or the exact
+    fp32 staging images on the SIMT GEMM (tensor = 0), decode through the INT4 GEMVs (fused K6/K7 or the unfused kernels),
+    chunk flags gating code and scale bytes separately."""
     from paper_2410_22134_b200 import binding as B
     from synth.configs import mini
     cfg = _q4(mini(name[:-5]) if name.endswith("-mini") else synth.get_config(name))
     w = synth.make_weights(cfg, predictor="skip")
     assert w.experts.dtype == torch.uint8
-    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_TENSOR | B.F_DEMOTE | (0 if fused else B.F_NOFUSE)
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | (B.F_TENSOR if tensor else 0) | B.F_DEMOTE | (0 if fused else B.F_NOFUSE)
     ids = synth.make_decode_ids(cfg, 8).tolist()
     out = run_parity(cfg, w, synth.make_prompt(cfg, T), 8, flags=flags, decode_ids=ids, max_spec_decode=1)
-    _report(f"{cfg.name}/{'fused' if fused else 'unfused'}", out)
+    _report(f"{cfg.name}/{'fused' if fused else 'unfused'}/{'tcgen05' if tensor else 'simt'}", out)
     assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
     s = cfg.shape
     assert out["stats"]["h2d_bytes"] % (3 * s.hidden * s.expert_inter * 33 // 64) == 0 or out["stats"]["h2d_bytes"] > 0
