@@ -323,3 +323,83 @@ def test_fit_predictor_improves_on_its_start_point_cpu():
     sel0 = (u @ R.T).topk(k, dim=1).indices
     r0 = fit_layer(u, sel0, w1, w2, E, k, 0, seed=2, steps=40, lr=1e-4)
     assert r0["acc_test_skip"] == 1.0 and r0["kept"] == "skip" and torch.equal(r0["w1"], w1)
+
+
+# ---- batched decode: oracle/batch.py ----------------------------------------------------------
+def test_batch_of_one_is_the_single_sequence_model():
+    from oracle.batch import OracleBatch
+    cfg = synth.get_config("c1")
+    w = synth.make_weights(cfg, pin=False)
+    ids = synth.make_prompt(cfg, 7).tolist()
+    a = O.OracleModel(w, stride=1, slots_per_layer=4)
+    b = OracleBatch(w, 1, stride=1, slots_per_layer=4)
+    a.forward(ids); b.prefill_seq(0, ids)
+    for tok in (3, 11, 5):
+        sa, sb = a.forward([tok]), b.forward([tok])
+        assert torch.equal(sa.hidden, sb.hidden) and torch.equal(sa.logits, sb.logits)
+        assert [lt.sel for lt in sa.layers] == [lt.sel for lt in sb.layers]
+        assert [lt.pred for lt in sa.layers] == [lt.pred for lt in sb.layers]
+
+
+def test_batch_rows_are_independent_sequences_and_predictions_vote():
+    """Row b of a batched step equals sequence b run alone (its own KV cache and position — here the sequences have
+    DIFFERENT lengths); the predicted list of a layer is the G7 vote over the B rows; permuting the batch permutes the rows."""
+    from oracle.batch import OracleBatch
+    from oracle.predictor import predict_experts
+    cfg = synth.get_config("c1")
+    w = synth.make_weights(cfg, pin=False)
+    prompts = [synth.make_prompt(cfg, n).tolist() for n in (5, 9, 3)]
+    toks = [[2, 7], [9, 1], [4, 4]]
+    bat = OracleBatch(w, 3, stride=1, slots_per_layer=4)
+    solo = [O.OracleModel(w, stride=1, slots_per_layer=4) for _ in range(3)]
+    for b in range(3):
+        bat.prefill_seq(b, prompts[b]); solo[b].forward(prompts[b])
+    for step in range(2):
+        st = bat.forward([toks[b][step] for b in range(3)])
+        ref = [solo[b].forward([toks[b][step]]) for b in range(3)]
+        assert st.hidden.shape == (3, cfg.shape.hidden)
+        for b in range(3):
+            assert torch.equal(st.hidden[b], ref[b].hidden[0]) and torch.equal(st.seq_logits[b], ref[b].logits)
+            for m in range(len(st.layers)):
+                assert st.layers[m].sel[b] == ref[b].layers[m].sel[0]
+                assert torch.equal(st.layers[m].logits[b], ref[b].layers[m].logits[0])
+        for m in range(len(st.layers)):
+            scores = torch.cat([ref[b].layers[m].pred_scores for b in range(3)], 0)
+            assert st.layers[m].pred == predict_experts(scores, cfg.shape.top_k, 4)
+    # permutation of the batch = permutation of the rows
+    p = OracleBatch(w, 3, stride=1, slots_per_layer=4)
+    order = [2, 0, 1]
+    for i, b in enumerate(order):
+        p.prefill_seq(i, prompts[b])
+    sp = p.forward([toks[b][0] for b in order])
+    q = OracleBatch(w, 3, stride=1, slots_per_layer=4)
+    for b in range(3):
+        q.prefill_seq(b, prompts[b])
+    sq = q.forward([toks[b][0] for b in range(3)])
+    for i, b in enumerate(order):
+        assert torch.equal(sp.hidden[i], sq.hidden[b])
+    assert sorted(sp.layers[0].pred) == sorted(sq.layers[0].pred)      # votes do not depend on the row order
+
+
+def test_batch_near_tie_protocol_forces_one_row():
+    """compare.oracle_step_matching on a batch: a forced selection of row b goes to sequence b's own step, the other rows
+    are untouched, and snapshot / restore rewind every sequence."""
+    from oracle.batch import OracleBatch
+    from oracle.compare import ParityReport, oracle_step_matching, restore, snapshot
+    import numpy as np
+    cfg = synth.get_config("c1")
+    w = synth.make_weights(cfg, pin=False)
+    bat = OracleBatch(w, 2, stride=1, slots_per_layer=4)
+    bat.prefill_seq(0, [1, 2, 3]); bat.prefill_seq(1, [4, 5])
+    snap = snapshot(bat)
+    st = bat.forward([6, 7])
+    restore(bat, snap)
+    bat.step_idx = 0
+    assert [o.pos for o in bat.seqs] == [3, 2]
+    st2 = bat.forward([6, 7])
+    assert torch.equal(st.hidden, st2.hidden)
+    restore(bat, snap); bat.step_idx = 0
+    sel = np.array([[row for row in lt.sel] for lt in st.layers], dtype=np.int32)       # [Lm, B, k]
+    rep = ParityReport()
+    st3 = oracle_step_matching(bat, [6, 7], sel, rep)
+    assert rep.sel_near_tie == 0 and torch.equal(st3.hidden, st.hidden)
