@@ -655,6 +655,60 @@ def run_modes(args):
     print(json.dumps({"modes": "ladder" if args.ladder else "goodpred", "rows": len(rows), "h2d_gbs": h2d}), flush=True)
 
 
+def run_batch_sweep(args):
+    """PAPER.md §7.5: decode at batch sizes 1-4.  nb sequences with their own seeded prompts are prefilled one
+    by one, then every decode step is ONE promoe_decode_batch call (one gate / slot-table step per layer over the union of
+    the rows' experts).  One JSON line per batch size: tokens/s = nb x steps / device time."""
+    import dataclasses
+    import torch
+    import synth
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+    torch.cuda.set_device(0)
+    over = {}
+    if args.prompt_len:
+        over["prompt_len"] = args.prompt_len
+    if args.decode_steps:
+        over["decode_steps"] = args.decode_steps
+    if args.int4:
+        over["shape_overrides"] = {"wdtype": 2}
+    cfg = synth.get_config(args.config, **over)
+    s = cfg.shape
+    Be = expert_image_bytes(s)
+    h2d = B.promoe_bench_h2d(256 << 20, 2, 5)
+    w = synth.make_weights(cfg, predictor="skip")
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_WARM | (B.F_TENSOR if args.tensor else 0) | (B.F_DEMOTE if args.demote else 0)
+    pm = B.PRED_NONE if args.predictor == "none" else B.PRED_MLP
+    for nb in (1, 2, 3, 4):
+        g = torch.Generator().manual_seed(4242)
+        prompts = [torch.randint(0, s.vocab, (cfg.prompt_len,), generator=g, dtype=torch.int32).tolist() for _ in range(nb)]
+        dec = torch.randint(0, s.vocab, (cfg.decode_steps, nb), generator=g, dtype=torch.int32).tolist()
+        eng = ProMoE(w, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_kb << 10, predictor_mode=pm, flags=flags,
+                     max_spec_decode=args.max_spec_decode, max_spec_prefill=args.max_spec_prefill, fetch_ctas=args.fetch_ctas,
+                     max_batch=nb)
+        res = None
+        for rep_ in range(2):                     # one warm-up pass, one timed
+            eng.reset()
+            for b in range(nb):
+                eng.prefill_seq(b, prompts[b], want_logits=False)
+            s1 = eng.stats()
+            for row in dec:
+                eng.decode_batch(list(range(nb)), row)
+            s2 = eng.stats()
+            res = {k: s2[k] - s1[k] for k in s1}
+        eng.close()
+        dec_s = res["step_ms"] / 1e3
+        line = {"mode": "batched decode", "config": cfg.name, "batch": nb, "int4": args.int4, "predictor": args.predictor,
+                "decode_tokens_per_s": nb * cfg.decode_steps / dec_s, "ms_per_step": 1e3 * dec_s / cfg.decode_steps,
+                "experts_needed_per_layer_step": res["accesses"] / (cfg.decode_steps * (s.n_layers - s.n_dense_layers)),
+                "hit_rate": (res["hits_resident"] + res["hits_prefetch"]) / max(1, res["accesses"]),
+                "need_mb_per_step": res["need_experts"] * Be / 1e6 / cfg.decode_steps,
+                "moved_mb_per_step": res["h2d_bytes"] / 1e6 / cfg.decode_steps,
+                "decode_roofline_frac": res["need_experts"] * Be / (h2d * 1e9) / dec_s,
+                "path": "fused decode step + device-side fetch worker" if nb == 1 else "T > 1 layer loop (copy-engine fills, per-row fused attention)"}
+        print(json.dumps(line), flush=True)
+
+
 def spawn_command(n_gpus: int, argv):
     """Command line that runs this script as n_gpus ranks on one node (127.0.0.1 rendezvous, a free port)."""
     import socket
@@ -680,6 +734,7 @@ def main():
                     "this is the configuration ncu can profile: a kernel-serialising profiler cannot run the persistent fetch worker)")
     ap.add_argument("--int4", type=int, default=0, help="routed experts as INT4 group-quantised images (SURVEY N3; wdtype 2)")
     ap.add_argument("--ladder", action="store_true", help="ablation ladder of PAPER.md §7.3 / Fig. 12 (one JSON line per rung)")
+    ap.add_argument("--batch-sweep", action="store_true", help="decode at batch sizes 1-4 (PAPER.md §7.5), one JSON line per batch size")
     ap.add_argument("--goodpred", action="store_true", help="Accuracy / FetchRate / GoodPred of skip vs fitted at strides 1-3 (one JSON line per row)")
     ap.add_argument("--decode", default="random", choices=["random", "greedy"],
                     help="decode ids: seeded random (locality-neutral, default) or greedy argmax")
@@ -705,6 +760,9 @@ def main():
         return
     if args.ladder or args.goodpred:
         run_modes(args)
+        return
+    if args.batch_sweep:
+        run_batch_sweep(args)
         return
     import synth
     over = {}

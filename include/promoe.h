@@ -104,6 +104,9 @@ typedef struct {
                               < 0 = no worker: legal only when nothing is ever fetched (every expert resident) — for runs under
                               a profiler that serialises kernels; a needed fetch then ends in PROMOE_ETIMEOUT.  Physical only */
   void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
+  int32_t max_batch;       /* sequences the handle can hold (each with its own KV cache and position) for batched decode, P:381-413;
+                              0 = 1.  promoe_prefill / promoe_decode work on sequence 0 */
+  int32_t reserved;
 } promoe_opts_t;
 
 /* Device pointers to the always-resident parameters.  Per-layer arrays are HOST arrays of n_layers DEVICE
@@ -182,6 +185,15 @@ PROMOE_API int promoe_load_experts(promoe_t* h, const void* const* host_ptrs, si
 PROMOE_API int promoe_prefill(promoe_t* h, const int32_t* ids_host, int32_t n_tokens, float* logits_out);
 /* Decode one token (caller samples; tests teacher-force).  logits_out as above. */
 PROMOE_API int promoe_decode(promoe_t* h, int32_t token_id, float* logits_out);
+
+/* Batched decode (§7.5: batch sizes 1-4).  The handle holds opts.max_batch independent sequences.
+ * promoe_prefill_seq = promoe_prefill on sequence `seq` (its own KV cache and position).  promoe_decode_batch decodes ONE new
+ * token for each of the n_seq DISTINCT sequences seqs[0..n_seq): the layers run once over the n_seq rows — one gate per layer
+ * (needed experts = the union over the rows), one slot-table step, the stride predictor voting over the rows (G7),
+ * grouped expert FFNs over the permuted rows — while every row attends to its own sequence.  logits_out = HOST ptr to
+ * n_seq * vocab floats (row b = sequence seqs[b]) or NULL.  Traces of the step have T = n_seq rows. */
+PROMOE_API int promoe_prefill_seq(promoe_t* h, int32_t seq, const int32_t* ids_host, int32_t n_tokens, float* logits_out);
+PROMOE_API int promoe_decode_batch(promoe_t* h, int32_t n_seq, const int32_t* seqs, const int32_t* token_ids, float* logits_out);
 
 /* predictor_mode TRACE: lists for the NEXT step call; pred[m*(1+E)] = n, then n expert ids = the list the
  * predictor at MoE layer m would emit for layer m+stride.  Host ptr, copied. */

@@ -26,7 +26,7 @@ EXPORTS = [
     "promoe_prefill", "promoe_decode", "promoe_set_prediction_trace", "promoe_stats", "promoe_get_trace",
     "promoe_reset", "promoe_get_slots", "promoe_op_linear", "promoe_op_route",
     "promoe_op_permute", "promoe_op_expert_ffn", "promoe_op_expert_ffn_static", "promoe_op_expert_ffn_static_max_inter",
-    "promoe_op_attention",
+    "promoe_op_attention", "promoe_prefill_seq", "promoe_decode_batch",
 ]
 BENCH_EXPORTS = ["promoe_bench_h2d", "promoe_bench_kernel_time"]   # include/promoe_bench.h (bench.py only)
 
@@ -43,7 +43,7 @@ class promoe_opts_t(C.Structure):
                 ("predictor_mode", C.c_int32), ("flags", C.c_int32), ("max_inflight", C.c_int32),
                 ("high_group", C.c_int32), ("max_spec_decode", C.c_int32), ("max_spec_prefill", C.c_int32),
                 ("low_cap_chunks", C.c_int32), ("fetch_ctas", C.c_int32),
-                ("compute_stream", C.c_void_p)]
+                ("compute_stream", C.c_void_p), ("max_batch", C.c_int32), ("reserved", C.c_int32)]
 
 
 class promoe_dense_t(C.Structure):
@@ -92,6 +92,8 @@ def lib() -> C.CDLL:
     L.promoe_load_experts.argtypes = [vp, C.POINTER(vp), sz]
     L.promoe_prefill.argtypes = [vp, vp, i32, vp]
     L.promoe_decode.argtypes = [vp, i32, vp]
+    L.promoe_prefill_seq.argtypes = [vp, i32, vp, i32, vp]
+    L.promoe_decode_batch.argtypes = [vp, i32, vp, vp, vp]
     L.promoe_set_prediction_trace.argtypes = [vp, vp, sz]
     L.promoe_stats.argtypes = [vp, C.POINTER(promoe_stats_t)]
     L.promoe_get_trace.argtypes = [vp, C.c_int, C.POINTER(vp), C.POINTER(sz)]
@@ -147,6 +149,19 @@ def promoe_prefill(h, ids: np.ndarray, logits_out: Optional[np.ndarray]) -> None
 
 def promoe_decode(h, token_id: int, logits_out: Optional[np.ndarray]) -> None:
     _check(lib().promoe_decode(h, int(token_id), logits_out.ctypes.data if logits_out is not None else None), h)
+
+
+def promoe_prefill_seq(h, seq: int, ids: np.ndarray, logits_out: Optional[np.ndarray]) -> None:
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    _check(lib().promoe_prefill_seq(h, int(seq), ids.ctypes.data, ids.size, logits_out.ctypes.data if logits_out is not None else None), h)
+
+
+def promoe_decode_batch(h, seqs: np.ndarray, token_ids: np.ndarray, logits_out: Optional[np.ndarray]) -> None:
+    seqs = np.ascontiguousarray(seqs, dtype=np.int32)
+    token_ids = np.ascontiguousarray(token_ids, dtype=np.int32)
+    assert seqs.size == token_ids.size
+    _check(lib().promoe_decode_batch(h, seqs.size, seqs.ctypes.data, token_ids.ctypes.data,
+                                     logits_out.ctypes.data if logits_out is not None else None), h)
 
 
 def promoe_set_prediction_trace(h, pred: np.ndarray) -> None:

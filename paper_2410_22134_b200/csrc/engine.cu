@@ -91,6 +91,9 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   h->max_spec_decode = op->max_spec_decode == 0 ? s.top_k : std::max(0, op->max_spec_decode);
   h->max_spec_prefill = op->max_spec_prefill <= 0 ? 0 : op->max_spec_prefill;
   h->maxT = s.max_seq;
+  h->max_batch = op->max_batch > 0 ? op->max_batch : 1;
+  if (h->max_batch > 8) { delete h; return bad("max_batch must be <= 8"); }
+  h->seq_pos.assign(h->max_batch, 0);
   h->qkv_w = (s.n_q_heads + 2 * s.n_kv_heads) * s.head_dim;
   h->ffn_w = s.n_shared_inter > s.dense_inter ? s.n_shared_inter : s.dense_inter;
   h->nsplit = 16;
@@ -108,9 +111,10 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->act, (size_t)T * k * s.expert_inter)); CK(dalloc(&h->yexp, (size_t)T * k * H));
     if (h->ffn_w) { CK(dalloc(&h->sact, (size_t)T * h->ffn_w)); CK(dalloc(&h->sy, (size_t)T * H)); }
     CK(dalloc(&h->sgate, (size_t)T)); CK(dalloc(&h->attn_ws, (size_t)s.n_q_heads * h->nsplit * (s.head_dim + 2)));
-    CK(dalloc(&h->xf, (size_t)H)); CK(dalloc(&h->logits, (size_t)s.vocab));
-    CK(dalloc(&h->kcache, (size_t)L * s.n_kv_heads * s.max_seq * s.head_dim));
-    CK(dalloc(&h->vcache, (size_t)L * s.n_kv_heads * s.max_seq * s.head_dim));
+    CK(dalloc(&h->xf, (size_t)H)); CK(dalloc(&h->logits, (size_t)s.vocab * h->max_batch));
+    h->kv_seq_elems = (size_t)L * s.n_kv_heads * s.max_seq * s.head_dim;
+    CK(dalloc(&h->kcache, h->kv_seq_elems * h->max_batch));
+    CK(dalloc(&h->vcache, h->kv_seq_elems * h->max_batch));
     CK(dalloc(&h->ids, (size_t)T));
     CK(dalloc(&h->sel, (size_t)Lm * T * k)); CK(dalloc(&h->gates, (size_t)Lm * T * k)); CK(dalloc(&h->margin, (size_t)Lm * T));
     CK(dalloc(&h->z, (size_t)Lm * T * E));
@@ -164,7 +168,7 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(cudaHostAlloc((void**)&h->cmd_host, sizeof(LayerCmd) * Lm, cudaHostAllocMapped));
     memset((void*)h->cmd_host, 0, sizeof(LayerCmd) * Lm);
     CK(cudaHostGetDevicePointer((void**)&h->cmd_dev, (void*)h->cmd_host, 0));
-    CK(cudaHostAlloc((void**)&h->logits_pin, sizeof(float) * (size_t)s.vocab, cudaHostAllocDefault));
+    CK(cudaHostAlloc((void**)&h->logits_pin, sizeof(float) * (size_t)s.vocab * h->max_batch, cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->ids_pin, sizeof(int32_t) * (size_t)T, cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->err_pin, sizeof(int), cudaHostAllocDefault));
     CK(cudaHostAlloc((void**)&h->flagsrc_host, sizeof(uint32_t) * kFlagSrcRing, cudaHostAllocDefault));
@@ -353,6 +357,7 @@ extern "C" int promoe_reset(promoe_t* h) {
   h->st = promoe_stats_t{};
   h->st.registered_host_bytes = reg;
   h->pos = 0;
+  std::fill(h->seq_pos.begin(), h->seq_pos.end(), 0);
   h->last_T = 0;
   return promoe_init_cache_state(h, true);
 }

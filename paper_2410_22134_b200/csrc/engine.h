@@ -135,7 +135,12 @@ struct promoe {
   unsigned long long* src_dev = nullptr;  // [Lm*E] device-visible addresses of the host expert images
   int fetch_ctas = 4;
   bool phys_dirty = false;                // the device path has moved bytes since the host's SlotPhys was last synced
-  int pos = 0;
+  int pos = 0;                            // position of sequence 0 (= seq_pos[0]; kept for the single-sequence calls)
+  int max_batch = 1;
+  std::vector<int> seq_pos;               // [max_batch] tokens held by each sequence
+  size_t kv_seq_elems = 0;                // elements of one sequence's K (or V) cache: L * nkv * max_seq * d
+  // the step being enqueued: which sequence(s) its rows belong to (run_step / run_batch_step set these)
+  int cur_n_seq = 1; int cur_seq[8] = {0}; int cur_pos[8] = {0}; bool cur_batch = false;
   uint32_t step_seq = 0;
   int last_T = 0;
   std::vector<uint8_t> trace_buf;         // host staging for promoe_get_trace

@@ -151,7 +151,8 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   a.x = h->x; a.gain = h->ln1[l]; a.eps = s.rms_eps; a.K = H;
   a.seg[0] = GemvSeg{h->wqkv[l], h->qkv, h->qkv_w, 0}; a.nseg = 1;
   launch_norm_multi_gemv(a, wd, cs);
-  launch_attn_decode_fused(h->qkv, h->cos_t, h->sin_t, h->kcache + (size_t)l * kv_layer, h->vcache + (size_t)l * kv_layer,   // K2
+  const size_t kv_seq = (size_t)h->cur_seq[0] * h->kv_seq_elems;
+  launch_attn_decode_fused(h->qkv, h->cos_t, h->sin_t, h->kcache + kv_seq + (size_t)l * kv_layer, h->vcache + kv_seq + (size_t)l * kv_layer,   // K2
                            h->attn_ws, h->attn, h->attn_cnt, pos0, nq, nkv, d, s.max_seq, h->nsplit, cs);
   launch_gemv(h->attn, h->wo[l], h->x, H, nq * d, wd, LIN_ACC, cs);          // K3
   NormGemvArgs b{};                                                                      // K4
@@ -219,18 +220,35 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
 
 static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fused);
 
-static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_out) {
+// One step.  seqs == nullptr: T tokens of ONE sequence `seq` (prefill, or decode with T = 1).  seqs != nullptr: a batched
+// decode step — row b is the new token of sequence seqs[b] (T = n rows); it takes the T > 1 path of the layer loop
+// with per-row attention, and returns the logits of every row.
+static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_out, int seq = 0, const int32_t* seqs = nullptr) {
   const promoe_shape_t& s = h->s;
   const int H = s.hidden, E = s.n_experts, k = s.top_k, C = h->C, Lm = h->Lm, I = s.expert_inter;
   const int nq = s.n_q_heads, nkv = s.n_kv_heads, d = s.head_dim, wd = h->wdd;
   if (!h->dense_loaded || !h->experts_loaded) { h->err = "step before load_dense / load_experts"; return PROMOE_ESTATE; }
   if (T < 1 || !ids_host) { h->err = "step: no tokens"; return PROMOE_EINVAL; }
-  if (h->pos + T > s.max_seq) { h->err = "step: sequence exceeds max_seq"; return PROMOE_ESTATE; }
+  const bool batch = seqs != nullptr;
+  if (batch) {
+    if (T > h->max_batch) { h->err = "decode_batch: more rows than max_batch"; return PROMOE_EINVAL; }
+    for (int b = 0; b < T; ++b) {
+      if (seqs[b] < 0 || seqs[b] >= h->max_batch) { h->err = "decode_batch: sequence index out of range"; return PROMOE_EINVAL; }
+      for (int c = 0; c < b; ++c) if (seqs[c] == seqs[b]) { h->err = "decode_batch: a sequence appears twice"; return PROMOE_EINVAL; }
+      if (h->seq_pos[seqs[b]] + 1 > s.max_seq) { h->err = "step: sequence exceeds max_seq"; return PROMOE_ESTATE; }
+    }
+  } else {
+    if (seq < 0 || seq >= h->max_batch) { h->err = "step: sequence index out of range"; return PROMOE_EINVAL; }
+    if (h->seq_pos[seq] + T > s.max_seq) { h->err = "step: sequence exceeds max_seq"; return PROMOE_ESTATE; }
+  }
   for (int t = 0; t < T; ++t)
     if (ids_host[t] < 0 || ids_host[t] >= s.vocab) { h->err = "step: token id out of range"; return PROMOE_EINVAL; }
   cudaStream_t cs = h->cs;
   const uint32_t step_seq = ++h->step_seq;
-  const int pos0 = h->pos;
+  h->cur_batch = batch;
+  h->cur_n_seq = batch ? T : 1;
+  for (int b = 0; b < h->cur_n_seq; ++b) { h->cur_seq[b] = batch ? seqs[b] : seq; h->cur_pos[b] = h->seq_pos[h->cur_seq[b]]; }
+  const int pos0 = h->cur_pos[0];
   // residency at step start, for B_need: needed \ resident-at-step-start
   std::fill(h->start_resident.begin(), h->start_resident.end(), 0);
   for (int m = 0; m < Lm; ++m)
@@ -240,7 +258,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     }
   for (auto& v : h->pending_pred) v.clear();
 
-  const bool fused = T == 1 && !(h->o.flags & PROMOE_F_NOFUSE);
+  const bool fused = T == 1 && !batch && !(h->o.flags & PROMOE_F_NOFUSE);
   h->want_done_events = T > 1;
   if (!fused) RC(ce_sync_phys_from_device(h));      // the copy-engine path tracks slots on the host
   if (T > 1) RC(ce_retire(h, true));   // prefill orders compute after fills with events: start from a drained copy stream
@@ -268,13 +286,16 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     launch_embed(h->ids, h->emb, h->x, T, H, wd, cs, worker ? h->alive : nullptr, step_seq, h->err_dev);
     rc_layers = run_layers(h, T, step_seq, pos0, fused);
   }
-  if (rc_layers == PROMOE_OK && e_end == cudaSuccess) {   // ---- last token: final norm + lm_head
-    NormGemvArgs f{};
-    f.x = h->x + (size_t)(T - 1) * H; f.gain = h->final_norm; f.eps = s.rms_eps; f.K = H;
-    f.seg[0] = GemvSeg{h->lm_head, h->logits, s.vocab, 0}; f.nseg = 1;
-    launch_norm_multi_gemv(f, wd, cs);
+  const int n_logit_rows = batch ? T : 1;
+  if (rc_layers == PROMOE_OK && e_end == cudaSuccess) {   // ---- last token (batch: every row): final norm + lm_head
+    for (int b = 0; b < n_logit_rows; ++b) {
+      NormGemvArgs f{};
+      f.x = h->x + (size_t)(batch ? b : T - 1) * H; f.gain = h->final_norm; f.eps = s.rms_eps; f.K = H;
+      f.seg[0] = GemvSeg{h->lm_head, h->logits + (size_t)b * s.vocab, s.vocab, 0}; f.nseg = 1;
+      launch_norm_multi_gemv(f, wd, cs);
+    }
     e_end = cudaEventRecord(h->step_end, cs);
-    if (e_end == cudaSuccess && logits_out) e_end = cudaMemcpyAsync(h->logits_pin, h->logits, (size_t)s.vocab * 4, cudaMemcpyDeviceToHost, cs);
+    if (e_end == cudaSuccess && logits_out) e_end = cudaMemcpyAsync(h->logits_pin, h->logits, (size_t)s.vocab * 4 * n_logit_rows, cudaMemcpyDeviceToHost, cs);
     if (e_end == cudaSuccess) e_end = cudaMemcpyAsync(h->err_pin, h->err_dev, 4, cudaMemcpyDeviceToHost, cs);
   }
   const bool failed = rc_layers != PROMOE_OK || e_end != cudaSuccess;
@@ -309,7 +330,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
   if (e_end != cudaSuccess) { h->err = std::string("step: ") + cudaGetErrorString(e_end); return PROMOE_ECUDA; }
   CKS(cudaStreamSynchronize(cs));
   const int err_host = *h->err_pin;
-  if (logits_out) memcpy(logits_out, h->logits_pin, (size_t)s.vocab * 4);
+  if (logits_out) memcpy(logits_out, h->logits_pin, (size_t)s.vocab * 4 * n_logit_rows);
   float ms = 0.f;
   CKS(cudaEventElapsedTime(&ms, h->step_start, h->step_end));
   if (fused) {     // statistics: logical from the command ring, physical from the worker's counters
@@ -326,7 +347,9 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
   }
   h->st.steps++; h->st.tokens += (uint64_t)T;
   h->st.step_ms += ms; h->st.last_step_ms = ms;
-  h->pos += T;
+  if (batch) for (int b = 0; b < T; ++b) h->seq_pos[seqs[b]] += 1;
+  else h->seq_pos[seq] += T;
+  h->pos = h->seq_pos[0];
   h->last_T = T;
   if (err_host) {
     h->st.timeouts++;
@@ -350,11 +373,21 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     // ---- attention block (A1-A3)
     launch_rmsnorm(h->x, h->ln1[l], h->u1, T, H, s.rms_eps, cs);
     RC(linear(h, h->u1, h->wqkv[l], h->qkv, T, h->qkv_w, H, 0));
-    float* kc = h->kcache + (size_t)l * kv_layer;
-    float* vc = h->vcache + (size_t)l * kv_layer;
-    launch_rope_append(h->qkv, h->cos_t, h->sin_t, kc, vc, T, pos0, nq, nkv, d, s.max_seq, cs);
-    if (T == 1) launch_attn_decode(h->qkv, kc, vc, h->attn, h->attn_ws, pos0 + 1, nq, nkv, d, s.max_seq, h->nsplit, cs);
-    else launch_attn_prefill(h->qkv, kc, vc, h->attn, T, pos0, nq, nkv, d, s.max_seq, cs);
+    if (h->cur_batch) {
+      // batched decode: row b attends to ITS sequence — the fused decode attention (RoPE + append + split attention + merge)
+      // once per row on that sequence's cache, at that sequence's position
+      for (int b = 0; b < T; ++b) {
+        const size_t off = (size_t)h->cur_seq[b] * h->kv_seq_elems + (size_t)l * kv_layer;
+        launch_attn_decode_fused(h->qkv + (size_t)b * h->qkv_w, h->cos_t, h->sin_t, h->kcache + off, h->vcache + off, h->attn_ws,
+                                 h->attn + (size_t)b * nq * d, h->attn_cnt, h->cur_pos[b], nq, nkv, d, s.max_seq, h->nsplit, cs);
+      }
+    } else {
+      float* kc = h->kcache + (size_t)h->cur_seq[0] * h->kv_seq_elems + (size_t)l * kv_layer;
+      float* vc = h->vcache + (size_t)h->cur_seq[0] * h->kv_seq_elems + (size_t)l * kv_layer;
+      launch_rope_append(h->qkv, h->cos_t, h->sin_t, kc, vc, T, pos0, nq, nkv, d, s.max_seq, cs);
+      if (T == 1) launch_attn_decode(h->qkv, kc, vc, h->attn, h->attn_ws, pos0 + 1, nq, nkv, d, s.max_seq, h->nsplit, cs);
+      else launch_attn_prefill(h->qkv, kc, vc, h->attn, T, pos0, nq, nkv, d, s.max_seq, cs);
+    }
     RC(linear(h, h->attn, h->wo[l], h->x, T, H, nq * d, LIN_ACC));
     launch_rmsnorm(h->x, h->ln2[l], h->u, T, H, s.rms_eps, cs);
     const bool tc = use_tc(h, T);
@@ -394,7 +427,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
       plist = h->pred_list + (size_t)m * (1 + E);
     }
     if (T > 1) launch_permute(sel, T, k, E, h->count + (size_t)m * E, offset, perm, inv, cs);   // A8
-    launch_slot_table(h->tbl, m, h->o.stride, T == 1 ? h->max_spec_decode : h->max_spec_prefill, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
+    launch_slot_table(h->tbl, m, h->o.stride, (T == 1 || h->cur_batch) ? h->max_spec_decode : h->max_spec_prefill, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
                       ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb,
                       h->problems, h->n_prob, h->row_of, h->cmd_dev + m, seq,
                       h->trace_precise + (size_t)m * (1 + 5 * E),
@@ -471,4 +504,13 @@ extern "C" int promoe_prefill(promoe_t* h, const int32_t* ids_host, int32_t n_to
 extern "C" int promoe_decode(promoe_t* h, int32_t token_id, float* logits_out) {
   if (!h) return PROMOE_EINVAL;
   return run_step(h, &token_id, 1, logits_out);
+}
+extern "C" int promoe_prefill_seq(promoe_t* h, int32_t seq, const int32_t* ids_host, int32_t n_tokens, float* logits_out) {
+  if (!h) return PROMOE_EINVAL;
+  return run_step(h, ids_host, n_tokens, logits_out, seq);
+}
+extern "C" int promoe_decode_batch(promoe_t* h, int32_t n_seq, const int32_t* seqs, const int32_t* token_ids, float* logits_out) {
+  if (!h || !seqs || !token_ids || n_seq < 1) return PROMOE_EINVAL;
+  if (n_seq == 1) return run_step(h, token_ids, 1, logits_out, seqs[0]);      // one row: the fused decode step of that sequence
+  return run_step(h, token_ids, n_seq, logits_out, 0, seqs);
 }

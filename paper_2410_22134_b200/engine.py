@@ -26,7 +26,7 @@ class ProMoE:
     def __init__(self, weights, cache_slots: int, stride: int = 1, chunk_bytes: int = 0,
                  predictor_mode: int = B.PRED_MLP, flags: int = B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TRACE,
                  max_inflight: int = 0, high_group: int = 0, max_spec_decode: int = 0, max_spec_prefill: int = 0,
-                 low_cap_chunks: int = 0, fetch_ctas: int = 0, device: str = "cuda:0"):
+                 low_cap_chunks: int = 0, fetch_ctas: int = 0, max_batch: int = 1, device: str = "cuda:0"):
         if not torch.cuda.is_available():
             raise RuntimeError("ProMoE needs a CUDA device (there is no CPU fallback)")
         B.lib()
@@ -42,7 +42,8 @@ class ProMoE:
                                predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight, high_group=high_group,
                                max_spec_decode=max_spec_decode, max_spec_prefill=max_spec_prefill,
                                low_cap_chunks=low_cap_chunks, fetch_ctas=fetch_ctas,
-                               compute_stream=None)
+                               compute_stream=None, max_batch=max_batch)
+        self.max_batch = max_batch
         self.h = B.promoe_create(shape_struct(s), opts)
         # dense parameters → device (borrowed by the library; kept alive here)
         self._dev: Dict[str, torch.Tensor] = {k: v.to(self.device).contiguous() for k, v in weights.dense.items()}
@@ -71,6 +72,7 @@ class ProMoE:
         ptrs = [base + (m * s.n_experts + e) * self.expert_bytes for m in range(self.n_moe) for e in range(s.n_experts)]
         B.promoe_load_experts(self.h, ptrs, self.expert_bytes)
         self._logits = np.empty(s.vocab, dtype=np.float32)
+        self._blogits = np.empty((max(1, max_batch), s.vocab), dtype=np.float32)
 
     # ---- steps ----------------------------------------------------------------------------------------------
     def prefill(self, ids, want_logits: bool = True) -> Optional[np.ndarray]:
@@ -81,6 +83,18 @@ class ProMoE:
     def decode(self, token_id: int, want_logits: bool = True) -> Optional[np.ndarray]:
         B.promoe_decode(self.h, int(token_id), self._logits if want_logits else None)
         return self._logits.copy() if want_logits else None
+
+    def prefill_seq(self, seq: int, ids, want_logits: bool = True) -> Optional[np.ndarray]:
+        ids = np.ascontiguousarray(np.asarray(ids, dtype=np.int32))
+        B.promoe_prefill_seq(self.h, seq, ids, self._logits if want_logits else None)
+        return self._logits.copy() if want_logits else None
+
+    def decode_batch(self, seqs, token_ids, want_logits: bool = True) -> Optional[np.ndarray]:
+        """One new token for each sequence in `seqs`; returns logits [len(seqs), vocab]."""
+        n = len(seqs)
+        out = self._blogits[:n]
+        B.promoe_decode_batch(self.h, np.asarray(seqs, dtype=np.int32), np.asarray(token_ids, dtype=np.int32), out if want_logits else None)
+        return out.copy() if want_logits else None
 
     def set_prediction_trace(self, lists: List[Optional[List[int]]]) -> None:
         E = self.s.n_experts

@@ -407,3 +407,65 @@ def test_int4_outputs_independent_of_cache_parameters():
         for a, b in zip(base["logits"], out["logits"]):
             assert np.array_equal(a, b), f"INT4: logits differ bitwise for {kw}"
         assert out["stats"]["misses"] > 0
+
+
+# ---- batched decode (§7.5: batch 1-4) -------------------------------------------------
+@pytest.mark.parametrize("name,nb,tensor", [("c1", 1, 0), ("c1", 2, 0), ("c1", 4, 0), ("c1b", 4, 1), ("c2-mini", 3, 1), ("c3-mini", 4, 1),
+                                            ("c4-mini", 2, 1)])
+def test_batched_decode(name, nb, tensor):
+    """promoe_decode_batch: nb sequences of DIFFERENT lengths, one new token each per step — rows bit-exact in routing and
+    within tolerance in hidden state against the sequences run alone (oracle/batch.py), one slot-table step per layer over
+    the union of the rows' experts (traces bit-exact against O3), predictor votes over the rows, logits of every row."""
+    from paper_2410_22134_b200 import binding as B
+    from synth.configs import mini
+    cfg = mini(name[:-5]) if name.endswith("-mini") else synth.get_config(name)
+    w = synth.make_weights(cfg, predictor="skip")
+    lens = [17, 9, 23, 5][:nb]
+    g = torch.Generator().manual_seed(99)
+    prompts = [torch.randint(0, cfg.shape.vocab, (n,), generator=g).tolist() for n in lens]
+    steps = 6
+    dec = torch.randint(0, cfg.shape.vocab, (steps, nb), generator=g).tolist()
+    flags = B.F_PREEMPT | B.F_REORDER | B.F_TRACE | B.F_WARM | B.F_DEMOTE | (B.F_TENSOR if tensor else 0)
+    from tests.harness import run_parity_batch
+    out = run_parity_batch(cfg, w, prompts, dec, flags=flags, max_spec_decode=1)
+    r, s = out["report"], out["stats"]
+    print(f"[{name} batch {nb}] steps {r.steps} near-ties {r.sel_near_tie}/{r.pred_near_tie} hidden-ratio {r.max_hidden_ratio:.3f} "
+          f"acc {s['accesses']} A {s['hits_resident']} B {s['hits_prefetch']} C {s['misses']}")
+    assert r.steps == nb + steps and r.max_hidden_ratio <= 1.0 and s["timeouts"] == 0
+    assert s["tokens"] == sum(lens) + steps * nb
+
+
+def test_batched_decode_rows_equal_single_sequence_runs_bitwise_in_routing():
+    """GPU vs GPU: the selections of row b of a batched run equal those of sequence b decoded alone (same prompt, same
+    tokens) — batching changes which experts share a step, never what a token computes; and error paths."""
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+    cfg = synth.get_config("c1")
+    w = synth.make_weights(cfg)
+    g = torch.Generator().manual_seed(5)
+    prompts = [torch.randint(0, 1000, (n,), generator=g).tolist() for n in (7, 12, 4)]
+    toks = torch.randint(0, 1000, (4, 3), generator=g).tolist()
+    eng = ProMoE(w, cache_slots=8, max_batch=3)
+    solo = ProMoE(w, cache_slots=8)
+    try:
+        for b, p in enumerate(prompts):
+            eng.prefill_seq(b, p)
+        batch_sel, batch_logits = [], []
+        for row in toks:
+            batch_logits.append(eng.decode_batch([0, 1, 2], row))
+            batch_sel.append(eng.trace(3)["sel"].copy())                 # [Lm, 3, k]
+        for b, p in enumerate(prompts):
+            solo.reset(); solo.prefill(p)
+            for i, row in enumerate(toks):
+                lg = solo.decode(row[b])
+                assert solo.trace(1)["sel"][:, 0].tolist() == batch_sel[i][:, b].tolist()
+                assert np.abs(lg - batch_logits[i][b]).max() <= 1e-3 * max(1.0, np.abs(lg).max())
+        with pytest.raises(B.PromoeError):
+            eng.decode_batch([0, 0], [1, 2])            # a sequence twice
+        with pytest.raises(B.PromoeError):
+            eng.decode_batch([0, 3], [1, 2])            # sequence index out of range
+        with pytest.raises(B.PromoeError):
+            eng.prefill_seq(5, [1, 2])
+        assert eng.decode_batch([2], [7]).shape == (1, 1000)        # one row: the fused step of that sequence
+    finally:
+        eng.close(); solo.close()

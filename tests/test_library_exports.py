@@ -29,6 +29,6 @@ def test_struct_layouts_match_header():
     from paper_2410_22134_b200 import binding as B
     # sizes computed from the header's field lists (all int32/float/uint64/double/pointers, natural alignment)
     assert ctypes.sizeof(B.promoe_shape_t) == 17 * 4 + 2 * 4
-    assert ctypes.sizeof(B.promoe_opts_t) == 56
+    assert ctypes.sizeof(B.promoe_opts_t) == 64
     assert ctypes.sizeof(B.promoe_dense_t) == 15 * 8
     assert ctypes.sizeof(B.promoe_stats_t) == 27 * 8 + 3 * 8 + 8
