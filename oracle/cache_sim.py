@@ -45,6 +45,10 @@ Two switches (readings G16, G17), both off the paper's text:
      stamp 0 at that gate, before the class-C allocations: it is the next victim, so a wrong prediction costs the
      cache one LRU victim (which the next miss would have taken anyway) instead of a most-recently-used slot.
      The paper keeps mispredicted prefetches as ordinary MRU entries.
+  static_slots=S > 0 — the "static" baseline of §7.1: it "caches a fixed set of experts and utilizes two additional
+     expert buffers to load any missing experts".  Slots 0..S-1 of every layer are never victims (with a warm start they hold
+     experts 0..S-1 for good); only the remaining C - S slots — the staging buffers, S = C - 2 for the paper's two — take
+     allocations, by LRU among themselves.  DESIGN.md reading G21.
 """
 from __future__ import annotations
 
@@ -101,9 +105,11 @@ class CacheStats:
 
 class ProMoECacheSim:
     def __init__(self, n_moe_layers: int, n_experts: int, slots_per_layer: int, warm: bool = True,
-                 reorder: bool = True, demote: bool = False):
+                 reorder: bool = True, demote: bool = False, static_slots: int = 0):
         self.L, self.E, self.C = n_moe_layers, n_experts, slots_per_layer
         self.reorder, self.demote = reorder, demote
+        assert 0 <= static_slots < slots_per_layer
+        self.static_slots = static_slots
         self.slot_expert = [[EMPTY] * self.C for _ in range(self.L)]
         self.stamp = [[0] * self.C for _ in range(self.L)]
         self.origin = [[RESIDENT] * self.C for _ in range(self.L)]
@@ -129,11 +135,11 @@ class ProMoECacheSim:
 
     def _victim(self, m: int, protected: set) -> int:
         row = self.slot_expert[m]
-        for s in range(self.C):
+        for s in range(self.static_slots, self.C):
             if row[s] == EMPTY:
                 return s
         best, best_stamp = -1, None
-        for s in range(self.C):
+        for s in range(self.static_slots, self.C):
             if row[s] in protected:
                 continue
             if best_stamp is None or self.stamp[m][s] < best_stamp:

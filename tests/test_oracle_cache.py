@@ -340,3 +340,45 @@ def test_demotion_never_changes_outputs_of_a_reactive_run():
         ra, rb = a.run_step(needed, [None, None], 1), b.run_step(needed, [None, None], 1)
         assert [x[0].as_tuples() for x in ra] == [x[0].as_tuples() for x in rb]
     assert a.slot_expert == b.slot_expert and a.stamp == b.stamp
+
+
+# ---- static_slots: the "static" baseline (a fixed set + two staging buffers) -------------------------------------
+def test_static_cache_keeps_its_fixed_set_and_cycles_two_buffers():
+    """C = 6, 4 static slots (experts 0..3 for good) + 2 staging buffers.  Misses alternate between the two buffers by LRU;
+    an expert of the fixed set always hits; nothing ever lands in slots 0..3."""
+    rng = random.Random(4)
+    L, E, C, k = 2, 16, 6, 3
+    sim = ProMoECacheSim(L, E, C, warm=True, static_slots=C - 2)
+    staging = [TextbookLRU(2, [4, 5]) for _ in range(L)]          # the warm start put experts 4, 5 into the two buffers
+    for step in range(200):
+        needed = [sorted(rng.sample(range(E), k)) for _ in range(L)]
+        out = sim.run_step(needed, [None] * L, stride=1)
+        for m in range(L):
+            rec = out[m][0]
+            assert sim.slot_expert[m][:4] == [0, 1, 2, 3]
+            hits = [e for e in needed[m] if e < 4 or e in staging[m].d]
+            misses = [e for e in needed[m] if e >= 4 and e not in staging[m].d]
+            assert rec.expert == hits + misses and [c for c in rec.cls] == [CLASS_A] * len(hits) + [CLASS_C] * len(misses)
+            assert all(s >= 4 for s, c in zip(rec.slot, rec.cls) if c == CLASS_C)
+            for e in hits + misses:
+                if e >= 4:
+                    staging[m].access(e)
+            # a buffer that holds a needed expert is pinned until that expert has been computed (G2): more buffer users
+            # (hits in a buffer + misses) than buffers → the last miss waits for a finish (dep)
+            if len([e for e in hits if e >= 4]) + len(misses) <= 2:
+                assert all(d == -1 for d in rec.dep)
+            else:
+                assert rec.dep[-1] >= 0
+            assert sorted(sim.slot_expert[m][4:]) == sorted(staging[m].d)
+    # against the LRU cache of the same size on the same stream: the static cache never evicts its fixed set
+    assert sim.stats.hits + sim.stats.misses == sim.stats.accesses
+
+
+def test_static_cache_three_misses_wait_for_a_buffer():
+    """Hand-worked: buffers hold 4 (older), 5.  Gate needs {1, 7, 8, 9}: 1 hits; 7 -> buffer of 4, 8 -> buffer of 5, 9 has no
+    unpinned buffer left (7 and 8 are needed and not yet computed) and waits for launch position 0 ... the first finish
+    that frees a BUFFER is position 1 (expert 7): dep = 1."""
+    sim = ProMoECacheSim(1, 16, 6, warm=True, static_slots=4)
+    sim.begin_step()
+    rec = sim.push_precise(0, [1, 7, 8, 9])
+    assert rec.as_tuples() == [(1, CLASS_A, 1, -1, -1), (7, CLASS_C, 4, 4, -1), (8, CLASS_C, 5, 5, -1), (9, CLASS_C, 4, 7, 1)]
