@@ -615,7 +615,8 @@ def run_modes(args):
     P, R, D, U, TN, W = B.F_PREEMPT, B.F_REORDER, B.F_DEMOTE, B.F_UNCHUNKED, (B.F_TENSOR if args.tensor else 0), B.F_WARM
     if args.ladder:
         st = base.stride
-        rows = [("base: LRU, ID order, no prefetch", "none", st, W | TN, 0),
+        rows = [("static cache (fixed set + top_k staging buffers, P:317)", "static", st, W | TN, 0),
+                ("base: LRU, ID order, no prefetch", "none", st, W | TN, 0),
                 ("+prefetch (un-chunked, no preemption)", "skip", st, W | TN | U, args.max_spec_decode),
                 ("+chunked", "skip", st, W | TN, args.max_spec_decode),
                 ("+early preemption", "skip", st, W | TN | P, args.max_spec_decode),
@@ -630,8 +631,9 @@ def run_modes(args):
         w, rep = weights_for(stride, "fitted" if kind == "fitted" else "skip")
         cfg = dataclasses.replace(base, stride=stride)
         eng = ProMoE(w, cache_slots=cfg.cache_slots, stride=stride, chunk_bytes=args.chunk_kb << 10,
-                     predictor_mode=B.PRED_NONE if kind == "none" else B.PRED_MLP, flags=flags, max_inflight=args.inflight,
-                     max_spec_decode=ms, max_spec_prefill=args.max_spec_prefill, fetch_ctas=args.fetch_ctas)
+                     predictor_mode=B.PRED_NONE if kind in ("none", "static") else B.PRED_MLP, flags=flags, max_inflight=args.inflight,
+                     max_spec_decode=ms, max_spec_prefill=args.max_spec_prefill, fetch_ctas=args.fetch_ctas,
+                     static_slots=cfg.slots_per_layer - s.top_k if kind == "static" else 0)
         run_request(eng, cfg, prompt, decode_ids, False)
         r = run_request(eng, cfg, prompt, decode_ids, False)
         eng.close()

@@ -106,7 +106,10 @@ typedef struct {
   void* compute_stream;    /* cudaStream_t owned by the caller (torch); NULL = library creates one */
   int32_t max_batch;       /* sequences the handle can hold (each with its own KV cache and position) for batched decode, P:381-413;
                               0 = 1.  promoe_prefill / promoe_decode work on sequence 0 */
-  int32_t reserved;
+  int32_t static_slots;    /* > 0: the "static" baseline of P:317 — slots [0, static_slots) of every layer never take an allocation
+                              (with PROMOE_F_WARM they hold experts 0..static_slots-1 for good); the remaining slots are the staging
+                              buffers (the paper uses two; here at least top_k must remain, so that one decode step never recycles a buffer:
+                              static_slots <= slots per layer - top_k).  0 = an ordinary LRU cache */
 } promoe_opts_t;
 
 /* Device pointers to the always-resident parameters.  Per-layer arrays are HOST arrays of n_layers DEVICE

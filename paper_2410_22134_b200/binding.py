@@ -43,7 +43,7 @@ class promoe_opts_t(C.Structure):
                 ("predictor_mode", C.c_int32), ("flags", C.c_int32), ("max_inflight", C.c_int32),
                 ("high_group", C.c_int32), ("max_spec_decode", C.c_int32), ("max_spec_prefill", C.c_int32),
                 ("low_cap_chunks", C.c_int32), ("fetch_ctas", C.c_int32),
-                ("compute_stream", C.c_void_p), ("max_batch", C.c_int32), ("reserved", C.c_int32)]
+                ("compute_stream", C.c_void_p), ("max_batch", C.c_int32), ("static_slots", C.c_int32)]
 
 
 class promoe_dense_t(C.Structure):

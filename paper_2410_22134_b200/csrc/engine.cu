@@ -94,6 +94,9 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
   h->max_batch = op->max_batch > 0 ? op->max_batch : 1;
   if (h->max_batch > 8) { delete h; return bad("max_batch must be <= 8"); }
   h->seq_pos.assign(h->max_batch, 0);
+  h->static_slots = op->static_slots > 0 ? op->static_slots : 0;
+  // the fused decode step runs the k experts of a layer side by side: a staging buffer must never be recycled inside one step
+  if (h->static_slots > C - s.top_k) { delete h; return bad("static_slots must leave at least top_k staging slots per layer"); }
   h->qkv_w = (s.n_q_heads + 2 * s.n_kv_heads) * s.head_dim;
   h->ffn_w = s.n_shared_inter > s.dense_inter ? s.n_shared_inter : s.dense_inter;
   h->nsplit = 16;

@@ -137,6 +137,7 @@ struct promoe {
   bool phys_dirty = false;                // the device path has moved bytes since the host's SlotPhys was last synced
   int pos = 0;                            // position of sequence 0 (= seq_pos[0]; kept for the single-sequence calls)
   int max_batch = 1;
+  int static_slots = 0;                   // static-cache baseline (G21): slots [0, static_slots) of every layer never take an allocation
   std::vector<int> seq_pos;               // [max_batch] tokens held by each sequence
   size_t kv_seq_elems = 0;                // elements of one sequence's K (or V) cache: L * nkv * max_seq * d
   // the step being enqueued: which sequence(s) its rows belong to (run_step / run_batch_step set these)

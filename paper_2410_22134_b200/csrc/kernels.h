@@ -87,7 +87,8 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* j_of_problem, LayerCmd* cmd,
                        uint32_t seq, int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st,
-                       const RouteFuse* fuse = nullptr, LayerCmd* cmd_dev2 = nullptr, const LayerCmd* cmd_prev = nullptr);
+                       const RouteFuse* fuse = nullptr, LayerCmd* cmd_dev2 = nullptr, const LayerCmd* cmd_prev = nullptr,
+                       int* err = nullptr);
 
 // A7 (fused decode): the device-side prefetch worker (kernels_fetch.cu).
 struct FetchArgs {

@@ -11,12 +11,13 @@ constexpr int kMaxE = 256;
 struct SlotView {
   int32_t* slot_expert; int32_t* expert_slot; unsigned long long* stamp; uint32_t* gen; uint8_t* origin;
   unsigned long long* clock; int C, E;   // all pointers: SHARED-memory copies of one layer's rows (+ a local clock)
+  int s0;                                // first slot that may take an allocation (static-cache baseline G21: slots < s0 are fixed)
   __device__ void touch(int s) { stamp[s] = ++(*clock); }
   // Alg. 1 l.4 cache.replace_with: lowest EMPTY slot, else smallest stamp among unprotected slots; -1 if none.
   __device__ int victim(const uint8_t* prot) const {
-    for (int s = 0; s < C; ++s) if (slot_expert[s] < 0) return s;
+    for (int s = s0; s < C; ++s) if (slot_expert[s] < 0) return s;
     int best = -1; unsigned long long bs = 0;
-    for (int s = 0; s < C; ++s) {
+    for (int s = s0; s < C; ++s) {
       if (prot[slot_expert[s]]) continue;
       if (best < 0 || stamp[s] < bs) { best = s; bs = stamp[s]; }
     }
@@ -75,7 +76,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
                                                          int32_t* n_problems, int32_t* row_of, LayerCmd* cmd,
                                                          uint32_t seq, int32_t* trace_precise,
                                                          int32_t* trace_pred, RouteFuse rf, LayerCmd* cmd2, int mode,
-                                                         const LayerCmd* cmd_prev) {
+                                                         const LayerCmd* cmd_prev, int* err) {
   __shared__ uint8_t needed[kMaxE];
   __shared__ uint8_t prot[kMaxE];
   __shared__ int16_t order[kMaxE];
@@ -115,9 +116,9 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   // so nothing in the stream order says its table rows have been written back: wait for its `seq_done`.
   if (cmd_prev) {
     __shared__ int prev_ok;
-    if (threadIdx.x == 0) prev_ok = wait_gate_word((const unsigned*)&cmd_prev->seq_done, seq - 1u, nullptr);
+    if (threadIdx.x == 0) prev_ok = wait_gate_word((const unsigned*)&cmd_prev->seq_done, seq - 1u, err);
     __syncthreads();
-    (void)prev_ok;      // a time-out here surfaces through the expert kernels' own flag waits
+    (void)prev_ok;      // a time-out raises the error word: the step ends in PROMOE_ETIMEOUT
   }
   for (int i = threadIdx.x; i < C; i += blockDim.x) {
     t_se[0][i] = tbl.slot_expert[(size_t)m * C + i]; t_stamp[0][i] = tbl.stamp[(size_t)m * C + i];
@@ -141,7 +142,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   if (threadIdx.x == 0 && !(mode & 1)) {
     // G16: ID-order baseline (Fig. 12 "Base"): ascending id, classified at its turn, plain LRU victim over ALL
     // slots — a needed expert may lose its slot before its turn and is then fetched again (§5.3)
-    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
+    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E, mode >> 8};
     int n = 0;
     for (int e = 0; e < E; ++e) if (needed[e]) order[n++] = e;
     if (trace_precise) trace_precise[0] = n;
@@ -167,7 +168,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     n_built = n;        // hand-over to the common tail below
   }
   if (threadIdx.x == 0 && (mode & 1)) {
-    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
+    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E, mode >> 8};
     // classes A (cached) → B (being prefetched) → C (not begun), ascending id inside
     int n = 0;
     if (T == 1) {      // decode: only the k selected experts — sort them by id instead of scanning all E
@@ -215,7 +216,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     n_built = n;
   }
   if (threadIdx.x == 0) {
-    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E};
+    SlotView v{t_se[0], t_es[0], t_stamp[0], t_gen[0], t_org[0], &t_clock, C, E, mode >> 8};
     const int n = n_built;
     for (int sl = 0; sl < C; ++sl) v.origin[sl] = 0;
     // problem table + decode row map + trace
@@ -247,16 +248,30 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
   // first publication (posted writes to mapped pinned memory; every writer fences its own stores; seq last)
   // (fused decode: a second copy in device memory feeds the fetch kernel, kernels_fetch.cu — the host copy is only read
   // after the step, for the statistics)
-  for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) { cmd->need[i] = rec[i]; if (cmd2) cmd2->need[i] = rec[i]; }
-  if (threadIdx.x == 0) { cmd->n_needed = s_n; if (cmd2) cmd2->n_needed = s_n; }
-  __threadfence_system();
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    if (cmd2) { volatile uint32_t* s2 = &cmd2->seq; *s2 = seq; }
-    volatile uint32_t* sq = &cmd->seq; *sq = seq;
+  if (cmd2) {
+    // fused decode: the readers of this publication are on the DEVICE (fetch worker, K6's gate word) — device ring first, behind
+    // a gpu-scope fence; the mapped host copy (read after the step, for the statistics) follows off the critical path, where the
+    // system-scope fence and the posted PCIe writes cost nothing
+    for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd2->need[i] = rec[i];
+    if (threadIdx.x == 0) cmd2->n_needed = s_n;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(&cmd2->seq), "r"(seq) : "memory");
+    pdl_done();      // the expert kernels may take their places while the host copy and the predictor half run
+    for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
+    if (threadIdx.x == 0) cmd->n_needed = s_n;
+    __threadfence_system();
+    __syncthreads();
+    if (threadIdx.x == 0) { volatile uint32_t* sq = &cmd->seq; *sq = seq; }
+  } else {
+    for (int i = threadIdx.x; i < 7 * s_n; i += blockDim.x) cmd->need[i] = rec[i];
+    if (threadIdx.x == 0) cmd->n_needed = s_n;
+    __threadfence_system();
+    __syncthreads();
+    if (threadIdx.x == 0) { volatile uint32_t* sq = &cmd->seq; *sq = seq; }
   }
 
-  pdl_done();      // the expert kernels may take their places while the predictor half runs
+  if (!cmd2) pdl_done();      // the expert kernels may take their places while the predictor half runs
   // ================= phase 2: predictor W2 + list (fused decode only) + PushPredicted(m + stride) =================
   if (rf.zraw && rf.pred_out) {
     const int nwarps = blockDim.x >> 5;
@@ -318,7 +333,7 @@ __global__ void __launch_bounds__(1024) slot_table_kernel(SlotTable tbl, int m, 
     // predictions; no victim → skip; at most max_spec allocations (knob G3; most confident first)
     int np = 0;
     if (have_t) {
-      SlotView t{t_se[1], t_es[1], t_stamp[1], t_gen[1], t_org[1], &t_clock, C, E};
+      SlotView t{t_se[1], t_es[1], t_stamp[1], t_gen[1], t_org[1], &t_clock, C, E, mode >> 8};
       np = s_pred[0];
       int allocs = 0;
       for (int i = 0; i < np; ++i) {
@@ -377,14 +392,15 @@ void launch_slot_table(SlotTable tbl, int m, int stride, int max_spec, const int
                        const uint32_t* flag_base, int flags_per_slot, int H, int inter, int wbytes,
                        FfnProblem* problems, int32_t* n_problems, int32_t* row_of, LayerCmd* cmd, uint32_t seq,
                        int32_t* trace_precise, int32_t* trace_pred, cudaStream_t st, const RouteFuse* rf, LayerCmd* cmd_dev2,
-                       const LayerCmd* cmd_prev) {
+                       const LayerCmd* cmd_prev, int* err) {
   ++g_launches;
-  const int mode = reorder;     // bit 0: reordered inference / 0 = ID order (G16); bit 1: demote mispredictions (G17)
+  const int mode = reorder;     // bit 0: reordered inference / 0 = ID order (G16); bit 1: demote mispredictions (G17);
+                                // bits 8+: number of fixed slots of the static-cache baseline (G21)
   RouteFuse f{};
   if (rf) f = *rf;
   launch_pdl(slot_table_kernel, dim3(1), dim3((rf && T == 1) ? 1024 : 256), 0, st, tbl, m, stride, max_spec, sel, T, k, offset, pred_list,
              slot_base, slot_bytes, flag_base, flags_per_slot, H, inter, wbytes, problems, n_problems, row_of, cmd, seq,
-             trace_precise, trace_pred, f, cmd_dev2, mode, cmd_prev);
+             trace_precise, trace_pred, f, cmd_dev2, mode, cmd_prev, err);
 }
 
 // Load every kernel of this file NOW.  CUDA loads kernels lazily, on their first launch, and that load waits for every

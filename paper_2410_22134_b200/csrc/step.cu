@@ -194,10 +194,10 @@ static int decode_layer_fused(promoe_t* h, int l, uint32_t step_seq, int pos0) {
   rf.p1 = h->p1; rf.pred_w2 = mlp ? h->pred_w2[l] : nullptr; rf.ph = s.pred_hidden; rf.wdtype = wd;
   rf.pred_out = mlp ? plist : nullptr; rf.k = k; rf.cap = C;
   launch_slot_table(h->tbl, m, h->o.stride, h->max_spec_decode, sel, 1, k, nullptr, plist,
-                    ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb, h->problems,
+                    ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0) | (h->static_slots << 8), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb, h->problems,
                     h->n_prob, h->row_of, h->cmd_dev + m, seq, h->trace_precise + (size_t)m * (1 + 5 * E),
                     (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs, &rf, h->cmd_fetch + m,
-                    m > 0 ? h->cmd_fetch + (m - 1) : nullptr);
+                    m > 0 ? h->cmd_fetch + (m - 1) : nullptr, h->err_dev);
   // A7 runs beside this stream: the fetch worker (kernels_fetch.cu, resident since the start of the step) sees the
   // command K5 publishes in device memory and pulls the missing chunks over the link; the flag-gated kernels K6/K7 are
   // enqueued right away and wait (ld.acquire.sys on the chunk flags, __nanosleep between polls) for exactly the bytes
@@ -428,7 +428,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     }
     if (T > 1) launch_permute(sel, T, k, E, h->count + (size_t)m * E, offset, perm, inv, cs);   // A8
     launch_slot_table(h->tbl, m, h->o.stride, (T == 1 || h->cur_batch) ? h->max_spec_decode : h->max_spec_prefill, sel, T, k, T > 1 ? offset : nullptr, plist,     // A6
-                      ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb,
+                      ((h->o.flags & PROMOE_F_REORDER) ? 1 : 0) | ((h->o.flags & PROMOE_F_DEMOTE) ? 2 : 0) | (h->static_slots << 8), h->slots, h->Be, h->flags, h->n_chunks, H, I, h->q4 ? 0 : h->wb,
                       h->problems, h->n_prob, h->row_of, h->cmd_dev + m, seq,
                       h->trace_precise + (size_t)m * (1 + 5 * E),
                       (m + h->o.stride < Lm) ? h->trace_pred + (size_t)(m + h->o.stride) * (1 + 4 * E) : nullptr, cs);

@@ -26,7 +26,7 @@ class ProMoE:
     def __init__(self, weights, cache_slots: int, stride: int = 1, chunk_bytes: int = 0,
                  predictor_mode: int = B.PRED_MLP, flags: int = B.F_PREEMPT | B.F_REORDER | B.F_WARM | B.F_TRACE,
                  max_inflight: int = 0, high_group: int = 0, max_spec_decode: int = 0, max_spec_prefill: int = 0,
-                 low_cap_chunks: int = 0, fetch_ctas: int = 0, max_batch: int = 1, device: str = "cuda:0"):
+                 low_cap_chunks: int = 0, fetch_ctas: int = 0, max_batch: int = 1, static_slots: int = 0, device: str = "cuda:0"):
         if not torch.cuda.is_available():
             raise RuntimeError("ProMoE needs a CUDA device (there is no CPU fallback)")
         B.lib()
@@ -42,7 +42,7 @@ class ProMoE:
                                predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight, high_group=high_group,
                                max_spec_decode=max_spec_decode, max_spec_prefill=max_spec_prefill,
                                low_cap_chunks=low_cap_chunks, fetch_ctas=fetch_ctas,
-                               compute_stream=None, max_batch=max_batch)
+                               compute_stream=None, max_batch=max_batch, static_slots=static_slots)
         self.max_batch = max_batch
         self.h = B.promoe_create(shape_struct(s), opts)
         # dense parameters → device (borrowed by the library; kept alive here)

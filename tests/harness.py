@@ -17,7 +17,7 @@ from oracle.forward import OracleModel
 def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional[int] = None,
                stride: Optional[int] = None, chunk_bytes: int = 0, predictor_mode: int = 1, flags: Optional[int] = None,
                decode_ids: Optional[List[int]] = None, max_inflight: int = 0, warm: bool = True, high_group: int = 0,
-               max_spec_decode: int = 0, max_spec_prefill: int = 0) -> Dict:
+               max_spec_decode: int = 0, max_spec_prefill: int = 0, static_slots: int = 0) -> Dict:
     from paper_2410_22134_b200 import binding as B
     from paper_2410_22134_b200.engine import ProMoE
 
@@ -30,11 +30,11 @@ def run_parity(cfg, weights, prompt, decode_steps: int, *, cache_slots: Optional
     C = cache_slots // n_moe
     eng = ProMoE(weights, cache_slots=cache_slots, stride=stride, chunk_bytes=chunk_bytes,
                  predictor_mode=predictor_mode, flags=flags, max_inflight=max_inflight, high_group=high_group,
-                 max_spec_decode=max_spec_decode, max_spec_prefill=max_spec_prefill)
+                 max_spec_decode=max_spec_decode, max_spec_prefill=max_spec_prefill, static_slots=static_slots)
     use_pred = predictor_mode == B.PRED_MLP
     ora = OracleModel(weights, stride=stride, slots_per_layer=C, use_predictor=use_pred)
     sim = ProMoECacheSim(n_moe, s.n_experts, C, warm=bool(flags & B.F_WARM), reorder=bool(flags & B.F_REORDER),
-                         demote=bool(flags & B.F_DEMOTE))
+                         demote=bool(flags & B.F_DEMOTE), static_slots=static_slots)
     rep = ParityReport()
     # library defaults (include/promoe.h): decode top_k allocations per push, prefill none
     ms_dec = s.top_k if max_spec_decode == 0 else max(0, max_spec_decode)

@@ -120,6 +120,31 @@ def test_ablation_modes(name, T, mode):
     assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
 
 
+@pytest.mark.parametrize("name,T,reorder", [("c1", 32, 1), ("c1b", 32, 0), ("c2-mini", 64, 1), ("c4-mini", 40, 1)])
+def test_static_cache_baseline(name, T, reorder):
+    """The "static" baseline of P:317 (a fixed set of experts + staging buffers, no prefetch): slots [0, C - top_k) never take an
+    allocation, the top_k staging slots cycle by LRU; traces bit-exact against O3 with static_slots (c4-mini: C = top_k = 2,
+    so static_slots = 0 is the only legal value there — the create call must reject 1)."""
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+    from synth.configs import mini
+    cfg = mini(name[:-5]) if name.endswith("-mini") else synth.get_config(name)
+    w = synth.make_weights(cfg, predictor="skip")
+    C, k = cfg.slots_per_layer, cfg.shape.top_k
+    if C - k < 1:
+        with pytest.raises(B.PromoeError):
+            ProMoE(w, cache_slots=cfg.cache_slots, static_slots=1)
+        return
+    flags = B.F_PREEMPT | B.F_TRACE | B.F_WARM | (B.F_REORDER if reorder else 0) | (B.F_TENSOR if cfg.shape.wdtype == 1 else 0)
+    ids = synth.make_decode_ids(cfg, 8).tolist()
+    out = run_parity(cfg, w, synth.make_prompt(cfg, T), 8, flags=flags, predictor_mode=B.PRED_NONE, decode_ids=ids,
+                     static_slots=C - k)
+    _report(f"{name}/static", out)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+    for m in range(cfg.shape.n_moe_layers):
+        assert out["sim"].slot_expert[m][:C - k] == list(range(C - k))          # the fixed set never moved
+
+
 def test_fitted_predictor_parity():
     """the stride predictor fitted offline on the model's own traces (PROMOE_TRACE_U +
     selections, 9:1 split) is at least as accurate as its `skip` start point on held-out tokens, and the step that runs
