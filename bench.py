@@ -259,6 +259,40 @@ def run_request(eng, cfg, prompt, decode_ids, greedy: bool, record=None, inject=
             "pre": {k: d(s0, s1, k) for k in s0}, "dec": {k: d(s1, s2, k) for k in s1}}
 
 
+def also_config(args, name, h2d_gbs, flags, local):
+    """One request of another BASELINE.json config (after one warm-up request): ProMoE with the run's settings and the reactive
+    cache, decode / prefill tokens/s and the H2D roofline fractions (every bf16 config is H2D-bound)."""
+    import synth
+    from paper_2410_22134_b200 import binding as B
+    from paper_2410_22134_b200.engine import ProMoE
+    cfg = synth.get_config(name)
+    s = cfg.shape
+    Be = expert_image_bytes(s)
+    w = synth.make_weights(cfg, predictor="skip")
+    prompt = synth.make_prompt(cfg).tolist()
+    decode_ids = synth.make_decode_ids(cfg).tolist()
+    out = {"workload": f"{name}: prompt {cfg.prompt_len} + {cfg.decode_steps} decode, cache {cfg.slots_per_layer}/{s.n_experts} per layer, stride {cfg.stride}"}
+    need_reactive = None
+    for label, pm in (("reactive_no_prefetch", B.PRED_NONE), ("promoe", B.PRED_MLP)):
+        eng = ProMoE(w, cache_slots=cfg.cache_slots, stride=cfg.stride, chunk_bytes=args.chunk_kb << 10, predictor_mode=pm, flags=flags,
+                     max_inflight=args.inflight, max_spec_decode=args.max_spec_decode, max_spec_prefill=args.max_spec_prefill,
+                     fetch_ctas=args.fetch_ctas, device=f"cuda:{local}")
+        run_request(eng, cfg, prompt, decode_ids, False)
+        r = run_request(eng, cfg, prompt, decode_ids, False)
+        eng.close()
+        dec_s, pre_s = r["decode_ms"] / 1e3, r["prefill_ms"] / 1e3
+        need_d, need_p = r["dec"]["need_experts"] * Be, r["pre"]["need_experts"] * Be
+        if pm == B.PRED_NONE:
+            need_reactive = (need_d, need_p)
+        out[label] = {"decode_tokens_per_s": cfg.decode_steps / dec_s, "prefill_tokens_per_s": cfg.prompt_len / pre_s,
+                      "decode_roofline_frac": need_d / (h2d_gbs * 1e9) / dec_s, "prefill_roofline_frac": need_p / (h2d_gbs * 1e9) / pre_s,
+                      "decode_frac_vs_reactive_need": need_reactive[0] / (h2d_gbs * 1e9) / dec_s,
+                      "prefill_frac_vs_reactive_need": need_reactive[1] / (h2d_gbs * 1e9) / pre_s,
+                      "hit_rate": (r["dec"]["hits_resident"] + r["dec"]["hits_prefetch"]) / max(1, r["dec"]["accesses"]),
+                      "predictor_accuracy": r["dec"]["predicted_correct"] / max(1, r["dec"]["predicted"])}
+    return out
+
+
 def replica_weights(cfg, pred_kind, local, world, dist, tag=None):
     """Weights of one replica.  world > 1: the replicas of a node share ONE host copy of the routed experts — a /dev/shm
     mapping drawn by local rank 0 and mapped by the others (every rank's library registers it with cudaHostRegister);
@@ -467,6 +501,14 @@ def run_ours(args, cfg, rank, world, dist):
         cpu = {"value": o["decode_tok_s"], "unit": "tokens/s", "cores": o["cores"], "kind": "oracle",
                "prefill_tokens_per_s": o["prefill_tok_s"], "seconds": o["seconds"],
                "sample": ref_sample_text(cfg, rpl, rds)}
+    also = None
+    if rank == 0 and world == 1 and args.also and args.also != cfg.name:
+        # a second BASELINE.json config in the same run (one request each for ProMoE and the reactive cache), so that the round's
+        # bench record carries more than the headline workload; not part of `value`
+        del weights
+        import gc
+        gc.collect(); torch.cuda.empty_cache()
+        also = {args.also: also_config(args, args.also, h2d_gbs, flags, local)}
     if rank != 0:
         return
     line = {"metric": METRIC, "value": g_dec_tok / g_dec_s, "unit": "tokens/s", "n_gpus": world, "steps": K,
@@ -484,7 +526,7 @@ def run_ours(args, cfg, rank, world, dist):
             "step_roofline": {"h2d_gbs_measured": h2d_gbs, "hbm_gbs": peaks["hbm_gbs"], "bf16_tflops": peaks["bf16_tflops_sustained"],
                               "peaks": peaks["source"], "decode": roof_dec, "prefill": roof_pre},
             "cache": {"decode": cs_dec, "prefill": cs_pre, "hidden_copy_fraction_decode": hidden},
-            "all_resident": allhit, "variants": variants, "predictor_fit": fit_report, "cpu_baseline": cpu}
+            "all_resident": allhit, "variants": variants, "predictor_fit": fit_report, "also": also, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
 
 
@@ -734,6 +776,7 @@ def main():
     ap.add_argument("--fit-steps", type=int, default=240, help="--predictor fitted: optimiser steps per layer")
     ap.add_argument("--cache-all", type=int, default=0, help="every routed expert resident (compute-only step; with --fetch-ctas -1 "
                     "this is the configuration ncu can profile: a kernel-serialising profiler cannot run the persistent fetch worker)")
+    ap.add_argument("--also", default="c3", help="a second config measured briefly in the same run and reported under `also` ('' = none)")
     ap.add_argument("--int4", type=int, default=0, help="routed experts as INT4 group-quantised images (SURVEY N3; wdtype 2)")
     ap.add_argument("--ladder", action="store_true", help="ablation ladder of PAPER.md §7.3 / Fig. 12 (one JSON line per rung)")
     ap.add_argument("--batch-sweep", action="store_true", help="decode at batch sizes 1-4 (PAPER.md §7.5), one JSON line per batch size")

@@ -89,8 +89,9 @@ typedef struct {
                               high_group chunks per copy operation */
   int32_t predictor_mode;
   int32_t flags;
-  int32_t max_inflight;    /* prefill / unfused decode (copy engines): LOW chunks kept in flight on the copy stream (P:191 bounded
-                              preemption delay); 0 = default 2.  The fused decode step has one LOW chunk per fetch CTA in flight */
+  int32_t max_inflight;    /* LOW (predicted) chunks in flight (P:191 bounded preemption delay).  Prefill / unfused decode (copy
+                              engines): chunks kept on the copy stream, 0 = default 2.  Fused decode (device-side worker): the number
+                              of fetch CTAs that copy LOW chunks, one chunk each at a time, 0 = default 1 */
   int32_t high_group;      /* chunks per HIGH (precise) copy operation; 0 = the whole remaining fill in ONE copy (measured
                               fastest); ready flags are written behind every operation */
   int32_t max_spec_decode; /* experts of one PushPredicted that may ALLOCATE a slot in a decode step (listed order = most

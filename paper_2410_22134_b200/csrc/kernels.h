@@ -104,6 +104,7 @@ struct FetchArgs {
   uint32_t* alive;             // ← step once the worker runs
   uint32_t step;
   int Lm, C, E, n_chunks, preempt, unchunked, low_cap;
+  int low_ctas;                // CTAs that may copy LOW chunks (one chunk each at a time): bounds what a gate finds in its way
 };
 constexpr int kFetchCounters = 16;
 cudaError_t launch_fetch(const FetchArgs& a, int ctas, cudaStream_t st);

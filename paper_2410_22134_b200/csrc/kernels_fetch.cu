@@ -275,9 +275,10 @@ struct Scout {
         if (!busy_low && poll((const uint32_t*)&a.cmd[m].seq, a.step * 4096u + (uint32_t)m + 1u)) { on_gate(); phase = 1; continue; }
       }
       // LOW work (also while waiting for the predicted part, and — without early preemption — after the last gate).
-      // Only CTA 0 copies LOW chunks: one chunk in progress and one waiting bound what a gate can find in its way
-      // (P:191), whatever the number of workers; the other CTAs keep the list only to know what HIGH must skip.
-      while (head < tail && blockIdx.x == 0) {
+      // Only the first low_ctas CTAs copy LOW chunks (default 1): one chunk in progress and one waiting per such CTA bound what
+      // a gate can find in its way, whatever the number of workers; the other CTAs keep the list only to know what HIGH
+      // must skip.  Several LOW CTAs share a job through the claim words (no chunk is taken twice).
+      while (head < tail && (int)blockIdx.x < a.low_ctas) {
         const LowJob j = jobs[head];
         const size_t so = (size_t)j.layer * a.C + j.slot;
         int cur = j.cursor, got = 0;

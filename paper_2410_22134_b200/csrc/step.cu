@@ -272,6 +272,7 @@ static int run_step(promoe_t* h, const int32_t* ids_host, int T, float* logits_o
     fa.flags = h->flags; fa.claims = h->claims; fa.complete = h->complete; fa.ctr = h->fetch_ctr; fa.err = h->err_dev;
     fa.alive = h->alive; fa.step = step_seq; fa.Lm = Lm; fa.C = C; fa.E = E; fa.n_chunks = h->n_chunks;
     fa.preempt = (h->o.flags & PROMOE_F_PREEMPT) != 0; fa.unchunked = h->unchunked; fa.low_cap = h->low_cap;
+    fa.low_ctas = h->unchunked ? 1 : std::max(1, std::min(h->o.max_inflight > 0 ? h->o.max_inflight : 1, h->fetch_ctas));
     // nothing may be queued BEHIND the worker on its stream, and no copy may be submitted behind a kernel that waits:
     // a pending operation behind a spinning kernel blocks later copy submissions (profiles/r02_spin_probe.md)
     CKS(launch_fetch(fa, h->fetch_ctas, h->fs));
