@@ -777,6 +777,7 @@ def main():
     ap.add_argument("--cache-all", type=int, default=0, help="every routed expert resident (compute-only step; with --fetch-ctas -1 "
                     "this is the configuration ncu can profile: a kernel-serialising profiler cannot run the persistent fetch worker)")
     ap.add_argument("--also", default="c3", help="a second config measured briefly in the same run and reported under `also` ('' = none)")
+    ap.add_argument("--stride", type=int, default=0, help="predictor stride (0 = the config's: c2 2, c3 / c4 1)")
     ap.add_argument("--int4", type=int, default=0, help="routed experts as INT4 group-quantised images (SURVEY N3; wdtype 2)")
     ap.add_argument("--ladder", action="store_true", help="ablation ladder of PAPER.md §7.3 / Fig. 12 (one JSON line per rung)")
     ap.add_argument("--batch-sweep", action="store_true", help="decode at batch sizes 1-4 (PAPER.md §7.5), one JSON line per batch size")
@@ -817,6 +818,8 @@ def main():
         over["decode_steps"] = args.decode_steps
     if args.int4:
         over["shape_overrides"] = {"wdtype": 2}
+    if args.stride:
+        over["stride"] = args.stride
     cfg = synth.get_config(args.config, **over)
     if args.cache_all:
         import dataclasses
