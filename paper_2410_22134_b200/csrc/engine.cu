@@ -121,6 +121,7 @@ extern "C" int promoe_create(const promoe_shape_t* sp, const promoe_opts_t* op, 
     CK(dalloc(&h->ids, (size_t)T));
     CK(dalloc(&h->sel, (size_t)Lm * T * k)); CK(dalloc(&h->gates, (size_t)Lm * T * k)); CK(dalloc(&h->margin, (size_t)Lm * T));
     CK(dalloc(&h->z, (size_t)Lm * T * E));
+    CK(dalloc(&h->votes_ws, (size_t)257)); CK(cudaMemset(h->votes_ws, 0, 257 * 4));
     if (op->flags & PROMOE_F_TRACE_U) CK(dalloc(&h->trace_u, (size_t)Lm * T * H));
     CK(dalloc(&h->count, (size_t)Lm * E)); CK(dalloc(&h->offset, (size_t)Lm * (E + 1)));
     CK(dalloc(&h->perm, (size_t)Lm * T * k)); CK(dalloc(&h->inv, (size_t)Lm * T * k));
@@ -202,7 +203,7 @@ extern "C" void promoe_destroy(promoe_t* h) {
                   h->count, h->offset, h->perm, h->inv, h->gates, h->margin, h->z, h->pred_list, h->trace_precise,
                   h->trace_pred, h->row_of, h->n_prob, h->problems, h->shared_prob, h->err_dev, h->attn_cnt, h->slots, h->flags,
                   h->tbl.slot_expert, h->tbl.expert_slot, h->tbl.stamp, h->tbl.gen, h->tbl.origin, h->tbl.clock,
-                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch, h->trace_u, h->q4_stage, h->problems_deq, h->q4_stage_bf, h->q4_gu};
+                  h->claims, h->complete, h->alive, h->fetch_ctr, h->src_dev, h->cmd_fetch, h->trace_u, h->q4_stage, h->problems_deq, h->q4_stage_bf, h->q4_gu, h->votes_ws};
   for (void* b : bufs) if (b) cudaFree(b);
   if (h->xsA) cudaFree(h->xsA);
   if (h->xsG) cudaFree(h->xsG);
@@ -290,6 +291,7 @@ int promoe_init_cache_state(promoe_t* h, bool copy_warm) {
   CK(cudaMemset(h->tbl.origin, 0, (size_t)Lm * C));
   CK(cudaMemset(h->flags, 0, (size_t)Lm * C * h->n_chunks * 4));
   CK(cudaMemset(h->err_dev, 0, 4));
+  CK(cudaMemset(h->votes_ws, 0, 257 * 4));
   CK(cudaMemset(h->attn_cnt, 0, (size_t)h->s.n_q_heads * 4));
   h->mirror = se;
   h->low.clear();

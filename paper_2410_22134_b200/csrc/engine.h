@@ -76,6 +76,7 @@ struct promoe {
   // per-MoE-layer routing / permutation buffers (double as traces)
   int32_t *sel = nullptr, *count = nullptr, *offset = nullptr, *perm = nullptr, *inv = nullptr;
   float *gates = nullptr, *margin = nullptr, *z = nullptr;
+  int32_t* votes_ws = nullptr;            // [257] zeroed: vote histogram + arrival counter of the multi-CTA predictor list kernel
   float* trace_u = nullptr;               // [Lm, maxT, H] with PROMOE_F_TRACE_U, else nullptr
   int32_t *pred_list = nullptr, *trace_precise = nullptr, *trace_pred = nullptr, *row_of = nullptr,
           *n_prob = nullptr;

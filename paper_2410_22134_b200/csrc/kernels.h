@@ -44,7 +44,7 @@ void launch_topk_gate(const float* z, const float* bias, int T, int E, int k, fl
                       float* gates, float* margin, cudaStream_t st);
 // A5 predictor list: per-token top-k of scores p [T,E]; T==1: the top-k list; T>1: votes -> top-cap (G7).
 // out list: pred[0] = n, pred[1..n] = experts.
-void launch_pred_list(const float* p, int T, int E, int k, int cap, int32_t* pred, cudaStream_t st);
+void launch_pred_list(const float* p, int T, int E, int k, int cap, int32_t* pred, cudaStream_t st, int32_t* ws = nullptr);
 
 // A8 permutation: histogram -> exclusive scan -> stable scatter (single CTA, atomics-free).
 void launch_permute(const int32_t* sel, int T, int k, int E, int32_t* count, int32_t* offset, int32_t* perm,

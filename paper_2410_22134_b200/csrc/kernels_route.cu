@@ -52,16 +52,20 @@ void launch_topk_gate(const float* z, const float* bias, int T, int E, int k, fl
 // A5 predictor list.  One CTA.  T == 1: the top-k list of p.  T > 1 (reading G7): per-token top-k →
 // vote histogram (shared-memory integer atomics: order-independent, hence deterministic) → experts by votes
 // descending, ties → lower id → the first min(#voted, cap).
+// grid of CTAs (8 warps, one token per warp and turn); T > 1: every CTA adds its vote histogram into ws[0..E) (integer
+// atomics: the sums do not depend on the order) and the LAST CTA to arrive (ws[256]) ranks the experts and leaves ws zeroed
+// for the next call.  (One CTA for all tokens took 100 us at T = 512 — on the pre-gate critical path of every prefill layer.)
 template <int NPL>
 __global__ void __launch_bounds__(256) pred_list_kernel(const float* __restrict__ p, int T, int E, int k, int cap,
-                                                        int32_t* __restrict__ pred) {
+                                                        int32_t* __restrict__ pred, int32_t* __restrict__ ws) {
   __shared__ int votes[32 * NPL];
   __shared__ int s_sel[8][kMaxK];
   __shared__ float s_val[8][kMaxK];
+  __shared__ int s_last;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (int e = threadIdx.x; e < 32 * NPL; e += 256) votes[e] = 0;
   __syncthreads();
-  for (int t = w; t < T; t += 8) {
+  for (int t = blockIdx.x * 8 + w; t < T; t += gridDim.x * 8) {
     float v[NPL];
 #pragma unroll
     for (int q = 0; q < NPL; ++q) {
@@ -81,6 +85,19 @@ __global__ void __launch_bounds__(256) pred_list_kernel(const float* __restrict_
   }
   if (T == 1) return;
   __syncthreads();
+  if (gridDim.x > 1) {
+    for (int e = threadIdx.x; e < E; e += 256) if (votes[e]) atomicAdd(&ws[e], votes[e]);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&ws[256], 1) == (int)gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int e = threadIdx.x; e < 32 * NPL; e += 256) votes[e] = e < E ? __ldcg(&ws[e]) : 0;
+    __syncthreads();
+    for (int e = threadIdx.x; e < E; e += 256) ws[e] = 0;      // leave the workspace zeroed for the next call
+    if (threadIdx.x == 0) ws[256] = 0;
+  }
   // rank of expert e among voted experts by (votes desc, id asc)
   int nvoted = 0;
   for (int e = 0; e < E; ++e) nvoted += votes[e] > 0;
@@ -93,104 +110,81 @@ __global__ void __launch_bounds__(256) pred_list_kernel(const float* __restrict_
   }
   if (threadIdx.x == 0) pred[0] = min(nvoted, cap);
 }
-void launch_pred_list(const float* p, int T, int E, int k, int cap, int32_t* pred, cudaStream_t st) {
+void launch_pred_list(const float* p, int T, int E, int k, int cap, int32_t* pred, cudaStream_t st, int32_t* ws) {
   ++g_launches;
-  if (E <= 32) pred_list_kernel<1><<<1, 256, 0, st>>>(p, T, E, k, cap, pred);
-  else if (E <= 64) pred_list_kernel<2><<<1, 256, 0, st>>>(p, T, E, k, cap, pred);
-  else if (E <= 128) pred_list_kernel<4><<<1, 256, 0, st>>>(p, T, E, k, cap, pred);
-  else pred_list_kernel<8><<<1, 256, 0, st>>>(p, T, E, k, cap, pred);
+  const int blocks = (ws && T > 8) ? min(64, (T + 7) / 8) : 1;      // ws: 257 zeroed int32 (votes + arrival counter)
+  if (E <= 32) pred_list_kernel<1><<<blocks, 256, 0, st>>>(p, T, E, k, cap, pred, ws);
+  else if (E <= 64) pred_list_kernel<2><<<blocks, 256, 0, st>>>(p, T, E, k, cap, pred, ws);
+  else if (E <= 128) pred_list_kernel<4><<<blocks, 256, 0, st>>>(p, T, E, k, cap, pred, ws);
+  else pred_list_kernel<8><<<blocks, 256, 0, st>>>(p, T, E, k, cap, pred, ws);
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// A8 permutation, single CTA of 1024 threads, no atomics.  Thread i owns the contiguous pair range
-// [i*per, (i+1)*per) of the flattened (t, j) list, so "token-ascending inside a group" is preserved:
-//   pass 1: per-thread histogram in shared memory cnt[thread][e]  (E <= 256 → processed in expert slabs)
-//   pass 2: for each expert, exclusive scan over threads (warp shuffles + one cross-warp step)
-//   pass 3: scatter.
-// To bound shared memory the experts are processed in slabs of 8; T*k <= 16384.
-constexpr int PT = 1024, SLAB = 8;
+// A8 permutation: stable counting sort of the flattened (t, j) pairs by expert — one CTA of 32 warps, no atomics.
+// Warp w owns the contiguous pair range [w*per, (w+1)*per) and walks it 32 pairs at a time; inside a chunk
+// `__match_any_sync` groups the lanes that hold the same expert, so a pair's rank among the chunk's pairs of its expert is
+// a popcount and one leader lane per expert updates the warp's own counter row — "token-ascending inside a group" holds
+// because ranges, chunks and lanes are all in pair order.
+//   pass 1: per-warp histograms cnt[w][e];  scan: base[w][e] = Σ_{w' < w} cnt[w'][e], count[e], offset[e];
+//   pass 2: pos = offset[e] + base[w][e] + rank in chunk, then base[w][e] += pairs of e in the chunk.
+// Three block-wide barriers in all (the first version made 16 slab passes: 54 us at T·k = 2048, on the pre-gate critical path).
+constexpr int PT = 1024, PW = PT / 32;
 __global__ void __launch_bounds__(PT) permute_kernel(const int32_t* __restrict__ sel, int n, int E,
                                                      int32_t* __restrict__ count, int32_t* __restrict__ offset,
                                                      int32_t* __restrict__ perm, int32_t* __restrict__ inv) {
-  __shared__ int warp_tot[SLAB][32];
-  __shared__ int s_count[256];
+  __shared__ int cnt[PW][256];
   __shared__ int s_offset[257];
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  const int per = (n + PT - 1) / PT;
-  const int b = min(n, tid * per), e_ = min(n, b + per);
-  // global histogram first (needed for offsets): per-thread partial counts, slab by slab
-  for (int e0 = 0; e0 < E; e0 += SLAB) {
-    int c[SLAB];
-#pragma unroll
-    for (int s = 0; s < SLAB; ++s) c[s] = 0;
-    for (int i = b; i < e_; ++i) {
-      const int d = sel[i] - e0;
-#pragma unroll
-      for (int s = 0; s < SLAB; ++s) c[s] += (d == s);
-    }
-#pragma unroll
-    for (int s = 0; s < SLAB; ++s) {
-      int tot = c[s];
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-      if (lane == 0) warp_tot[s][w] = tot;
-    }
-    __syncthreads();
-    if (tid < SLAB && e0 + tid < E) {
-      int tot = 0;
-      for (int i = 0; i < 32; ++i) tot += warp_tot[tid][i];
-      s_count[e0 + tid] = tot;
-    }
-    __syncthreads();
-  }
-  if (tid == 0) {
-    int acc = 0;
-    for (int e = 0; e < E; ++e) { s_offset[e] = acc; acc += s_count[e]; }
-    s_offset[E] = acc;
+  const int per = ((n + PW - 1) / PW + 31) & ~31;          // pairs per warp, a multiple of 32
+  const int b = min(n, w * per), e_ = min(n, b + per);
+  const unsigned lt = (1u << lane) - 1u;
+  for (int e = lane; e < E; e += 32) cnt[w][e] = 0;
+  __syncwarp();
+  for (int i0 = b; i0 < e_; i0 += 32) {
+    const int i = i0 + lane;
+    const bool act = i < e_;
+    const int ex = act ? sel[i] : -1 - lane;                  // inactive lanes: distinct keys that match nobody
+    const unsigned m = __match_any_sync(0xffffffffu, ex);
+    if (act && (m & lt) == 0) cnt[w][ex] += __popc(m);        // leader = lowest lane of the group
+    __syncwarp();
   }
   __syncthreads();
-  for (int e = tid; e < E; e += PT) count[e] = s_count[e];
+  for (int e = tid; e < E; e += PT) {                         // exclusive scan over the warps, per expert
+    int acc = 0;
+    for (int q = 0; q < PW; ++q) { const int c = cnt[q][e]; cnt[q][e] = acc; acc += c; }
+    count[e] = acc;
+    s_offset[e + 1] = acc;                                    // totals, turned into offsets below
+  }
+  __syncthreads();
+  if (w == 0) {                                               // exclusive scan over the experts (E <= 256: 8 per lane)
+    int loc[8], tot = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { const int e = lane * 8 + q; loc[q] = e < E ? s_offset[e + 1] : 0; tot += loc[q]; }
+    int incl = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int up = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += up; }
+    int run = incl - tot;
+    if (lane == 0) s_offset[0] = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { const int e = lane * 8 + q; run += loc[q]; if (e < E) s_offset[e + 1] = run; }
+  }
+  __syncthreads();
   for (int e = tid; e <= E; e += PT) offset[e] = s_offset[e];
-  // scatter, slab by slab: exclusive prefix of this thread's count over lower threads
-  for (int e0 = 0; e0 < E; e0 += SLAB) {
-    int c[SLAB], pre[SLAB];
-#pragma unroll
-    for (int s = 0; s < SLAB; ++s) c[s] = 0;
-    for (int i = b; i < e_; ++i) {
-      const int d = sel[i] - e0;
-#pragma unroll
-      for (int s = 0; s < SLAB; ++s) c[s] += (d == s);
+  for (int i0 = b; i0 < e_; i0 += 32) {
+    const int i = i0 + lane;
+    const bool act = i < e_;
+    const int ex = act ? sel[i] : -1 - lane;
+    const unsigned m = __match_any_sync(0xffffffffu, ex);
+    int basev = 0;
+    if (act) basev = cnt[w][ex];
+    __syncwarp();
+    if (act) {
+      const int pos = s_offset[ex] + basev + __popc(m & lt);
+      perm[pos] = i;
+      inv[i] = pos;
+      if ((m & lt) == 0) cnt[w][ex] = basev + __popc(m);
     }
-#pragma unroll
-    for (int s = 0; s < SLAB; ++s) {
-      int incl = c[s];
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int up = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += up;
-      }
-      pre[s] = incl - c[s];
-      if (lane == 31) warp_tot[s][w] = incl;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int s = 0; s < SLAB; ++s) {
-      int base = 0;
-      for (int i = 0; i < w; ++i) base += warp_tot[s][i];
-      pre[s] += base;
-    }
-    for (int i = b; i < e_; ++i) {
-      const int ex = sel[i], d = ex - e0;
-      if (d >= 0 && d < SLAB) {
-        int pos = 0;
-#pragma unroll
-        for (int s = 0; s < SLAB; ++s)
-          if (d == s) { pos = s_offset[ex] + pre[s]; pre[s]++; }
-        perm[pos] = i;
-        inv[i] = pos;
-      }
-    }
-    __syncthreads();
+    __syncwarp();
   }
 }
 void launch_permute(const int32_t* sel, int T, int k, int E, int32_t* count, int32_t* offset, int32_t* perm,

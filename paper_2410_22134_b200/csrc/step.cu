@@ -423,7 +423,7 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
         if (!tc_launch(h->tc, g, cs, &h->err)) return PROMOE_ECUDA;
       } else launch_gemm_simt(h->p1, h->pred_w2[l], h->p2, T, E, s.pred_hidden, wd, 0, cs);
       plist = h->pred_list + (size_t)m * (1 + E);
-      launch_pred_list(h->p2, T, E, k, C, plist, cs);
+      launch_pred_list(h->p2, T, E, k, C, plist, cs, h->votes_ws);
     } else if (h->o.predictor_mode == PROMOE_PRED_TRACE) {
       plist = h->pred_list + (size_t)m * (1 + E);
     }
