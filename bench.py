@@ -407,6 +407,9 @@ def run_ours(args, cfg, rank, world, dist):
         a = {k: sum(r[key][k] for r in reqs) for k in reqs[0][key]}
         acc = max(1, a["accesses"])
         return {"hit_rate": (a["hits_resident"] + a["hits_prefetch"]) / acc, "hit_rate_resident": a["hits_resident"] / acc,
+                # byte-accurate: class A / B accesses whose whole image had landed when the gate was processed (a logical hit on a
+                # partially fetched image still owes bytes: `owed_bytes_per_access`)
+                "hit_rate_landed": a["hits_landed"] / acc, "owed_bytes_per_access": a["owed_bytes_at_gate"] / acc,
                 "miss_rate": a["misses"] / acc,
                 "predictor_accuracy": a["predicted_correct"] / max(1, a["predicted"]),
                 "fetch_rate": a["fetched_at_gate"] / max(1, a["fetched_at_gate_of"]),

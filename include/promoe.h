@@ -70,8 +70,10 @@ typedef struct {
                                 LRU victim over all slots — a needed expert may be evicted before its turn (G16) */
 #define PROMOE_F_WARM 4      /* warm start: experts 0..C-1 resident in every layer (G4) */
 #define PROMOE_F_TRACE 8     /* record routing / permutation / cache traces for promoe_get_trace */
-#define PROMOE_F_NOFUSE 32  /* decode with the unfused per-op kernels (19 launches per layer) instead of the fused 7 */
-#define PROMOE_F_TENSOR 16   /* prefill GEMMs on tcgen05 tensor cores (bf16 weights only); else SIMT fp32 */
+#define PROMOE_F_NOFUSE 32   /* decode with the unfused per-op kernels and copy-engine fills (19 launches per layer, host in the layer
+                                loop) instead of the fused step on the device-side fetch worker */
+#define PROMOE_F_TENSOR 16   /* prefill GEMMs on tcgen05 tensor cores (bf16 weights; INT4 experts through exact bf16 hi/lo staging
+                                images); else SIMT fp32 */
 #define PROMOE_F_DEMOTE 128  /* a predicted (PRED) slot whose expert its gate did not select gets the oldest LRU stamp at that gate: a
                                 misprediction costs one LRU victim instead of a most-recently-used slot (G17; not in the
                                 paper, which keeps mispredicted prefetches as ordinary cache entries) */

@@ -494,3 +494,25 @@ def test_batched_decode_rows_equal_single_sequence_runs_bitwise_in_routing():
         assert eng.decode_batch([2], [7]).shape == (1, 1000)        # one row: the fused step of that sequence
     finally:
         eng.close(); solo.close()
+
+
+def test_batched_decode_int4_static_and_id_order_combinations():
+    """Cross-products the single-feature tests do not reach: batched decode with INT4 experts; the static cache in ID order
+    with INT4 experts; batched decode on a reactive ID-order cache."""
+    from paper_2410_22134_b200 import binding as B
+    from synth.configs import mini
+    from tests.harness import run_parity_batch
+    cfg = _q4(mini("c2"))
+    w = synth.make_weights(cfg, predictor="skip")
+    g = torch.Generator().manual_seed(7)
+    prompts = [torch.randint(0, cfg.shape.vocab, (n,), generator=g).tolist() for n in (11, 19)]
+    dec = torch.randint(0, cfg.shape.vocab, (4, 2), generator=g).tolist()
+    base = B.F_PREEMPT | B.F_TRACE | B.F_WARM | B.F_TENSOR
+    out = run_parity_batch(cfg, w, prompts, dec, flags=base | B.F_REORDER | B.F_DEMOTE, max_spec_decode=1)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+    out = run_parity_batch(cfg, w, prompts, dec, flags=base, predictor_mode=B.PRED_NONE)          # reactive, ID order
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
+    C, k = cfg.slots_per_layer, cfg.shape.top_k
+    ids = synth.make_decode_ids(cfg, 6).tolist()
+    out = run_parity(cfg, w, synth.make_prompt(cfg, 48), 6, flags=base, predictor_mode=B.PRED_NONE, decode_ids=ids, static_slots=C - k)
+    assert out["report"].max_hidden_ratio <= 1.0 and out["stats"]["timeouts"] == 0
