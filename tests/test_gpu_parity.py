@@ -219,9 +219,9 @@ def test_mini_configs(name, tensor):
     assert out["report"].max_hidden_ratio <= 1.0
 
 
-@pytest.mark.parametrize("name", ["c2", "c3", pytest.param("c4", marks=pytest.mark.skipif(
-    not __import__("os").environ.get("PROMOE_TEST_C4"), reason="90 GB of pinned host memory and minutes of oracle time: "
-    "set PROMOE_TEST_C4=1 (run once per round, result recorded in DESIGN.md)"))])
+# c4 at full size needs 90 GB of pinned host memory and minutes of oracle time: it joins the list only with PROMOE_TEST_C4=1 (run
+# once per round; this round's log: profiles/r02_c4_full_parity.txt).  c4-mini (full-size experts, |needed| > C) is always in the suite.
+@pytest.mark.parametrize("name", ["c2", "c3"] + (["c4"] if __import__("os").environ.get("PROMOE_TEST_C4") else []))
 def test_full_size_configs(name):
     """BASELINE.json configs[1], configs[2] at FULL size (all layers, real vocab, 25-30 GB of routed experts in pinned
     host memory) in the launch configuration bench.py times (tcgen05 prefill, fused decode, default chunking): a
