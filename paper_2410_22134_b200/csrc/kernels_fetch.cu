@@ -196,7 +196,13 @@ struct Scout {
     // after its own fetch (`complete` is only set by a scan that finds every flag raised): with the records taken in launch
     // order A → B → C those scans stood between the gate and the first byte of the missing expert (measured: 9-20 us from
     // the gate word to the first claim; 0.5 us to seeing the word).
-    if (lane == 0) {
+    if (n_needed <= 32) {        // decode: one parallel load of the classes, ranks by ballot
+      const int cl_ = lane < n_needed ? __ldcg((const int32_t*)cmd->need + 7 * lane + 1) : 0;
+      const unsigned need_m = __ballot_sync(0xffffffffu, lane < n_needed && cl_ != 0);
+      const unsigned a_m = __ballot_sync(0xffffffffu, lane < n_needed && cl_ == 0);
+      const unsigned lt_ = (1u << lane) - 1u;
+      if (lane < n_needed) hi_order[cl_ != 0 ? __popc(need_m & lt_) : __popc(need_m) + __popc(a_m & lt_)] = lane;
+    } else if (lane == 0) {
       int n = 0;
       for (int i = 0; i < n_needed; ++i) if (__ldcg((const int32_t*)cmd->need + 7 * i + 1) != 0) hi_order[n++] = i;
       for (int i = 0; i < n_needed; ++i) if (__ldcg((const int32_t*)cmd->need + 7 * i + 1) == 0) hi_order[n++] = i;
@@ -233,17 +239,22 @@ struct Scout {
     const LayerCmd* cmd = a.cmd + m;
     while (hi_rec < n_needed) {
       const int32_t* r = (const int32_t*)cmd->need + 7 * hi_order[hi_rec];
-      const int e = __ldcg(r), slot = __ldcg(r + 2);
+      const int e = __ldcg(r), cls_r = __ldcg(r + 1), slot = __ldcg(r + 2);
       const uint32_t gen = (uint32_t)__ldcg(r + 5);
       const size_t so = (size_t)m * a.C + slot;
       uint32_t* fl = a.flags + so * a.n_chunks;
       uint32_t* cl = a.claims + so * a.n_chunks;
-      if (!hi_scanned && hi_pass == 0 && hi_c0 == 0 && ld_acquire_gpu(a.complete + so) == gen) { ++hi_rec; continue; }
+      if (cls_r != 2 && !hi_scanned && hi_pass == 0 && hi_c0 == 0 && ld_acquire_gpu(a.complete + so) == gen) { ++hi_rec; continue; }
       while (hi_pass < 2) {
         while (hi_c0 < a.n_chunks) {
           if (!hi_scanned) {
-            int pend;
-            hi_mask = scan(fl, cl, gen, hi_c0, a.n_chunks, &pend);
+            int pend = 1;
+            // class C, own chunks: the slot's generation was made at this gate, so no flag can show it yet and nobody but
+            // this CTA goes for these chunks in pass 0 — no need to read 32 flags and 32 claims before the first claim
+            if (cls_r == 2 && hi_pass == 0 && gridDim.x > 1) {
+              const int left = a.n_chunks - hi_c0;
+              hi_mask = left >= 32 ? 0xffffffffu : ((1u << left) - 1u);
+            } else hi_mask = scan(fl, cl, gen, hi_c0, a.n_chunks, &pend);
             if (pend) hi_all = 0;
             if (hi_pass == 0 && gridDim.x > 1) {          // own chunks first
               unsigned own = 0;
