@@ -462,8 +462,9 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     } else {
       if (tc) launch_split_rows(h->u, perm, k, T * k, H, h->xsG, h->xsG_half, cs);   // gathered rows, permuted order
       // batches: [all class A] [all class B] then the class C experts as their fills land in copy order — one by one for bf16
-      // images (311 us of copy per expert against ≈ 30 us of compute), in groups of 8 for INT4 images, whose 6 launches per expert
-      // (dequantise, two [gate|up] passes, SwiGLU, two down passes) would otherwise out-last the 80 us copy of the next image
+      // images (311 us of copy per expert against ≈ 30 us of compute), in groups of up to 8 for INT4 images, whose 6 launches per
+      // expert (dequantise, two [gate|up] passes, SwiGLU, two down passes: ≈ 120 us of 22-CTA launches, profiles/r02_int4.md)
+      // out-last the 80 us copy of the next image
       const int c_group = h->q4 ? 8 : 1;
       int i = 0;
       size_t dnext = 0;
@@ -475,8 +476,11 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
         // copies start after 8 experts instead of after all of them (the link idled for the whole class-A batch: 0.3 ms per
         // layer with bf16 images, 0.75 ms with INT4 images and their dequantisation pass)
         if (cls != 2) while (j < n && cmd.need[7 * j + 1] == cls && (deferred.empty() || j - i < 8)) ++j;
-        else if (cmd.need[7 * i + 4] < 0)
-          while (j < n && j - i < c_group && cmd.need[7 * j + 1] == 2 && cmd.need[7 * j + 4] < 0) ++j;
+        else   // class C: experts whose fill has been issued (no slot dependency, or one the loop below has already released:
+               // `deferred` is in launch order, so those are the entries before `dnext`); a fill that is still held back
+               // waits for an event recorded BEHIND this batch and must not be waited for inside it
+          while (j < n && j - i < c_group && cmd.need[7 * j + 1] == 2 &&
+                 (cmd.need[7 * j + 4] < 0 || (dnext > 0 && j <= deferred[dnext - 1]))) ++j;
         int max_rows = 0;
         for (int q = i; q < j; ++q) {
           max_rows = std::max(max_rows, (int)cmd.need[7 * q + 6]);
