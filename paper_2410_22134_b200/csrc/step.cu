@@ -462,10 +462,11 @@ static int run_layers(promoe_t* h, int T, uint32_t step_seq, int pos0, bool fuse
     } else {
       if (tc) launch_split_rows(h->u, perm, k, T * k, H, h->xsG, h->xsG_half, cs);   // gathered rows, permuted order
       // batches: [all class A] [all class B] then the class C experts as their fills land in copy order — one by one for bf16
-      // images (311 us of copy per expert against ≈ 30 us of compute), in groups of up to 8 for INT4 images, whose 6 launches per
+      // images (311 us of copy per expert against ≈ 30 us of compute), in groups of up to 3 for INT4 images, whose 6 launches per
       // expert (dequantise, two [gate|up] passes, SwiGLU, two down passes: ≈ 120 us of 22-CTA launches, profiles/r02_int4.md)
-      // out-last the 80 us copy of the next image
-      const int c_group = h->q4 ? 8 : 1;
+      // out-last the 80 us copy of the next image; measured on c2 / c3: 2: 6231 / 8033 tok/s, 3: 6290 / 8235, 4: 6282 / 8152,
+      // 8: 6184 / 7861, 16: 5919 / 7426 (a larger group waits longer for its last image and leaves a longer tail)
+      const int c_group = h->q4 ? 3 : 1;
       int i = 0;
       size_t dnext = 0;
       while (i < n) {
